@@ -1,0 +1,150 @@
+/* dedisp_b200.h — C ABI of the B200-native direct incoherent dedispersion library.
+ *
+ * What every call computes (§2.1.1 eq 2.1-2.3; constant eq 1.14,
+ * PAPER.md:425; BASELINE.json north_star):
+ *
+ *     D[b][d][t] = sum_{c=0}^{nchans-1} X[b][c][ t + s(d,c) ]
+ *     s(d,c)     = floor( 4148.808 * DM_d * (f_c^-2 - fch1^-2) / tsamp + 0.5 )   (double)
+ *     f_c        = fch1 + c*foff   [MHz],   tsamp [s],   foff <= 0  (channel 0 = top of band
+ *                                                                      = reference, s(d,0)=0)
+ *
+ * Layouts ("stored in channel order, with time changing the fastest";
+ * PAPER.md:1202 the buffer holds nsamp + maxshift spectra; PAPER.md:956 the output is
+ * the (DM, t) plane; PAPER.md:1131 beams are [beam][chan][time]):
+ *     X : [nbeams][nchans][>= nsamp + maxshift]   time fastest, uint8 or float32
+ *     D : [nbeams][ndm][nsamp]                    time fastest, int32  or float32
+ * `nsamp` is always the number of OUTPUT samples per DM trial; input rows must hold
+ * nsamp + maxshift samples, maxshift = max_d s(d, nchans-1) (reading R7).
+ * uint8 input is accumulated in int32 and the result is exact; float32 input is
+ * accumulated in float32 in a fixed channel order that depends only on the plan
+ * (never on the tile position), so batch, streaming and one-shot results are bit-identical.
+ *
+ * Every step runs in hand-written sm_100a CUDA kernels; there is NO CPU fallback:
+ * without a usable sm_100 device the compute calls return DD_ERR_UNSUPPORTED / DD_ERR_CUDA.
+ *
+ * Conventions
+ *   - "DEVICE" pointers are CUDA device memory owned by the caller; "HOST" pointers are
+ *     ordinary (pageable or pinned) host memory owned by the caller.  The library owns only
+ *     what it allocates inside dd_plan / dd_stream.  X and D must not overlap.
+ *   - All functions return int (0 = DD_OK, <0 = error) unless stated otherwise; they never
+ *     throw, exit or print.  dd_last_error() gives a thread-local detail string.
+ *   - dd_execute / dd_stream_push enqueue work on `cuda_stream` (a cudaStream_t passed as
+ *     void*, NULL = legacy default stream) and return WITHOUT synchronising.  The
+ *     nine-argument dd_dedisperse_* calls and the *_host calls synchronise before returning.
+ *   - Errors: DD_ERR_BAD_ARG for null pointers, nchans < 1, ndm < 0, nsamp < 0, tsamp <= 0,
+ *     non-finite or negative DM, fch1 <= 0 or any f_c <= 0, foff > 0 (negative shifts),
+ *     a stride shorter than the row, a shift above INT32_MAX/2.  ndm == 0 or nsamp == 0 is
+ *     DD_OK and writes nothing.
+ */
+#ifndef DEDISP_B200_H
+#define DEDISP_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    DD_OK              =  0,
+    DD_ERR_BAD_ARG     = -1,
+    DD_ERR_UNSUPPORTED = -2,   /* no sm_100 device, or a dtype/kernel the plan does not have */
+    DD_ERR_NOMEM       = -3,
+    DD_ERR_CUDA        = -4,   /* a CUDA runtime call failed; see dd_last_error() */
+    DD_ERR_STATE       = -5    /* stream pushed beyond its declared max_chunk, etc. */
+};
+
+enum { DD_F32 = 0,   /* float32 in, float32 out  */
+       DD_U8  = 1 }; /* uint8   in, int32   out  */
+
+/* kernel selection for dd_plan_set_kernel (tests and benchmarks; default DD_KERNEL_AUTO) */
+enum { DD_KERNEL_AUTO    = 0,
+       DD_KERNEL_GENERIC = 1,   /* shared-memory channel-vector kernel, any DM list        */
+       DD_KERNEL_WINDOW  = 2 }; /* register-window kernel (TMA-staged), needs small spreads */
+
+const char* dd_strerror(int code);   /* static string for an error code */
+const char* dd_last_error(void);     /* thread-local detail of the last failure ("" if none) */
+const char* dd_version(void);        /* static "dedisp_b200 x.y (sm_100a)" */
+
+/* ---- the delay table (eq 2.2/2.3), host only, double precision -------- */
+
+/* maxshift = max over d, c of s(d,c).  dm_list: HOST, ndm doubles.  <0 = error code. */
+int64_t dd_max_shift(int nchans, double fch1, double foff, double tsamp,
+                     const double* dm_list, int ndm);
+
+/* The whole table, HOST int32 [ndm][nchans] in dm_list order; no GPU needed. */
+int dd_shift_table(int nchans, double fch1, double foff, double tsamp,
+                   const double* dm_list, int ndm, int32_t* host_out);
+
+/* ---- one-shot calls (north_star signature): X, D are DEVICE pointers ---------------------
+ * X: [nchans][nsamp + maxshift] contiguous; D: [ndm][nsamp] contiguous, rows in dm_list order.
+ * Builds a plan, runs it on the legacy default stream, synchronises, destroys the plan. */
+int dd_dedisperse_f32   (const float*   X, int nchans, int64_t nsamp, double fch1, double foff,
+                         double tsamp, const double* dm_list, int ndm, float*   D);
+int dd_dedisperse_u8_i32(const uint8_t* X, int nchans, int64_t nsamp, double fch1, double foff,
+                         double tsamp, const double* dm_list, int ndm, int32_t* D);
+
+/* Same, with HOST X and D (pageable or pinned): the library allocates device buffers, copies
+ * X up, computes, copies D back, overlapping the three in time slices.  This is the
+ * end-to-end call bench.py times ("e2e"). */
+int dd_dedisperse_f32_host   (const float*   X, int nchans, int64_t nsamp, double fch1, double foff,
+                              double tsamp, const double* dm_list, int ndm, float*   D);
+int dd_dedisperse_u8_i32_host(const uint8_t* X, int nchans, int64_t nsamp, double fch1, double foff,
+                              double tsamp, const double* dm_list, int ndm, int32_t* D);
+
+/* ---- plan form: the table is built once ("computed once during thread
+ * initialisation and transferred to GPU memory") and reused ------------------------------- */
+typedef struct dd_plan dd_plan;
+
+/* dm_list: HOST; any finite non-negative values in any order (duplicates allowed); output rows
+ * are written in the caller's order.  Uploads the device tables on the current device. */
+int     dd_plan_create(dd_plan** out, int dtype, int nchans, double fch1, double foff,
+                       double tsamp, const double* dm_list, int ndm);
+void    dd_plan_destroy(dd_plan* plan);
+int64_t dd_plan_max_shift(const dd_plan* plan);                 /* <0 = error */
+int     dd_plan_ndm(const dd_plan* plan);
+int     dd_plan_nchans(const dd_plan* plan);
+/* the plan's own delay table, HOST int32 [ndm][nchans] in caller DM order (tests compare it
+ * with the oracle's independently built table) */
+int     dd_plan_shift_table(const dd_plan* plan, int32_t* host_out);
+int     dd_plan_set_kernel(dd_plan* plan, int kernel);          /* DD_KERNEL_* */
+/* which kernel dd_execute would launch for these strides/pointers: DD_KERNEL_GENERIC or _WINDOW */
+int     dd_plan_kernel_for(const dd_plan* plan, const void* X, int64_t in_stride,
+                           int64_t in_beam_stride, int64_t out_stride, int64_t out_beam_stride);
+/* number of kernels dd_execute launches per call (for bench.py's gpu_launches) */
+int     dd_plan_launches_per_execute(const dd_plan* plan);
+
+/* X, D: DEVICE.  Strides are in ELEMENTS.  in_stride >= nsamp_out + maxshift is the distance
+ * between channel rows, in_beam_stride between beams (ignored if nbeams == 1); same for D.
+ * Reads X[b][c][0 .. nsamp_out + s(d,c)), writes D[b][d][0 .. nsamp_out). */
+int     dd_execute(const dd_plan* plan, const void* X, int64_t in_stride, int64_t in_beam_stride,
+                   void* D, int64_t out_stride, int64_t out_beam_stride,
+                   int64_t nsamp_out, int nbeams, void* cuda_stream);
+
+/* X, D: HOST (pinned memory makes the copies asynchronous), one beam.  Uploads X in time slices,
+ * runs dd_execute per slice and downloads D, the three overlapped on internal streams; returns
+ * after everything has landed in D.  Device buffers are cached in the plan between calls. */
+int     dd_execute_host(dd_plan* plan, const void* X, int64_t in_stride, void* D,
+                        int64_t out_stride, int64_t nsamp_out);
+
+/* ---- streaming (the last maxshift spectra are kept at the head of the buffer
+ * and the next input appended; buffer sizing eq 3.3) ------------------- */
+typedef struct dd_stream dd_stream;
+
+/* The stream keeps a device work buffer of nbeams*nchans*(maxshift + max_chunk) elements
+ * (double-buffered).  The plan must outlive the stream. */
+int     dd_stream_create(dd_stream** out, const dd_plan* plan, int64_t max_chunk, int nbeams);
+/* X_new: DEVICE [nbeams][nchans][n_new] (strides in elements), 0 <= n_new <= max_chunk.
+ * Emits into D_out (DEVICE, [nbeams][ndm][>= *n_out]) every output sample whose full sweep is
+ * now available: *n_out = max(0, total_in - maxshift) - total_out_so_far.  The concatenation
+ * of the emitted blocks equals the one-shot result on the concatenated input, bit for bit. */
+int     dd_stream_push(dd_stream* s, const void* X_new, int64_t in_stride, int64_t in_beam_stride,
+                       int64_t n_new, void* D_out, int64_t out_stride, int64_t out_beam_stride,
+                       int64_t* n_out, void* cuda_stream);
+int     dd_stream_reset(dd_stream* s);
+void    dd_stream_destroy(dd_stream* s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DEDISP_B200_H */

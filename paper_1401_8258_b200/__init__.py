@@ -1,0 +1,12 @@
+"""B200-native direct incoherent dedispersion (arxiv/paper_1401_8258, §2.1.1 / §2.4).
+
+``binding`` wraps the C ABI of ``include/dedisp_b200.h`` one to one; ``synth`` holds the seeded
+input generators and the BASELINE.json workload shapes (no arithmetic of the method).
+"""
+from .binding import (  # noqa: F401
+    DD_OK, DD_ERR_BAD_ARG, DD_ERR_UNSUPPORTED, DD_ERR_NOMEM, DD_ERR_CUDA, DD_ERR_STATE,
+    DD_F32, DD_U8, DD_KERNEL_AUTO, DD_KERNEL_GENERIC, DD_KERNEL_WINDOW,
+    DedispError, Plan, Stream, lib,
+    dd_version, dd_max_shift, dd_shift_table,
+    dd_dedisperse_f32, dd_dedisperse_u8_i32, dd_dedisperse_f32_host, dd_dedisperse_u8_i32_host,
+)

@@ -1,0 +1,229 @@
+"""ctypes binding of ``include/dedisp_b200.h`` — argument marshalling only.
+
+Every function here has the name and argument order of the C call it wraps; tensors / arrays are
+turned into raw pointers and nothing else happens in Python.  All compute runs in the CUDA
+library; if ``libdedisp_b200.so`` is missing and cannot be built, importing the library fails
+loudly — there is no CPU path.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+DD_OK, DD_ERR_BAD_ARG, DD_ERR_UNSUPPORTED, DD_ERR_NOMEM, DD_ERR_CUDA, DD_ERR_STATE = 0, -1, -2, -3, -4, -5
+DD_F32, DD_U8 = 0, 1
+DD_KERNEL_AUTO, DD_KERNEL_GENERIC, DD_KERNEL_WINDOW = 0, 1, 2
+
+_dp = C.POINTER(C.c_double)
+_vp = C.c_void_p
+_i64 = C.c_int64
+
+# name -> (restype, argtypes): one entry per function declared in include/dedisp_b200.h
+SIGNATURES = {
+    "dd_strerror": (C.c_char_p, [C.c_int]),
+    "dd_last_error": (C.c_char_p, []),
+    "dd_version": (C.c_char_p, []),
+    "dd_max_shift": (_i64, [C.c_int, C.c_double, C.c_double, C.c_double, _dp, C.c_int]),
+    "dd_shift_table": (C.c_int, [C.c_int, C.c_double, C.c_double, C.c_double, _dp, C.c_int, _vp]),
+    "dd_dedisperse_f32": (C.c_int, [_vp, C.c_int, _i64, C.c_double, C.c_double, C.c_double, _dp, C.c_int, _vp]),
+    "dd_dedisperse_u8_i32": (C.c_int, [_vp, C.c_int, _i64, C.c_double, C.c_double, C.c_double, _dp, C.c_int, _vp]),
+    "dd_dedisperse_f32_host": (C.c_int, [_vp, C.c_int, _i64, C.c_double, C.c_double, C.c_double, _dp, C.c_int, _vp]),
+    "dd_dedisperse_u8_i32_host": (C.c_int, [_vp, C.c_int, _i64, C.c_double, C.c_double, C.c_double, _dp, C.c_int, _vp]),
+    "dd_plan_create": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, _dp, C.c_int]),
+    "dd_plan_destroy": (None, [_vp]),
+    "dd_plan_max_shift": (_i64, [_vp]),
+    "dd_plan_ndm": (C.c_int, [_vp]),
+    "dd_plan_nchans": (C.c_int, [_vp]),
+    "dd_plan_shift_table": (C.c_int, [_vp, _vp]),
+    "dd_plan_set_kernel": (C.c_int, [_vp, C.c_int]),
+    "dd_plan_kernel_for": (C.c_int, [_vp, _vp, _i64, _i64, _i64, _i64]),
+    "dd_plan_launches_per_execute": (C.c_int, [_vp]),
+    "dd_execute": (C.c_int, [_vp, _vp, _i64, _i64, _vp, _i64, _i64, _i64, C.c_int, _vp]),
+    "dd_execute_host": (C.c_int, [_vp, _vp, _i64, _vp, _i64, _i64]),
+    "dd_stream_create": (C.c_int, [C.POINTER(_vp), _vp, _i64, C.c_int]),
+    "dd_stream_push": (C.c_int, [_vp, _vp, _i64, _i64, _i64, _vp, _i64, _i64, C.POINTER(_i64), _vp]),
+    "dd_stream_reset": (C.c_int, [_vp]),
+    "dd_stream_destroy": (None, [_vp]),
+}
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load (building if stale and nvcc is present) the CUDA library.  Raises if impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    try:
+        path = _build.build()
+    except Exception:
+        if not os.path.exists(path):
+            raise RuntimeError(
+                "libdedisp_b200.so is missing and could not be built with nvcc; "
+                "this package has no CPU fallback") from None
+    l = C.CDLL(path)
+    for name, (res, args) in SIGNATURES.items():
+        f = getattr(l, name)          # AttributeError if the .so lacks a declared symbol
+        f.restype = res
+        f.argtypes = args
+    _lib = l
+    return l
+
+
+class DedispError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        l = lib()
+        self.code = code
+        detail = l.dd_last_error().decode()
+        super().__init__("%s: %s (%d)%s" % (where, l.dd_strerror(code).decode(), code,
+                                            ": " + detail if detail else ""))
+
+
+def _check(code: int, where: str) -> int:
+    if code < 0:
+        raise DedispError(int(code), where)
+    return int(code)
+
+
+def _ptr(obj) -> int:
+    """Raw address of a torch tensor, numpy array, or int (None -> 0)."""
+    if obj is None:
+        return 0
+    if isinstance(obj, int):
+        return obj
+    if hasattr(obj, "data_ptr"):
+        return int(obj.data_ptr())
+    if isinstance(obj, np.ndarray):
+        return int(obj.ctypes.data)
+    raise TypeError("expected a tensor, ndarray or integer address, got %r" % type(obj))
+
+
+def _dms(dm_list):
+    a = np.ascontiguousarray(np.asarray(dm_list, dtype=np.float64))
+    return a, a.ctypes.data_as(_dp), int(a.size)
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        return 0
+    if isinstance(stream, int):
+        return stream
+    return int(stream.cuda_stream)       # torch.cuda.Stream
+
+
+# ------------------------------------------------------------------ plain calls
+
+def dd_version() -> str:
+    return lib().dd_version().decode()
+
+
+def dd_max_shift(nchans, fch1, foff, tsamp, dm_list) -> int:
+    a, p, n = _dms(dm_list)
+    return _check(lib().dd_max_shift(nchans, fch1, foff, tsamp, p, n), "dd_max_shift")
+
+
+def dd_shift_table(nchans, fch1, foff, tsamp, dm_list) -> np.ndarray:
+    a, p, n = _dms(dm_list)
+    out = np.empty((n, nchans), dtype=np.int32)
+    _check(lib().dd_shift_table(nchans, fch1, foff, tsamp, p, n, out.ctypes.data), "dd_shift_table")
+    return out
+
+
+def dd_dedisperse_f32(X, nchans, nsamp, fch1, foff, tsamp, dm_list, D) -> None:
+    a, p, n = _dms(dm_list)
+    _check(lib().dd_dedisperse_f32(_ptr(X), nchans, nsamp, fch1, foff, tsamp, p, n, _ptr(D)), "dd_dedisperse_f32")
+
+
+def dd_dedisperse_u8_i32(X, nchans, nsamp, fch1, foff, tsamp, dm_list, D) -> None:
+    a, p, n = _dms(dm_list)
+    _check(lib().dd_dedisperse_u8_i32(_ptr(X), nchans, nsamp, fch1, foff, tsamp, p, n, _ptr(D)), "dd_dedisperse_u8_i32")
+
+
+def dd_dedisperse_f32_host(X, nchans, nsamp, fch1, foff, tsamp, dm_list, D) -> None:
+    a, p, n = _dms(dm_list)
+    _check(lib().dd_dedisperse_f32_host(_ptr(X), nchans, nsamp, fch1, foff, tsamp, p, n, _ptr(D)), "dd_dedisperse_f32_host")
+
+
+def dd_dedisperse_u8_i32_host(X, nchans, nsamp, fch1, foff, tsamp, dm_list, D) -> None:
+    a, p, n = _dms(dm_list)
+    _check(lib().dd_dedisperse_u8_i32_host(_ptr(X), nchans, nsamp, fch1, foff, tsamp, p, n, _ptr(D)), "dd_dedisperse_u8_i32_host")
+
+
+# ------------------------------------------------------------------ plan / stream handles
+
+class Plan:
+    """Owns a ``dd_plan*``; methods are the dd_plan_* / dd_execute* calls."""
+
+    def __init__(self, dtype, nchans, fch1, foff, tsamp, dm_list):
+        a, p, n = _dms(dm_list)
+        h = _vp()
+        _check(lib().dd_plan_create(C.byref(h), dtype, nchans, fch1, foff, tsamp, p, n), "dd_plan_create")
+        self._h = h
+        self.dtype, self.nchans, self.ndm = dtype, nchans, n
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib().dd_plan_destroy(self._h)
+            self._h = None
+
+    __del__ = destroy
+
+    def max_shift(self) -> int:
+        return _check(lib().dd_plan_max_shift(self._h), "dd_plan_max_shift")
+
+    def shift_table(self) -> np.ndarray:
+        out = np.empty((self.ndm, self.nchans), dtype=np.int32)
+        _check(lib().dd_plan_shift_table(self._h, out.ctypes.data), "dd_plan_shift_table")
+        return out
+
+    def set_kernel(self, kernel: int) -> None:
+        _check(lib().dd_plan_set_kernel(self._h, kernel), "dd_plan_set_kernel")
+
+    def kernel_for(self, X, in_stride, in_beam_stride=0, out_stride=0, out_beam_stride=0) -> int:
+        return _check(lib().dd_plan_kernel_for(self._h, _ptr(X), in_stride, in_beam_stride, out_stride,
+                                               out_beam_stride), "dd_plan_kernel_for")
+
+    def launches_per_execute(self) -> int:
+        return _check(lib().dd_plan_launches_per_execute(self._h), "dd_plan_launches_per_execute")
+
+    def execute(self, X, in_stride, in_beam_stride, D, out_stride, out_beam_stride, nsamp_out, nbeams=1,
+                stream=None) -> None:
+        _check(lib().dd_execute(self._h, _ptr(X), in_stride, in_beam_stride, _ptr(D), out_stride,
+                                out_beam_stride, nsamp_out, nbeams, _stream_ptr(stream)), "dd_execute")
+
+    def execute_host(self, X, in_stride, D, out_stride, nsamp_out) -> None:
+        _check(lib().dd_execute_host(self._h, _ptr(X), in_stride, _ptr(D), out_stride, nsamp_out),
+               "dd_execute_host")
+
+
+class Stream:
+    """Owns a ``dd_stream*`` (chunked streaming with the maxshift carry)."""
+
+    def __init__(self, plan: Plan, max_chunk: int, nbeams: int = 1):
+        h = _vp()
+        _check(lib().dd_stream_create(C.byref(h), plan._h, max_chunk, nbeams), "dd_stream_create")
+        self._h = h
+        self.plan = plan            # keep the plan alive
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib().dd_stream_destroy(self._h)
+            self._h = None
+
+    __del__ = destroy
+
+    def push(self, X_new, in_stride, in_beam_stride, n_new, D_out, out_stride, out_beam_stride,
+             stream=None) -> int:
+        n_out = _i64(0)
+        _check(lib().dd_stream_push(self._h, _ptr(X_new), in_stride, in_beam_stride, n_new, _ptr(D_out),
+                                    out_stride, out_beam_stride, C.byref(n_out), _stream_ptr(stream)),
+               "dd_stream_push")
+        return int(n_out.value)
+
+    def reset(self) -> None:
+        _check(lib().dd_stream_reset(self._h), "dd_stream_reset")

@@ -1,0 +1,529 @@
+// C-ABI entry points (include/dedisp_b200.h): argument checking, plan / stream objects, kernel
+// selection.  No arithmetic of the method lives here except through plan.cpp (the delay table)
+// and the kernels.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstring>
+#include <new>
+
+#include "dd_internal.h"
+
+namespace dd {
+
+static thread_local std::string g_last_error;
+
+void set_error(const std::string& msg) { g_last_error = msg; }
+int fail(int code, const std::string& msg)
+{
+    g_last_error = msg;
+    return code;
+}
+
+static int cuda_fail(const char* what, cudaError_t e)
+{
+    return fail(DD_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define DD_CUDA(call)                                           \
+    do {                                                        \
+        cudaError_t e__ = (call);                               \
+        if (e__ != cudaSuccess) return cuda_fail(#call, e__);   \
+    } while (0)
+
+// The library is sm_100a only: refuse anything else loudly (no CPU fallback, north_star).
+static int require_sm100(int* device_out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(DD_ERR_UNSUPPORTED, std::string("no usable CUDA device: ") + cudaGetErrorString(e));
+    }
+    int major = 0;
+    e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e != cudaSuccess) return cuda_fail("cudaDeviceGetAttribute", e);
+    if (major != 10)
+        return fail(DD_ERR_UNSUPPORTED, "device is not sm_100 (B200); this library has no other path");
+    if (device_out) *device_out = dev;
+    return DD_OK;
+}
+
+static size_t elem_size(int dtype) { return dtype == DD_F32 ? 4 : 1; }
+
+}  // namespace dd
+
+using namespace dd;
+
+// host-call workspace cached in the plan (see dd_execute_host)
+struct dd_host_ws {
+    void* dX = nullptr;
+    void* dD = nullptr;
+    size_t x_bytes = 0, d_bytes = 0;
+    cudaStream_t s_in = nullptr, s_run = nullptr, s_out = nullptr;
+    std::vector<cudaEvent_t> ev_in, ev_run;
+};
+
+struct dd_stream {
+    const dd_plan* plan = nullptr;
+    int64_t max_chunk = 0;
+    int nbeams = 1;
+    int64_t cap = 0;        // row length of the work buffers (elements), multiple of 64
+    int64_t have = 0;       // samples currently held per channel (the carry)
+    int64_t total_in = 0, total_out = 0;
+    void* buf[2] = {nullptr, nullptr};
+    int cur = 0;
+};
+
+extern "C" {
+
+const char* dd_strerror(int code)
+{
+    switch (code) {
+        case DD_OK: return "ok";
+        case DD_ERR_BAD_ARG: return "bad argument";
+        case DD_ERR_UNSUPPORTED: return "unsupported (needs an sm_100 / B200 device)";
+        case DD_ERR_NOMEM: return "out of memory";
+        case DD_ERR_CUDA: return "CUDA runtime error";
+        case DD_ERR_STATE: return "invalid state";
+    }
+    return "unknown error";
+}
+
+const char* dd_last_error(void) { return g_last_error.c_str(); }
+const char* dd_version(void) { return "dedisp_b200 0.1 (sm_100a)"; }
+
+int64_t dd_max_shift(int nchans, double fch1, double foff, double tsamp, const double* dm_list, int ndm)
+{
+    return host_max_shift(nchans, fch1, foff, tsamp, dm_list, ndm);
+}
+
+int dd_shift_table(int nchans, double fch1, double foff, double tsamp, const double* dm_list, int ndm,
+                   int32_t* host_out)
+{
+    if (ndm > 0 && !host_out) return fail(DD_ERR_BAD_ARG, "host_out is null");
+    HostTable t;
+    int rc = build_host_table(nchans, fch1, foff, tsamp, dm_list, ndm, &t);
+    if (rc != DD_OK) return rc;
+    for (int r = 0; r < ndm; ++r)
+        std::memcpy(host_out + (size_t)t.order[r] * nchans, &t.shift[(size_t)r * nchans],
+                    (size_t)nchans * sizeof(int32_t));
+    return DD_OK;
+}
+
+// ------------------------------------------------------------------------------ plan
+
+int dd_plan_create(dd_plan** out, int dtype, int nchans, double fch1, double foff, double tsamp,
+                   const double* dm_list, int ndm)
+{
+    if (!out) return fail(DD_ERR_BAD_ARG, "out is null");
+    *out = nullptr;
+    if (dtype != DD_F32 && dtype != DD_U8) return fail(DD_ERR_BAD_ARG, "dtype must be DD_F32 or DD_U8");
+    dd_plan* p = new (std::nothrow) dd_plan;
+    if (!p) return fail(DD_ERR_NOMEM, "plan allocation failed");
+    p->dtype = dtype;
+    p->nchans = nchans;
+    p->ndm = ndm;
+    p->fch1 = fch1;
+    p->foff = foff;
+    p->tsamp = tsamp;
+    int rc = build_host_table(nchans, fch1, foff, tsamp, dm_list, ndm, &p->host);
+    if (rc != DD_OK) {
+        delete p;
+        return rc;
+    }
+    rc = require_sm100(&p->device);
+    if (rc != DD_OK) {
+        delete p;
+        return rc;
+    }
+    // generic kernel tiling: the most trials per block whose channel vector still fits
+    p->generic_kb = 1;
+    p->generic_spread = 0;
+    const int cands[] = {16, 8, 4, 2};
+    for (int kb : cands) {
+        int64_t sp = max_tile_spread(p->host, kb);
+        if (sp <= 512) {
+            p->generic_kb = kb;
+            p->generic_spread = (int)sp;
+            break;
+        }
+    }
+    if (ndm > 0) {
+        cudaError_t e = cudaMalloc(&p->d_shift, p->host.shift.size() * sizeof(int32_t));
+        if (e == cudaSuccess) e = cudaMalloc(&p->d_order, (size_t)ndm * sizeof(int32_t));
+        if (e != cudaSuccess) {
+            dd_plan_destroy(p);
+            cudaGetLastError();
+            return fail(DD_ERR_NOMEM, std::string("device table allocation: ") + cudaGetErrorString(e));
+        }
+        e = cudaMemcpy(p->d_shift, p->host.shift.data(), p->host.shift.size() * sizeof(int32_t),
+                       cudaMemcpyHostToDevice);
+        if (e == cudaSuccess)
+            e = cudaMemcpy(p->d_order, p->host.order.data(), (size_t)ndm * sizeof(int32_t),
+                           cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) {
+            dd_plan_destroy(p);
+            return cuda_fail("table upload", e);
+        }
+    }
+    rc = build_window_plan(p);
+    if (rc != DD_OK) {
+        dd_plan_destroy(p);
+        return rc;
+    }
+    *out = p;
+    return DD_OK;
+}
+
+void dd_plan_destroy(dd_plan* p)
+{
+    if (!p) return;
+    if (p->host_ws) {
+        dd_host_ws* w = p->host_ws;
+        if (w->dX) cudaFree(w->dX);
+        if (w->dD) cudaFree(w->dD);
+        for (auto e : w->ev_in) cudaEventDestroy(e);
+        for (auto e : w->ev_run) cudaEventDestroy(e);
+        if (w->s_in) cudaStreamDestroy(w->s_in);
+        if (w->s_run) cudaStreamDestroy(w->s_run);
+        if (w->s_out) cudaStreamDestroy(w->s_out);
+        delete w;
+    }
+    destroy_window_plan(p);
+    if (p->d_shift) cudaFree(p->d_shift);
+    if (p->d_order) cudaFree(p->d_order);
+    delete p;
+}
+
+int64_t dd_plan_max_shift(const dd_plan* p)
+{
+    if (!p) return fail(DD_ERR_BAD_ARG, "plan is null");
+    return p->host.maxshift;
+}
+int dd_plan_ndm(const dd_plan* p) { return p ? p->ndm : fail(DD_ERR_BAD_ARG, "plan is null"); }
+int dd_plan_nchans(const dd_plan* p) { return p ? p->nchans : fail(DD_ERR_BAD_ARG, "plan is null"); }
+
+int dd_plan_shift_table(const dd_plan* p, int32_t* host_out)
+{
+    if (!p || !host_out) return fail(DD_ERR_BAD_ARG, "null argument");
+    for (int r = 0; r < p->ndm; ++r)
+        std::memcpy(host_out + (size_t)p->host.order[r] * p->nchans,
+                    &p->host.shift[(size_t)r * p->nchans], (size_t)p->nchans * sizeof(int32_t));
+    return DD_OK;
+}
+
+int dd_plan_set_kernel(dd_plan* p, int kernel)
+{
+    if (!p) return fail(DD_ERR_BAD_ARG, "plan is null");
+    if (kernel != DD_KERNEL_AUTO && kernel != DD_KERNEL_GENERIC && kernel != DD_KERNEL_WINDOW)
+        return fail(DD_ERR_BAD_ARG, "unknown kernel id");
+    if (kernel == DD_KERNEL_WINDOW && !window_plan_usable(p))
+        return fail(DD_ERR_UNSUPPORTED, "the register-window kernel does not take this plan");
+    p->kernel_pref = kernel;
+    return DD_OK;
+}
+
+int dd_plan_kernel_for(const dd_plan* p, const void* X, int64_t in_stride, int64_t in_beam_stride,
+                       int64_t out_stride, int64_t out_beam_stride)
+{
+    if (!p) return fail(DD_ERR_BAD_ARG, "plan is null");
+    if (p->kernel_pref == DD_KERNEL_GENERIC) return DD_KERNEL_GENERIC;
+    if (window_plan_usable(p) &&
+        window_args_ok(p, X, in_stride, in_beam_stride, out_stride, out_beam_stride))
+        return DD_KERNEL_WINDOW;
+    return DD_KERNEL_GENERIC;
+}
+
+int dd_plan_launches_per_execute(const dd_plan* p)
+{
+    if (!p) return fail(DD_ERR_BAD_ARG, "plan is null");
+    return 1;
+}
+
+int dd_execute(const dd_plan* p, const void* X, int64_t in_stride, int64_t in_beam_stride, void* D,
+               int64_t out_stride, int64_t out_beam_stride, int64_t nsamp_out, int nbeams,
+               void* cuda_stream)
+{
+    if (!p) return fail(DD_ERR_BAD_ARG, "plan is null");
+    if (nsamp_out < 0) return fail(DD_ERR_BAD_ARG, "nsamp_out must be >= 0");
+    if (nbeams < 1) return fail(DD_ERR_BAD_ARG, "nbeams must be >= 1");
+    if (p->ndm == 0 || nsamp_out == 0) return DD_OK;
+    if (!X || !D) return fail(DD_ERR_BAD_ARG, "X or D is null");
+    if (in_stride < nsamp_out + p->host.maxshift)
+        return fail(DD_ERR_BAD_ARG, "in_stride is shorter than nsamp_out + maxshift");
+    if (out_stride < nsamp_out) return fail(DD_ERR_BAD_ARG, "out_stride is shorter than nsamp_out");
+    if (nbeams > 1 && (in_beam_stride <= 0 || out_beam_stride <= 0))
+        return fail(DD_ERR_BAD_ARG, "beam strides must be positive when nbeams > 1");
+    if (p->dtype == DD_F32 && (((uintptr_t)X | (uintptr_t)D) & 3))
+        return fail(DD_ERR_BAD_ARG, "float32 buffers must be 4-byte aligned");
+    if (p->dtype == DD_U8 && ((uintptr_t)D & 3))
+        return fail(DD_ERR_BAD_ARG, "int32 output must be 4-byte aligned");
+
+    ExecArgs a;
+    a.X = X;
+    a.D = D;
+    a.in_stride = in_stride;
+    a.in_beam_stride = nbeams > 1 ? in_beam_stride : 0;
+    a.out_stride = out_stride;
+    a.out_beam_stride = nbeams > 1 ? out_beam_stride : 0;
+    a.nsamp_out = nsamp_out;
+    a.nbeams = nbeams;
+    a.nchans = p->nchans;
+    a.ndm = p->ndm;
+    a.d_shift = p->d_shift;
+    a.d_order = p->d_order;
+    a.stream = cuda_stream;
+
+    int k = dd_plan_kernel_for(p, X, in_stride, a.in_beam_stride, out_stride, a.out_beam_stride);
+    if (p->kernel_pref == DD_KERNEL_WINDOW && k != DD_KERNEL_WINDOW)
+        return fail(DD_ERR_UNSUPPORTED, "window kernel forced but pointers/strides are not 16-byte aligned");
+    if (k == DD_KERNEL_WINDOW) return launch_window(p, a);
+    return launch_generic(p->dtype, p->generic_kb, p->generic_spread, a);
+}
+
+// ------------------------------------------------------------------------------ one-shot
+
+static int one_shot(int dtype, const void* X, int nchans, int64_t nsamp, double fch1, double foff,
+                    double tsamp, const double* dm_list, int ndm, void* D)
+{
+    if (nsamp < 0) return fail(DD_ERR_BAD_ARG, "nsamp must be >= 0");
+    dd_plan* p = nullptr;
+    int rc = dd_plan_create(&p, dtype, nchans, fch1, foff, tsamp, dm_list, ndm);
+    if (rc != DD_OK) return rc;
+    rc = dd_execute(p, X, nsamp + p->host.maxshift, 0, D, nsamp, 0, nsamp, 1, nullptr);
+    if (rc == DD_OK) {
+        cudaError_t e = cudaStreamSynchronize(nullptr);
+        if (e != cudaSuccess) rc = cuda_fail("cudaStreamSynchronize", e);
+    }
+    dd_plan_destroy(p);
+    return rc;
+}
+
+int dd_dedisperse_f32(const float* X, int nchans, int64_t nsamp, double fch1, double foff, double tsamp,
+                      const double* dm_list, int ndm, float* D)
+{
+    return one_shot(DD_F32, X, nchans, nsamp, fch1, foff, tsamp, dm_list, ndm, D);
+}
+
+int dd_dedisperse_u8_i32(const uint8_t* X, int nchans, int64_t nsamp, double fch1, double foff,
+                         double tsamp, const double* dm_list, int ndm, int32_t* D)
+{
+    return one_shot(DD_U8, X, nchans, nsamp, fch1, foff, tsamp, dm_list, ndm, D);
+}
+
+// ------------------------------------------------------------------------------ host buffers
+
+static int64_t round_up(int64_t v, int64_t m) { return (v + m - 1) / m * m; }
+
+int dd_execute_host(dd_plan* p, const void* X, int64_t in_stride, void* D, int64_t out_stride,
+                    int64_t nsamp_out)
+{
+    if (!p) return fail(DD_ERR_BAD_ARG, "plan is null");
+    if (nsamp_out < 0) return fail(DD_ERR_BAD_ARG, "nsamp_out must be >= 0");
+    if (p->ndm == 0 || nsamp_out == 0) return DD_OK;
+    if (!X || !D) return fail(DD_ERR_BAD_ARG, "X or D is null");
+    const int64_t ms = p->host.maxshift;
+    if (in_stride < nsamp_out + ms) return fail(DD_ERR_BAD_ARG, "in_stride is shorter than nsamp_out + maxshift");
+    if (out_stride < nsamp_out) return fail(DD_ERR_BAD_ARG, "out_stride is shorter than nsamp_out");
+    const size_t es = elem_size(p->dtype);
+    const int64_t dstride_in = round_up(nsamp_out + ms, 64);
+    const int64_t dstride_out = round_up(nsamp_out, 64);
+    const size_t xb = (size_t)p->nchans * dstride_in * es;
+    const size_t db = (size_t)p->ndm * dstride_out * 4;
+
+    if (!p->host_ws) {
+        p->host_ws = new (std::nothrow) dd_host_ws;
+        if (!p->host_ws) return fail(DD_ERR_NOMEM, "workspace allocation failed");
+        dd_host_ws* w = p->host_ws;
+        DD_CUDA(cudaStreamCreateWithFlags(&w->s_in, cudaStreamNonBlocking));
+        DD_CUDA(cudaStreamCreateWithFlags(&w->s_run, cudaStreamNonBlocking));
+        DD_CUDA(cudaStreamCreateWithFlags(&w->s_out, cudaStreamNonBlocking));
+    }
+    dd_host_ws* w = p->host_ws;
+    if (w->x_bytes < xb) {
+        if (w->dX) cudaFree(w->dX);
+        w->dX = nullptr;
+        w->x_bytes = 0;
+        cudaError_t e = cudaMalloc(&w->dX, xb);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            return fail(DD_ERR_NOMEM, std::string("device X buffer: ") + cudaGetErrorString(e));
+        }
+        w->x_bytes = xb;
+    }
+    if (w->d_bytes < db) {
+        if (w->dD) cudaFree(w->dD);
+        w->dD = nullptr;
+        w->d_bytes = 0;
+        cudaError_t e = cudaMalloc(&w->dD, db);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            return fail(DD_ERR_NOMEM, std::string("device D buffer: ") + cudaGetErrorString(e));
+        }
+        w->d_bytes = db;
+    }
+
+    // time slices: copy-in of slice k+1 and copy-out of slice k-1 overlap the kernel of slice k
+    int64_t slice = round_up(std::max<int64_t>((nsamp_out + 7) / 8, 8192), 1024);
+    const int nslices = (int)((nsamp_out + slice - 1) / slice);
+    while ((int)w->ev_in.size() < nslices) {
+        cudaEvent_t a, b;
+        DD_CUDA(cudaEventCreateWithFlags(&a, cudaEventDisableTiming));
+        DD_CUDA(cudaEventCreateWithFlags(&b, cudaEventDisableTiming));
+        w->ev_in.push_back(a);
+        w->ev_run.push_back(b);
+    }
+    int64_t in_done = 0;   // input columns already uploaded
+    for (int k = 0; k < nslices; ++k) {
+        const int64_t ta = (int64_t)k * slice, tb = std::min(nsamp_out, ta + slice);
+        const int64_t in_end = tb + ms;
+        if (in_end > in_done) {
+            DD_CUDA(cudaMemcpy2DAsync((char*)w->dX + in_done * es, dstride_in * es,
+                                      (const char*)X + in_done * es, in_stride * es,
+                                      (size_t)(in_end - in_done) * es, p->nchans,
+                                      cudaMemcpyHostToDevice, w->s_in));
+            in_done = in_end;
+        }
+        DD_CUDA(cudaEventRecord(w->ev_in[k], w->s_in));
+        DD_CUDA(cudaStreamWaitEvent(w->s_run, w->ev_in[k], 0));
+        int rc = dd_execute(p, (const char*)w->dX + ta * es, dstride_in, 0, (char*)w->dD + ta * 4,
+                            dstride_out, 0, tb - ta, 1, w->s_run);
+        if (rc != DD_OK) return rc;
+        DD_CUDA(cudaEventRecord(w->ev_run[k], w->s_run));
+        DD_CUDA(cudaStreamWaitEvent(w->s_out, w->ev_run[k], 0));
+        DD_CUDA(cudaMemcpy2DAsync((char*)D + ta * 4, out_stride * 4, (const char*)w->dD + ta * 4,
+                                  dstride_out * 4, (size_t)(tb - ta) * 4, p->ndm,
+                                  cudaMemcpyDeviceToHost, w->s_out));
+    }
+    DD_CUDA(cudaStreamSynchronize(w->s_out));
+    DD_CUDA(cudaStreamSynchronize(w->s_run));
+    DD_CUDA(cudaStreamSynchronize(w->s_in));
+    return DD_OK;
+}
+
+static int one_shot_host(int dtype, const void* X, int nchans, int64_t nsamp, double fch1, double foff,
+                         double tsamp, const double* dm_list, int ndm, void* D)
+{
+    if (nsamp < 0) return fail(DD_ERR_BAD_ARG, "nsamp must be >= 0");
+    dd_plan* p = nullptr;
+    int rc = dd_plan_create(&p, dtype, nchans, fch1, foff, tsamp, dm_list, ndm);
+    if (rc != DD_OK) return rc;
+    rc = dd_execute_host(p, X, nsamp + p->host.maxshift, D, nsamp, nsamp);
+    dd_plan_destroy(p);
+    return rc;
+}
+
+int dd_dedisperse_f32_host(const float* X, int nchans, int64_t nsamp, double fch1, double foff,
+                           double tsamp, const double* dm_list, int ndm, float* D)
+{
+    return one_shot_host(DD_F32, X, nchans, nsamp, fch1, foff, tsamp, dm_list, ndm, D);
+}
+
+int dd_dedisperse_u8_i32_host(const uint8_t* X, int nchans, int64_t nsamp, double fch1, double foff,
+                              double tsamp, const double* dm_list, int ndm, int32_t* D)
+{
+    return one_shot_host(DD_U8, X, nchans, nsamp, fch1, foff, tsamp, dm_list, ndm, D);
+}
+
+// ------------------------------------------------------------------------------ streaming
+
+int dd_stream_create(dd_stream** out, const dd_plan* plan, int64_t max_chunk, int nbeams)
+{
+    if (!out) return fail(DD_ERR_BAD_ARG, "out is null");
+    *out = nullptr;
+    if (!plan) return fail(DD_ERR_BAD_ARG, "plan is null");
+    if (max_chunk < 1) return fail(DD_ERR_BAD_ARG, "max_chunk must be >= 1");
+    if (nbeams < 1) return fail(DD_ERR_BAD_ARG, "nbeams must be >= 1");
+    dd_stream* s = new (std::nothrow) dd_stream;
+    if (!s) return fail(DD_ERR_NOMEM, "stream allocation failed");
+    s->plan = plan;
+    s->max_chunk = max_chunk;
+    s->nbeams = nbeams;
+    s->cap = round_up(plan->host.maxshift + max_chunk, 64);
+    const size_t bytes = (size_t)nbeams * plan->nchans * s->cap * elem_size(plan->dtype);
+    for (int i = 0; i < 2; ++i) {
+        cudaError_t e = cudaMalloc(&s->buf[i], bytes);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            dd_stream_destroy(s);
+            return fail(DD_ERR_NOMEM, std::string("stream work buffer: ") + cudaGetErrorString(e));
+        }
+    }
+    *out = s;
+    return DD_OK;
+}
+
+int dd_stream_push(dd_stream* s, const void* X_new, int64_t in_stride, int64_t in_beam_stride,
+                   int64_t n_new, void* D_out, int64_t out_stride, int64_t out_beam_stride,
+                   int64_t* n_out, void* cuda_stream)
+{
+    if (n_out) *n_out = 0;
+    if (!s || !n_out) return fail(DD_ERR_BAD_ARG, "null argument");
+    if (n_new < 0) return fail(DD_ERR_BAD_ARG, "n_new must be >= 0");
+    if (n_new > s->max_chunk) return fail(DD_ERR_STATE, "n_new exceeds the stream's max_chunk");
+    if (n_new == 0) return DD_OK;
+    if (!X_new) return fail(DD_ERR_BAD_ARG, "X_new is null");
+    if (in_stride < n_new) return fail(DD_ERR_BAD_ARG, "in_stride is shorter than n_new");
+    const dd_plan* p = s->plan;
+    const size_t es = elem_size(p->dtype);
+    const int nch = p->nchans;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (s->nbeams > 1 && in_beam_stride <= 0) return fail(DD_ERR_BAD_ARG, "in_beam_stride must be positive");
+
+    // 1. append the new samples after the carry ("the next input buffer is copied
+    //    after the shifted samples")
+    char* cur = (char*)s->buf[s->cur];
+    const bool packed = s->nbeams == 1 || in_beam_stride == (int64_t)nch * in_stride;
+    if (packed) {
+        DD_CUDA(cudaMemcpy2DAsync(cur + s->have * es, s->cap * es, X_new, in_stride * es, n_new * es,
+                                  (size_t)nch * s->nbeams, cudaMemcpyDeviceToDevice, st));
+    } else {
+        for (int b = 0; b < s->nbeams; ++b)
+            DD_CUDA(cudaMemcpy2DAsync(cur + ((size_t)b * nch * s->cap + s->have) * es, s->cap * es,
+                                      (const char*)X_new + (size_t)b * in_beam_stride * es,
+                                      in_stride * es, n_new * es, nch, cudaMemcpyDeviceToDevice, st));
+    }
+    const int64_t total = s->have + n_new;
+    const int64_t emit = std::max<int64_t>(0, total - p->host.maxshift);
+    // 2. every output sample whose whole sweep is present
+    if (emit > 0 && p->ndm > 0) {
+        if (!D_out) return fail(DD_ERR_BAD_ARG, "D_out is null");
+        // the work buffer holds total = emit + maxshift valid samples; its stride is cap
+        int rc = dd_execute(p, cur, s->cap, (int64_t)nch * s->cap, D_out, out_stride, out_beam_stride,
+                            emit, s->nbeams, cuda_stream);
+        if (rc != DD_OK) return rc;
+    }
+    // 3. keep the last (total - emit) <= maxshift samples of every channel at the row head
+    const int64_t carry = total - emit;
+    if (emit > 0) {
+        char* nxt = (char*)s->buf[s->cur ^ 1];
+        if (carry > 0)
+            DD_CUDA(cudaMemcpy2DAsync(nxt, s->cap * es, cur + emit * es, s->cap * es, carry * es,
+                                      (size_t)nch * s->nbeams, cudaMemcpyDeviceToDevice, st));
+        s->cur ^= 1;
+    }
+    s->have = carry;
+    s->total_in += n_new;
+    s->total_out += emit;
+    *n_out = emit;
+    return DD_OK;
+}
+
+int dd_stream_reset(dd_stream* s)
+{
+    if (!s) return fail(DD_ERR_BAD_ARG, "stream is null");
+    s->have = 0;
+    s->total_in = s->total_out = 0;
+    return DD_OK;
+}
+
+void dd_stream_destroy(dd_stream* s)
+{
+    if (!s) return;
+    for (int i = 0; i < 2; ++i)
+        if (s->buf[i]) cudaFree(s->buf[i]);
+    delete s;
+}
+
+}  // extern "C"

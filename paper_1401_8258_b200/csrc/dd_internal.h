@@ -1,0 +1,81 @@
+// Internal declarations shared by the library's translation units (NOT part of the C ABI and
+// not shared with oracle/).
+#pragma once
+
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/dedisp_b200.h"
+
+namespace dd {
+
+// ---- error plumbing ---------------------------------------------------------------------
+void set_error(const std::string& msg);
+int fail(int code, const std::string& msg);
+
+// ---- host delay table (plan.cpp; eq 2.2/2.3) ------------------------------
+struct HostTable {
+    int nchans = 0;
+    int ndm = 0;
+    std::vector<int32_t> order;     // order[r] = caller index of the r-th smallest DM (stable)
+    std::vector<int32_t> shift;     // [ndm][nchans] in SORTED DM order (monotone in r and in c)
+    int64_t maxshift = 0;
+};
+
+// Validates the arguments (DD_ERR_BAD_ARG on failure) and fills the table.
+int build_host_table(int nchans, double fch1, double foff, double tsamp, const double* dm_list,
+                     int ndm, HostTable* out);
+// Validation + maxshift only (no table storage).
+int64_t host_max_shift(int nchans, double fch1, double foff, double tsamp, const double* dm_list,
+                       int ndm);
+
+// Largest s(d_last,c) - s(d_first,c) over all tiles of `kb` consecutive sorted DMs.
+int64_t max_tile_spread(const HostTable& t, int kb);
+
+// ---- kernel launchers (generic.cu / window.cu) ---------------------------------------------
+struct ExecArgs {
+    const void* X;
+    void* D;
+    int64_t in_stride, in_beam_stride, out_stride, out_beam_stride;
+    int64_t nsamp_out;
+    int nbeams;
+    int nchans, ndm;
+    const int32_t* d_shift;         // device [ndm][nchans], sorted DM order
+    const int32_t* d_order;         // device [ndm], sorted row -> caller row
+    void* stream;
+};
+
+// generic channel-vector kernel; kb in {16,8,4,2,1}; max_spread = largest tile spread (samples)
+int launch_generic(int dtype, int kb, int max_spread, const ExecArgs& a);
+
+}  // namespace dd
+
+struct dd_plan;
+struct dd_host_ws;
+struct dd_window_plan;
+
+namespace dd {
+// register-window kernel (window.cu): plan-time tables, eligibility, launch
+int build_window_plan(dd_plan* p);
+void destroy_window_plan(dd_plan* p);
+bool window_plan_usable(const dd_plan* p);
+bool window_args_ok(const dd_plan* p, const void* X, int64_t in_stride, int64_t in_beam_stride,
+                    int64_t out_stride, int64_t out_beam_stride);
+int launch_window(const dd_plan* p, const ExecArgs& a);
+}  // namespace dd
+
+struct dd_plan {
+    int dtype = DD_F32;
+    int nchans = 0, ndm = 0;
+    double fch1 = 0, foff = 0, tsamp = 0;
+    dd::HostTable host;
+    int device = -1;
+    int32_t* d_shift = nullptr;
+    int32_t* d_order = nullptr;
+    int kernel_pref = DD_KERNEL_AUTO;
+    int generic_kb = 1;
+    int generic_spread = 0;
+    dd_window_plan* window = nullptr;   // null: the register-window kernel does not take this plan
+    dd_host_ws* host_ws = nullptr;      // device buffers / streams cached by dd_execute_host
+};

@@ -1,0 +1,289 @@
+"""GPU parity tests proper: the CUDA path (through the C ABI) against the oracle, element by
+element, on the same seeded inputs.  Bit-exact for uint8->int32; |D_gpu - D_oracle| <=
+1e-5 * sum_c|X| per element for float32 (north_star)."""
+import numpy as np
+import pytest
+
+import oracle
+import paper_1401_8258_b200 as dd
+from paper_1401_8258_b200 import synth
+
+from _util import (assert_parity, assert_row_checksums, assert_sampled_parity, dd_dtype,
+                   gpu_dedisperse, make_case, small)
+
+pytestmark = pytest.mark.gpu
+
+KERNELS = [pytest.param(dd.DD_KERNEL_GENERIC, id="generic"), pytest.param(dd.DD_KERNEL_AUTO, id="auto")]
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_gpu():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    assert torch.cuda.get_device_capability(0)[0] == 10, "these kernels are sm_100a only"
+
+
+# ------------------------------------------------------------------ configs, shrunk to oracle size
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_config1_full(kernel):
+    # BASELINE.json configs[0] exactly: 64 ch, 32 DMs, 8192 samples, pulse of amplitude 3 at DM 10
+    w = synth.WORKLOADS[1]
+    X, ms = make_case(w)
+    tab = oracle.shift_table(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    synth.inject_pulse(X, 4000, 1, 3.0, tab[10])
+    D = gpu_dedisperse(w, X, kernel)
+    assert_parity(w, X, D)
+    d, t = np.unravel_index(D.argmax(), D.shape)
+    assert (d, t) == (10, 4000) and abs(D[10, 4000] / 8.0 - 24.0) < 4.0      # S/N ~ A*sqrt(nchans)
+
+
+CASES = [
+    # (workload, nchans, ndm, nsamp): several tiles of every kernel plus a ragged tail
+    (2, 256, 70, 9000 + 37),
+    (2, 1024, 40, 4096 + 1),
+    (3, 512, 50, 8192 + 333),
+    (4, 128, 100, 5000),
+    (5, 300, 61, 7001),
+    (5, 2048, 16, 3000),
+]
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("idx,nchans,ndm,nsamp", CASES)
+def test_shrunk_configs(idx, nchans, ndm, nsamp, kernel):
+    w = small(idx, nchans, ndm, nsamp)
+    X, ms = make_case(w, pulses=3)
+    D = gpu_dedisperse(w, X, kernel)
+    assert_parity(w, X, D)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("idx", [2, 3])
+def test_top_of_the_dm_grid(idx, kernel):
+    # the last trials of the full-size grids (largest shifts and spreads), few of them
+    w0 = synth.WORKLOADS[idx]
+    w = synth.scaled(w0, ndm=24, nsamp=3000)
+    dms = w0.dm_list[-24:]
+    ms = oracle.max_shift(w.nchans, w.fch1, w.foff, w.tsamp, dms)
+    X = synth.make_input(w, w.nsamp + ms)
+    D = gpu_dedisperse(w, X, kernel, dms=dms)
+    assert_parity(w, X, D, dms=dms)
+
+
+# ------------------------------------------------------------------ edge cases
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("dtype", ["f32", "u8"])
+def test_edges(dtype, kernel):
+    base = synth.scaled(synth.WORKLOADS[2], dtype=dtype)
+    # nchans = 1: identity for every DM; DM = 0 only; a single output sample; tiny everything
+    for nchans, ndm, nsamp in [(1, 5, 100), (7, 1, 1), (3, 2, 5), (33, 17, 1025), (64, 33, 2049)]:
+        w = synth.scaled(base, nchans=nchans, ndm=ndm, nsamp=nsamp, foff=-20.0 / nchans, dm_step=7.0)
+        X, ms = make_case(w)
+        D = gpu_dedisperse(w, X, kernel)
+        assert_parity(w, X, D)
+        if nchans == 1:
+            assert np.array_equal(D, np.broadcast_to(X[0, :nsamp].astype(D.dtype), D.shape))
+        if dtype == "u8":                                          # DM = 0 row = channel sum
+            assert np.array_equal(D[0], X[:, :nsamp].sum(axis=0, dtype=np.int64))
+
+
+def test_empty_inputs_write_nothing():
+    import torch
+    w = small(2, 16, 4, 64)
+    plan = dd.Plan(dd.DD_U8, w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    D = torch.full((4, 64), -7, dtype=torch.int32, device="cuda")
+    X = torch.zeros((16, 64 + plan.max_shift()), dtype=torch.uint8, device="cuda")
+    plan.execute(X, X.shape[1], 0, D, 64, 0, 0, 1)                 # nsamp_out = 0
+    torch.cuda.synchronize()
+    assert int((D != -7).sum()) == 0
+    empty = dd.Plan(dd.DD_U8, w.nchans, w.fch1, w.foff, w.tsamp, [])   # ndm = 0
+    empty.execute(X, X.shape[1], 0, D, 64, 0, 64, 1)
+    torch.cuda.synchronize()
+    assert int((D != -7).sum()) == 0 and empty.max_shift() == 0
+    with pytest.raises(dd.DedispError) as e:                       # stride shorter than the row
+        plan.execute(X, 10, 0, D, 64, 0, 64, 1)
+    assert e.value.code == dd.DD_ERR_BAD_ARG
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_unsorted_duplicate_nonuniform_dm_list(kernel):
+    w = small(3, 200, 45, 3000)
+    g = np.random.default_rng(11)
+    dms = g.uniform(0, 900, 45)
+    dms[3] = dms[30]
+    dms[7] = 0.0
+    ms = oracle.max_shift(w.nchans, w.fch1, w.foff, w.tsamp, dms)
+    X = synth.make_input(w, w.nsamp + ms)
+    D = gpu_dedisperse(w, X, kernel, dms=dms)
+    assert_parity(w, X, D, dms=dms)
+    assert np.array_equal(D[3], D[30])
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_large_dm_steps_fall_back_to_narrow_tiles(kernel):
+    # per-trial shift steps of hundreds of samples (Fig 2.9 regime)
+    w = small(1, 64, 9, 2500, dm_step=40.0)
+    X, ms = make_case(w)
+    assert ms > 15000
+    D = gpu_dedisperse(w, X, kernel)
+    assert_parity(w, X, D)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_all_255_input_does_not_overflow(kernel):
+    # P13: 2048 channels of 255 -> every element = 522240 exactly (packed partial sums must flush)
+    w = small(5, 2048, 12, 2100)
+    ms = oracle.max_shift(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    X = np.full((w.nchans, w.nsamp + ms), 255, dtype=np.uint8)
+    D = gpu_dedisperse(w, X, kernel)
+    assert np.all(D == 255 * 2048)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("dtype", ["f32", "u8"])
+def test_impulse_response_against_the_table(dtype, kernel):
+    # P6: X = delta at (c0, u0) => D[d][u0 - s(d,c0)] = 1, everything else 0
+    w = small(2, 96, 40, 5000, dtype=dtype)
+    tab = oracle.shift_table(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    ms = int(tab.max())
+    X = np.zeros((w.nchans, w.nsamp + ms), dtype=w.np_dtype)
+    c0, u0 = 77, 4100
+    X[c0, u0] = 1
+    D = gpu_dedisperse(w, X, kernel)
+    want = np.zeros_like(D)
+    for d in range(w.ndm):
+        want[d, u0 - tab[d, c0]] = 1
+    assert np.array_equal(D, want)
+
+
+# ------------------------------------------------------------------ strides, batch, streaming
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("dtype", ["f32", "u8"])
+def test_strides_offsets_and_batch_equal_loop_of_singles(dtype, kernel):
+    import torch
+    nb = 3
+    w = small(4, 96, 37, 3001, dtype=dtype, nbeams=nb)
+    tdt = torch.float32 if dtype == "f32" else torch.uint8
+    odt = torch.float32 if dtype == "f32" else torch.int32
+    plan = dd.Plan(dd_dtype(w), w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    plan.set_kernel(kernel)
+    ms = plan.max_shift()
+    assert ms == oracle.max_shift(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    xs = [synth.make_input(w, w.nsamp + ms, beam=b) for b in range(nb)]
+    # padded, offset (unaligned for u8) layout: rows of in_stride elements starting 3 elements in
+    in_stride, out_stride = w.nsamp + ms + 13, w.nsamp + 5
+    in_bs, out_bs = w.nchans * in_stride + 101, w.ndm * out_stride + 7
+    Xd = torch.zeros(3 + nb * in_bs, dtype=tdt, device="cuda")
+    for b in range(nb):
+        v = Xd[3 + b * in_bs: 3 + b * in_bs + w.nchans * in_stride].view(w.nchans, in_stride)
+        v[:, :w.nsamp + ms] = torch.from_numpy(xs[b]).cuda()
+    Dd = torch.full((1 + nb * out_bs,), -7, dtype=odt, device="cuda")
+    plan.execute(Xd[3:], in_stride, in_bs, Dd[1:], out_stride, out_bs, w.nsamp, nb)
+    torch.cuda.synchronize()
+    Dh = Dd.cpu().numpy()
+    for b in range(nb):
+        blk = Dh[1 + b * out_bs: 1 + b * out_bs + w.ndm * out_stride].reshape(w.ndm, out_stride)
+        assert_parity(w, xs[b], np.ascontiguousarray(blk[:, :w.nsamp]))
+        assert np.all(blk[:, w.nsamp:] == -7)                       # padding untouched
+        single = gpu_dedisperse(w, xs[b], kernel)                   # batch == loop of singles, bit for bit
+        assert np.array_equal(single, blk[:, :w.nsamp])
+    plan.destroy()
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("dtype", ["f32", "u8"])
+def test_streaming_equals_one_shot_bit_for_bit(dtype, kernel):
+    import torch
+    nb = 2
+    w = small(5, 160, 50, 6000, dtype=dtype, nbeams=nb)
+    odt = torch.float32 if dtype == "f32" else torch.int32
+    plan = dd.Plan(dd_dtype(w), w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    plan.set_kernel(kernel)
+    ms = plan.max_shift()
+    total = w.nsamp + ms
+    xs = np.stack([synth.make_input(w, total, beam=b) for b in range(nb)])
+    Xd = torch.from_numpy(xs).cuda()
+    one = torch.empty((nb, w.ndm, w.nsamp), dtype=odt, device="cuda")
+    plan.execute(Xd, total, w.nchans * total, one, w.nsamp, w.ndm * w.nsamp, w.nsamp, nb)
+    # chunks: smaller than maxshift, larger, ragged, and a 1-sample push
+    chunks, left = [], total
+    for c in [ms // 3 + 1, 1, 1500, 777, 2048]:
+        c = min(c, left); chunks.append(c); left -= c
+    while left > 0:
+        c = min(1900, left); chunks.append(c); left -= c
+    st = dd.Stream(plan, max(chunks), nb)
+    out = torch.full((nb, w.ndm, w.nsamp), -7, dtype=odt, device="cuda")
+    pos = emitted = 0
+    for c in chunks:
+        if c == 0:
+            continue
+        chunk = Xd[:, :, pos:pos + c].contiguous()
+        tmp = torch.empty((nb, w.ndm, c), dtype=odt, device="cuda")
+        n = st.push(chunk, c, w.nchans * c, c, tmp, c, w.ndm * c)
+        pos += c
+        assert n == max(0, pos - ms) - emitted
+        out[:, :, emitted:emitted + n] = tmp[:, :, :n]
+        emitted += n
+    torch.cuda.synchronize()
+    assert emitted == w.nsamp
+    assert torch.equal(out, one)
+    for b in range(nb):
+        assert_parity(w, xs[b], one[b].cpu().numpy())
+    with pytest.raises(dd.DedispError) as e:
+        st.push(Xd, total, 0, max(chunks) + 1, out, w.nsamp, 0)
+    assert e.value.code == dd.DD_ERR_STATE
+    st.destroy(); plan.destroy()
+
+
+@pytest.mark.parametrize("dtype", ["f32", "u8"])
+def test_one_shot_and_host_calls(dtype):
+    import torch
+    w = small(2, 128, 48, 20000 + 11, dtype=dtype)
+    X, ms = make_case(w)
+    odt = np.float32 if dtype == "f32" else np.int32
+    Xd = torch.from_numpy(X).cuda()
+    Dd = torch.empty((w.ndm, w.nsamp), dtype=torch.float32 if dtype == "f32" else torch.int32, device="cuda")
+    f = dd.dd_dedisperse_f32 if dtype == "f32" else dd.dd_dedisperse_u8_i32
+    f(Xd, w.nchans, w.nsamp, w.fch1, w.foff, w.tsamp, w.dm_list, Dd)
+    D1 = Dd.cpu().numpy()
+    assert_parity(w, X, D1)
+    fh = dd.dd_dedisperse_f32_host if dtype == "f32" else dd.dd_dedisperse_u8_i32_host
+    D2 = np.full((w.ndm, w.nsamp), -7, dtype=odt)
+    fh(X, w.nchans, w.nsamp, w.fch1, w.foff, w.tsamp, w.dm_list, D2)      # pageable host memory
+    assert np.array_equal(D1, D2)
+    # pinned host memory through the plan form, twice (cached workspace)
+    plan = dd.Plan(dd_dtype(w), w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    Xp = torch.from_numpy(X).pin_memory()
+    Dp = torch.empty((w.ndm, w.nsamp), dtype=Dd.dtype).pin_memory()
+    for _ in range(2):
+        Dp.fill_(-7)
+        plan.execute_host(Xp, X.shape[1], Dp, w.nsamp, w.nsamp)
+        assert np.array_equal(Dp.numpy(), D1)
+    plan.destroy()
+
+
+# ------------------------------------------------------------------ full sizes, bench configuration
+
+def _full_size(idx):
+    import torch
+    w = synth.WORKLOADS[idx]
+    tab = oracle.shift_table(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    ms = int(tab.max())
+    X = synth.make_input(w, w.nsamp + ms)
+    for d, t0, width in synth.pulse_plan(w, 5):
+        synth.inject_pulse(X, t0, width, 0.25 if w.dtype == "f32" else 8, tab[d])
+    D = gpu_dedisperse(w, X, dd.DD_KERNEL_AUTO)        # the launch configuration bench.py times
+    assert_sampled_parity(w, X, D, n=100000, seed=idx)
+    assert_row_checksums(w, X, D, tab)
+    rows = sorted({0, w.ndm - 1, w.ndm // 2} | {d for d, _, _ in synth.pulse_plan(w, 5)})
+    assert_parity(w, X, D, rows=rows)
+    return w, X, D, tab
+
+
+def test_config2_full_size_sampled_rows_and_checksums():
+    # BASELINE.json configs[1] as benchmarked: 1024 ch x 1024 DMs x 2^17 samples, uint8 -> int32
+    w, X, D, tab = _full_size(2)
+    assert np.array_equal(D[0], X[:, :w.nsamp].sum(axis=0, dtype=np.int64).astype(np.int32))   # DM = 0 row
