@@ -171,7 +171,7 @@ def run_ours(args, w):
     odt = torch.float32 if w.dtype == "f32" else torch.int32
     plan = dd.Plan(dtype, w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
     if args.kernel:
-        plan.set_kernel({"generic": dd.DD_KERNEL_GENERIC, "window": dd.DD_KERNEL_WINDOW}[args.kernel])
+        plan.set_kernel({"generic": dd.DD_KERNEL_GENERIC, "tma": dd.DD_KERNEL_TMA}[args.kernel])
     ms = plan.max_shift()
     nb = w.nbeams
     in_stride = (w.nsamp + ms + 63) // 64 * 64
@@ -186,7 +186,7 @@ def run_ours(args, w):
     Xd = Xh.cuda()
     Dd = torch.empty((nb, w.ndm, out_stride), dtype=odt, device="cuda")
     stream = torch.cuda.Stream()
-    kern = plan.kernel_for(Xd, in_stride, w.nchans * in_stride, out_stride, w.ndm * out_stride)
+    kern = plan.kernel_for(Xd, in_stride, w.nchans * in_stride, Dd, out_stride, w.ndm * out_stride, w.nsamp, nb)
 
     streamer = None
     if w.nchunks > 1:
@@ -287,7 +287,7 @@ def run_ours(args, w):
             "data": "synthetic",
             "config": {"workload": w.name, "nbeams": nb, "nchans": w.nchans, "ndm": w.ndm,
                        "nsamp": w.nsamp, "maxshift": ms, "tsamp": w.tsamp, "fch1": w.fch1, "foff": w.foff,
-                       "kernel": {1: "generic", 2: "window"}.get(kern, str(kern)),
+                       "kernel": {1: "generic", 2: "tma"}.get(kern, str(kern)),
                        "parallelism": "beam-per-rank" if world > 1 else "single",
                        "l2": "X+D per step = %.0f MB > 126 MB L2 (no flush needed)" % (hbm_bytes / 1e6)},
             "real_time_factor": w.nsamp * w.tsamp / (ms_per_step * 1e-3),
@@ -320,7 +320,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); default 2 = configs[1]")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--kernel", default=None, choices=["generic", "window"])
+    ap.add_argument("--kernel", default=None, choices=["generic", "tma"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -16,7 +16,7 @@ from . import build as _build
 
 DD_OK, DD_ERR_BAD_ARG, DD_ERR_UNSUPPORTED, DD_ERR_NOMEM, DD_ERR_CUDA, DD_ERR_STATE = 0, -1, -2, -3, -4, -5
 DD_F32, DD_U8 = 0, 1
-DD_KERNEL_AUTO, DD_KERNEL_GENERIC, DD_KERNEL_WINDOW = 0, 1, 2
+DD_KERNEL_AUTO, DD_KERNEL_GENERIC, DD_KERNEL_TMA = 0, 1, 2
 
 _dp = C.POINTER(C.c_double)
 _vp = C.c_void_p
@@ -40,7 +40,7 @@ SIGNATURES = {
     "dd_plan_nchans": (C.c_int, [_vp]),
     "dd_plan_shift_table": (C.c_int, [_vp, _vp]),
     "dd_plan_set_kernel": (C.c_int, [_vp, C.c_int]),
-    "dd_plan_kernel_for": (C.c_int, [_vp, _vp, _i64, _i64, _i64, _i64]),
+    "dd_plan_kernel_for": (C.c_int, [_vp, _vp, _i64, _i64, _vp, _i64, _i64, _i64, C.c_int]),
     "dd_plan_launches_per_execute": (C.c_int, [_vp]),
     "dd_execute": (C.c_int, [_vp, _vp, _i64, _i64, _vp, _i64, _i64, _i64, C.c_int, _vp]),
     "dd_execute_host": (C.c_int, [_vp, _vp, _i64, _vp, _i64, _i64]),
@@ -184,9 +184,9 @@ class Plan:
     def set_kernel(self, kernel: int) -> None:
         _check(lib().dd_plan_set_kernel(self._h, kernel), "dd_plan_set_kernel")
 
-    def kernel_for(self, X, in_stride, in_beam_stride=0, out_stride=0, out_beam_stride=0) -> int:
-        return _check(lib().dd_plan_kernel_for(self._h, _ptr(X), in_stride, in_beam_stride, out_stride,
-                                               out_beam_stride), "dd_plan_kernel_for")
+    def kernel_for(self, X, in_stride, in_beam_stride, D, out_stride, out_beam_stride, nsamp_out, nbeams=1) -> int:
+        return _check(lib().dd_plan_kernel_for(self._h, _ptr(X), in_stride, in_beam_stride, _ptr(D), out_stride,
+                                               out_beam_stride, nsamp_out, nbeams), "dd_plan_kernel_for")
 
     def launches_per_execute(self) -> int:
         return _check(lib().dd_plan_launches_per_execute(self._h), "dd_plan_launches_per_execute")

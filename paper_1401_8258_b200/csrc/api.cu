@@ -167,7 +167,7 @@ int dd_plan_create(dd_plan** out, int dtype, int nchans, double fch1, double fof
             return cuda_fail("table upload", e);
         }
     }
-    rc = build_window_plan(p);
+    rc = build_tma_plan(p);
     if (rc != DD_OK) {
         dd_plan_destroy(p);
         return rc;
@@ -190,7 +190,7 @@ void dd_plan_destroy(dd_plan* p)
         if (w->s_out) cudaStreamDestroy(w->s_out);
         delete w;
     }
-    destroy_window_plan(p);
+    destroy_tma_plan(p);
     if (p->d_shift) cudaFree(p->d_shift);
     if (p->d_order) cudaFree(p->d_order);
     delete p;
@@ -216,29 +216,57 @@ int dd_plan_shift_table(const dd_plan* p, int32_t* host_out)
 int dd_plan_set_kernel(dd_plan* p, int kernel)
 {
     if (!p) return fail(DD_ERR_BAD_ARG, "plan is null");
-    if (kernel != DD_KERNEL_AUTO && kernel != DD_KERNEL_GENERIC && kernel != DD_KERNEL_WINDOW)
+    if (kernel != DD_KERNEL_AUTO && kernel != DD_KERNEL_GENERIC && kernel != DD_KERNEL_TMA)
         return fail(DD_ERR_BAD_ARG, "unknown kernel id");
-    if (kernel == DD_KERNEL_WINDOW && !window_plan_usable(p))
-        return fail(DD_ERR_UNSUPPORTED, "the register-window kernel does not take this plan");
+    if (kernel == DD_KERNEL_TMA && !tma_plan_usable(p))
+        return fail(DD_ERR_UNSUPPORTED, "the TMA-staged kernel does not take this plan (dtype or per-trial delay steps)");
     p->kernel_pref = kernel;
     return DD_OK;
 }
 
+static void fill_args(const dd_plan* p, ExecArgs* a, const void* X, int64_t in_stride, int64_t in_beam_stride,
+                      void* D, int64_t out_stride, int64_t out_beam_stride, int64_t nsamp_out, int nbeams,
+                      void* cuda_stream)
+{
+    a->X = X;
+    a->D = D;
+    a->in_stride = in_stride;
+    a->in_beam_stride = nbeams > 1 ? in_beam_stride : 0;
+    a->out_stride = out_stride;
+    a->out_beam_stride = nbeams > 1 ? out_beam_stride : 0;
+    a->nsamp_out = nsamp_out;
+    a->nbeams = nbeams;
+    a->nchans = p->nchans;
+    a->ndm = p->ndm;
+    a->d_shift = p->d_shift;
+    a->d_order = p->d_order;
+    a->stream = cuda_stream;
+}
+
+static int kernel_for(const dd_plan* p, const ExecArgs& a)
+{
+    if (p->kernel_pref == DD_KERNEL_GENERIC) return DD_KERNEL_GENERIC;
+    if (tma_plan_usable(p) && tma_args_ok(p, a)) return DD_KERNEL_TMA;
+    return DD_KERNEL_GENERIC;
+}
+
 int dd_plan_kernel_for(const dd_plan* p, const void* X, int64_t in_stride, int64_t in_beam_stride,
-                       int64_t out_stride, int64_t out_beam_stride)
+                       const void* D, int64_t out_stride, int64_t out_beam_stride, int64_t nsamp_out,
+                       int nbeams)
 {
     if (!p) return fail(DD_ERR_BAD_ARG, "plan is null");
-    if (p->kernel_pref == DD_KERNEL_GENERIC) return DD_KERNEL_GENERIC;
-    if (window_plan_usable(p) &&
-        window_args_ok(p, X, in_stride, in_beam_stride, out_stride, out_beam_stride))
-        return DD_KERNEL_WINDOW;
-    return DD_KERNEL_GENERIC;
+    if (nbeams < 1 || nsamp_out < 0) return fail(DD_ERR_BAD_ARG, "bad nbeams / nsamp_out");
+    ExecArgs a;
+    fill_args(p, &a, X, in_stride, in_beam_stride, const_cast<void*>(D), out_stride, out_beam_stride,
+              nsamp_out, nbeams, nullptr);
+    return kernel_for(p, a);
 }
 
 int dd_plan_launches_per_execute(const dd_plan* p)
 {
     if (!p) return fail(DD_ERR_BAD_ARG, "plan is null");
-    return 1;
+    // the TMA-staged path runs the byte-shift front end and the dedispersion kernel
+    return (p->kernel_pref != DD_KERNEL_GENERIC && tma_plan_usable(p)) ? 2 : 1;
 }
 
 int dd_execute(const dd_plan* p, const void* X, int64_t in_stride, int64_t in_beam_stride, void* D,
@@ -261,24 +289,12 @@ int dd_execute(const dd_plan* p, const void* X, int64_t in_stride, int64_t in_be
         return fail(DD_ERR_BAD_ARG, "int32 output must be 4-byte aligned");
 
     ExecArgs a;
-    a.X = X;
-    a.D = D;
-    a.in_stride = in_stride;
-    a.in_beam_stride = nbeams > 1 ? in_beam_stride : 0;
-    a.out_stride = out_stride;
-    a.out_beam_stride = nbeams > 1 ? out_beam_stride : 0;
-    a.nsamp_out = nsamp_out;
-    a.nbeams = nbeams;
-    a.nchans = p->nchans;
-    a.ndm = p->ndm;
-    a.d_shift = p->d_shift;
-    a.d_order = p->d_order;
-    a.stream = cuda_stream;
-
-    int k = dd_plan_kernel_for(p, X, in_stride, a.in_beam_stride, out_stride, a.out_beam_stride);
-    if (p->kernel_pref == DD_KERNEL_WINDOW && k != DD_KERNEL_WINDOW)
-        return fail(DD_ERR_UNSUPPORTED, "window kernel forced but pointers/strides are not 16-byte aligned");
-    if (k == DD_KERNEL_WINDOW) return launch_window(p, a);
+    fill_args(p, &a, X, in_stride, in_beam_stride, D, out_stride, out_beam_stride, nsamp_out, nbeams,
+              cuda_stream);
+    const int k = kernel_for(p, a);
+    if (p->kernel_pref == DD_KERNEL_TMA && k != DD_KERNEL_TMA)
+        return fail(DD_ERR_UNSUPPORTED, "TMA kernel forced but the output is not 16-byte aligned or the buffer is tiny");
+    if (k == DD_KERNEL_TMA) return launch_tma(p, a);
     return launch_generic(p->dtype, p->generic_kb, p->generic_spread, a);
 }
 

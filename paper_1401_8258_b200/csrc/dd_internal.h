@@ -33,7 +33,7 @@ int64_t host_max_shift(int nchans, double fch1, double foff, double tsamp, const
 // Largest s(d_last,c) - s(d_first,c) over all tiles of `kb` consecutive sorted DMs.
 int64_t max_tile_spread(const HostTable& t, int kb);
 
-// ---- kernel launchers (generic.cu / window.cu) ---------------------------------------------
+// ---- kernel launchers (generic.cu / tma_u8.cu) ---------------------------------------------
 struct ExecArgs {
     const void* X;
     void* D;
@@ -53,16 +53,15 @@ int launch_generic(int dtype, int kb, int max_spread, const ExecArgs& a);
 
 struct dd_plan;
 struct dd_host_ws;
-struct dd_window_plan;
+struct dd_tma_plan;
 
 namespace dd {
-// register-window kernel (window.cu): plan-time tables, eligibility, launch
-int build_window_plan(dd_plan* p);
-void destroy_window_plan(dd_plan* p);
-bool window_plan_usable(const dd_plan* p);
-bool window_args_ok(const dd_plan* p, const void* X, int64_t in_stride, int64_t in_beam_stride,
-                    int64_t out_stride, int64_t out_beam_stride);
-int launch_window(const dd_plan* p, const ExecArgs& a);
+// TMA-staged kernels (tma_u8.cu): plan-time tables, eligibility, launch
+int build_tma_plan(dd_plan* p);
+void destroy_tma_plan(dd_plan* p);
+bool tma_plan_usable(const dd_plan* p);
+bool tma_args_ok(const dd_plan* p, const ExecArgs& a);
+int launch_tma(const dd_plan* p, const ExecArgs& a);
 }  // namespace dd
 
 struct dd_plan {
@@ -76,6 +75,6 @@ struct dd_plan {
     int kernel_pref = DD_KERNEL_AUTO;
     int generic_kb = 1;
     int generic_spread = 0;
-    dd_window_plan* window = nullptr;   // null: the register-window kernel does not take this plan
+    dd_tma_plan* tma = nullptr;         // null: the TMA-staged kernels do not take this plan
     dd_host_ws* host_ws = nullptr;      // device buffers / streams cached by dd_execute_host
 };

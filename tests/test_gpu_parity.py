@@ -14,6 +14,7 @@ from _util import (assert_parity, assert_row_checksums, assert_sampled_parity, d
 pytestmark = pytest.mark.gpu
 
 KERNELS = [pytest.param(dd.DD_KERNEL_GENERIC, id="generic"), pytest.param(dd.DD_KERNEL_AUTO, id="auto")]
+# AUTO takes the TMA-staged kernel whenever the plan and the buffers allow it (uint8, 16-byte aligned D)
 
 
 @pytest.fixture(scope="module", autouse=True)
