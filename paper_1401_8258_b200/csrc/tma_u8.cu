@@ -3,7 +3,7 @@
 // What is computed is eq 2.1 exactly; how it is computed differs from the
 // thesis' Alg. 1 in the three places where that design is bound on sm_100a:
 //
-//  a2 staging   A block owns kKB = 32 consecutive (sorted) trials x kTB = 1024 output samples.
+//  a2 staging   A block owns kKB = 64 consecutive (sorted) trials x kTB = 1024 output samples.
 //               For every channel the "channel vector" X[c][t0+s(d0,c) .. +1024+spread) (eq 2.14,
 //               PAPER.md:945) is brought into shared memory by the TMA engine (cp.async.bulk,
 //               completion on an mbarrier) -- no SM instruction touches it.  The row start
@@ -14,21 +14,23 @@
 //               workspace.  A block stages, per channel, the 16-byte aligned window of each W_r;
 //               every trial then reads ALIGNED 32-bit words whatever its delay:
 //               copy (a & 3), word (a >> 2), a = (t0+s(d0,c)) mod 16 + s(d,c) - s(d0,c).
-//  a3 unpack    A 32-bit word carries four samples.  `w & 0x00ff00ff` and `prmt(w,0,0x4341)`
-//               split it into two words of two 16-bit lanes each: 2 ALU instructions per 4 samples.
-//  a4 accumulate  Two 32-bit adds accumulate the four samples in 16-bit lanes (one word of
-//               shared memory, 2 unpack and 2 add instructions per FOUR sample-adds, against
-//               1 + 2 + 1 per ONE in Alg. 1).  16-bit lanes hold 257 samples of 255, so the
-//               partial sums are flushed into the int32 output every kFlush = 256 channels.
+//  a3/a4 unpack + accumulate   A 32-bit word w carries four samples b0..b3.  Per word the SM
+//               issues one LDS and three arithmetic instructions for FOUR sample-adds (Alg. 1:
+//               1 + 2 + 1 per ONE):  A += w & 0x00ff00ff  (LOP3 + add: b0 and b2 in 16-bit lanes)
+//               and  C = hi32(w * 2^24) + C  (one IMAD.HI.U32: C += w >> 8 = b1 + 2^8 b2 + 2^16 b3).
+//               After n <= 256 channels  sum b0 = A & 0xffff,  sum b2 = A >> 16,  and
+//               C - 2^8 sum b2 = sum b1 + 2^16 sum b3  (C <= 65280 * 65793 < 2^32), so all four
+//               sums are recovered exactly; they are flushed into the int32 output every
+//               kFlush = 256 channels.
 //  a5 store     The flush is a 16-byte read-modify-write of D (plain store for the first one); a
-//               block's D tile (128 KB) stays in L2 between flushes.
+//               block's D tile (256 KB) stays in L2 between flushes.
 //
 // Channels are added in the order c = 0,1,2,... for every output element; integer arithmetic,
 // so the result is exact and independent of tiling.
 //
-// Roofline: per 4 sample-adds the SM issues 1 LDS + 2 ALU-pipe + 2 adds
-// (IADD3 on the ALU pipe or IMAD.IADD on the FMA pipe, 64 lanes/clk/SM each, measured): 5 issue
-// slots per 4 adds -> at most 102 sample-adds/clk/SM = 80 % of the 128 adds/clk/SM roofline.
+// Roofline: 4 issue slots per 4 sample-adds -> the issue rate (128 thread
+// instructions/clk/SM) allows 128 sample-adds/clk/SM, the same as the add roofline; the ALU and
+// FMA pipes (64 lanes/clk/SM each, measured) carry 2 and 1-2 of the 4 instructions.
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -47,14 +49,16 @@ namespace dd {
 
 namespace {
 
-constexpr int kConsumerWarps = 8;
-constexpr int kThreads = 32 * (kConsumerWarps + 1);   // + one producer warp
+constexpr int kConsumerWarps = 16;
+constexpr int kThreads = 32 * kConsumerWarps;         // 512: 128 registers per thread, one block per SM
 constexpr int kKW = 4;                                // trials per consumer warp
 constexpr int kKB = kKW * kConsumerWarps;             // trials per block
 constexpr int kNK = 8;                                // 32-bit words per lane (lane-interleaved)
 constexpr int kTB = 32 * 4 * kNK;                     // output samples per block
 constexpr int kCH = 4;                                // channels per pipeline stage
-constexpr int kStages = 4;
+constexpr int kStages = 8;
+constexpr int kLead = kStages - 1;                    // groups staged ahead (as early as a stage can be free)
+constexpr int kMust = 3;                              // ... and at the latest this many groups ahead
 constexpr int kFlush = 256;                           // 256 * 255 < 65536
 constexpr int kMaxNY = 8;
 constexpr int kBoxW = 256;                            // granule of the staged window length (bytes)
@@ -133,18 +137,39 @@ dd_shift_copies_u8(const uint8_t* __restrict__ X, uint8_t* __restrict__ W, int64
     }
 }
 
-// Adds 32 samples (8 lane-interleaved words) of one channel into the packed accumulators of one trial.
-__device__ __forceinline__ void accumulate_words(uint32_t (&ae)[kNK], uint32_t (&ao)[kNK], const uint8_t* src)
+// The 8 lane-interleaved words (32 samples) of one channel that one trial needs.
+__device__ __forceinline__ void load_words(uint32_t (&w)[kNK], uint32_t saddr)
+{
+#pragma unroll
+    for (int k = 0; k < kNK; ++k)
+        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(w[k]) : "r"(saddr + k * 128));
+}
+// Adds them into the accumulators of that trial: A holds b0,b2 in 16-bit lanes, C the running
+// sum of w >> 8 (see the header).
+__device__ __forceinline__ void add_words(uint32_t (&A)[kNK], uint32_t (&C)[kNK], const uint32_t (&w)[kNK])
 {
 #pragma unroll
     for (int k = 0; k < kNK; ++k) {
-        const uint32_t w = *reinterpret_cast<const uint32_t*>(src + k * 128);
-        ae[k] += w & 0x00ff00ffu;                    // samples 0 and 2 of the word
-        ao[k] += __byte_perm(w, 0u, 0x4341);         // samples 1 and 3
+        A[k] += w[k] & 0x00ff00ffu;
+        asm("mad.hi.u32 %0, %1, 0x01000000, %0;" : "+r"(C[k]) : "r"(w[k]));
     }
 }
+__device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity)
+{
+    uint32_t done;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(done)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return done != 0;
+}
 
-__global__ void __launch_bounds__(kThreads, 2)
+__global__ void __launch_bounds__(kThreads, 1)
 dd_tma_u8_kernel(const U8Params p)
 {
     extern __shared__ __align__(1024) uint8_t smem[];
@@ -152,7 +177,7 @@ dd_tma_u8_kernel(const U8Params p)
     const int chan_pitch = 4 * copy_pitch;
     const int stage_pitch = kCH * chan_pitch;
     uint8_t* rows = smem;                                                     // [kStages][kCH][4][ny*256]
-    int32_t* offs = reinterpret_cast<int32_t*>(smem + kStages * stage_pitch); // [kStages][kCH][kKB]
+    int32_t* offs = reinterpret_cast<int32_t*>(smem + kStages * stage_pitch); // [kStages][16 warps][kCH][kKW]
     uint64_t* full = reinterpret_cast<uint64_t*>(offs + kStages * kCH * kKB);
     uint64_t* empty = full + kStages;
 
@@ -172,51 +197,73 @@ dd_tma_u8_kernel(const U8Params p)
     }
     __syncthreads();
 
-    if (warp == kConsumerWarps) {
-        // ---------------------------------------------------------------- producer warp
-        const int d = min(d0 + lane, p.ndm - 1);
-        const uint8_t* wrow0 = p.W + (int64_t)beam * p.nchans * p.wpitch + t0;
-        for (int g = 0; g < ngroups; ++g) {
-            const int st = g % kStages;
-            if (g >= kStages) mbar_wait(&empty[st], ((g / kStages) - 1) & 1);
-            const int nch = min(kCH, p.nchans - g * kCH);
-            int s0v[kCH];
+    // Producer role, taken in turn by every warp (group gp is staged by warp gp mod 16, kLead
+    // groups ahead of its use): per channel the lanes write the trials' read offsets, then lane 0
+    // arms the stage's mbarrier and issues the four bulk copies.
+    const uint8_t* wrow0 = p.W + (int64_t)beam * p.nchans * p.wpitch + t0;
+    auto produce = [&](int gp) {
+        const int st = gp % kStages;
+        const int nch = min(kCH, p.nchans - gp * kCH);
+        int s0v[kCH];
+#pragma unroll
+        for (int ch = 0; ch < kCH; ++ch) {
+            s0v[ch] = 0;
+            if (ch < nch) {
+                const int c = gp * kCH + ch;
+                const int32_t* trow = p.shift_t + (int64_t)c * p.ndm_pad + d0;   // padded to whole tiles
+                int s[kKB / 32];
+#pragma unroll
+                for (int q = 0; q < kKB / 32; ++q) s[q] = __ldg(trow + lane + 32 * q);
+                const int s0 = __shfl_sync(0xffffffffu, s[0], 0);
+#pragma unroll
+                for (int q = 0; q < kKB / 32; ++q) {
+                    const int a = (s0 & 15) + s[q] - s0;                // t0 is a multiple of 16
+                    const int dl = lane + 32 * q;                       // trial within the tile
+                    offs[((st * kConsumerWarps + dl / kKW) * kCH + ch) * kKW + dl % kKW] =
+                        (a & 3) * copy_pitch + (a & ~3);
+                }
+                s0v[ch] = s0;
+            }
+        }
+        __syncwarp();
+        if (lane == 0) {
+            mbar_arrive_expect_tx(&full[st], (uint32_t)(nch * chan_pitch));
 #pragma unroll
             for (int ch = 0; ch < kCH; ++ch) {
-                s0v[ch] = 0;
                 if (ch < nch) {
-                    const int c = g * kCH + ch;
-                    const int s = __ldg(p.shift_t + (int64_t)c * p.ndm_pad + d);
-                    const int s0 = __shfl_sync(0xffffffffu, s, 0);
-                    const int a = (s0 & 15) + s - s0;                   // t0 is a multiple of 16
-                    offs[(st * kCH + ch) * kKB + lane] = (a & 3) * copy_pitch + (a & ~3);
-                    s0v[ch] = s0;
-                }
-            }
-            __syncwarp();
-            if (lane == 0) {
-                mbar_arrive_expect_tx(&full[st], (uint32_t)(nch * chan_pitch));
+                    const uint8_t* src = wrow0 + (int64_t)(gp * kCH + ch) * p.wpitch + (s0v[ch] & ~15);
+                    uint8_t* dst = rows + st * stage_pitch + ch * chan_pitch;
 #pragma unroll
-                for (int ch = 0; ch < kCH; ++ch) {
-                    if (ch < nch) {
-                        const uint8_t* src = wrow0 + (int64_t)(g * kCH + ch) * p.wpitch + (s0v[ch] & ~15);
-                        uint8_t* dst = rows + st * stage_pitch + ch * chan_pitch;
-#pragma unroll
-                        for (int r = 0; r < 4; ++r)
-                            bulk_load(dst + r * copy_pitch, src + r * p.wcopy, (uint32_t)copy_pitch, &full[st]);
-                    }
+                    for (int r = 0; r < 4; ++r)
+                        bulk_load(dst + r * copy_pitch, src + r * p.wcopy, (uint32_t)copy_pitch, &full[st]);
                 }
             }
         }
-        return;
-    }
+        __syncwarp();
+    };
+    // A warp whose turn it is stages the group as soon as the stage's previous users have all
+    // released it; until then it keeps consuming and polls (a blocked producer would stall every
+    // other warp one group later).  kMust groups before the data is needed it waits.
+    int pending = -1;
+    auto try_produce = [&](bool must) {
+        const int st = pending % kStages;
+        if (pending >= kStages) {
+            const uint32_t par = ((pending / kStages) - 1) & 1;
+            if (must) mbar_wait(&empty[st], par);
+            else if (!mbar_test(&empty[st], par)) return;
+        }
+        produce(pending);
+        pending = -1;
+    };
+    for (int gp = 0; gp < kLead && gp < ngroups; ++gp)
+        if (gp % kConsumerWarps == warp) produce(gp);
 
     // -------------------------------------------------------------------- consumer warps
-    uint32_t ae[kKW][kNK], ao[kKW][kNK];
+    uint32_t A[kKW][kNK], C[kKW][kNK];
 #pragma unroll
     for (int j = 0; j < kKW; ++j)
 #pragma unroll
-        for (int k = 0; k < kNK; ++k) ae[j][k] = ao[j][k] = 0;
+        for (int k = 0; k < kNK; ++k) A[j][k] = C[j][k] = 0;
 
     int32_t* Db = p.D + (int64_t)beam * p.out_beam_stride;
     int nflush = 0;
@@ -230,8 +277,9 @@ dd_tma_u8_kernel(const U8Params p)
 #pragma unroll
                 for (int k = 0; k < kNK; ++k) {
                     const int64_t t = t0 + 4 * (lane + 32 * k);
-                    int4 v = make_int4((int)(ae[j][k] & 0xffffu), (int)(ao[j][k] & 0xffffu),
-                                       (int)(ae[j][k] >> 16), (int)(ao[j][k] >> 16));
+                    const uint32_t b0 = A[j][k] & 0xffffu, b2 = A[j][k] >> 16;
+                    const uint32_t r = C[j][k] - (b2 << 8);               // sum b1 + 2^16 sum b3
+                    int4 v = make_int4((int)b0, (int)(r & 0xffffu), (int)b2, (int)(r >> 16));
                     if (t + 3 < p.nsamp) {
                         int4* q = reinterpret_cast<int4*>(drow + t);
                         if (nflush) {
@@ -248,27 +296,45 @@ dd_tma_u8_kernel(const U8Params p)
                 }
             }
 #pragma unroll
-            for (int k = 0; k < kNK; ++k) ae[j][k] = ao[j][k] = 0;
+            for (int k = 0; k < kNK; ++k) A[j][k] = C[j][k] = 0;
         }
         ++nflush;
     };
 
+    auto channel = [&](int st, int ch, const int4 o4) {
+        const uint32_t base = smem_u32(rows + st * stage_pitch + ch * chan_pitch + lane * 4);
+        // loads of the next trial are in flight while the current one is unpacked and added
+        uint32_t wa[kNK], wb[kNK];
+        load_words(wa, base + o4.x);
+        load_words(wb, base + o4.y);
+        add_words(A[0], C[0], wa);
+        load_words(wa, base + o4.z);
+        add_words(A[1], C[1], wb);
+        load_words(wb, base + o4.w);
+        add_words(A[2], C[2], wa);
+        add_words(A[3], C[3], wb);
+    };
+
     for (int g = 0; g < ngroups; ++g) {
+        if (g + kLead < ngroups && (g + kLead) % kConsumerWarps == warp) pending = g + kLead;
+        if (pending >= 0) try_produce(pending - g <= kMust);
         const int st = g % kStages;
         mbar_wait(&full[st], (g / kStages) & 1);
-        const int nch = min(kCH, p.nchans - g * kCH);
-        for (int ch = 0; ch < nch; ++ch) {
-            const int4 o4 = *reinterpret_cast<const int4*>(offs + (st * kCH + ch) * kKB + warp * kKW);
-            const uint8_t* base = rows + st * stage_pitch + ch * chan_pitch + lane * 4;
-            accumulate_words(ae[0], ao[0], base + o4.x);
-            accumulate_words(ae[1], ao[1], base + o4.y);
-            accumulate_words(ae[2], ao[2], base + o4.z);
-            accumulate_words(ae[3], ao[3], base + o4.w);
-            const int c1 = g * kCH + ch + 1;
-            if ((c1 & (kFlush - 1)) == 0 && c1 < p.nchans) flush();
+        const int4* o = reinterpret_cast<const int4*>(offs + (st * kConsumerWarps + warp) * kCH * kKW);
+        if (g * kCH + kCH <= p.nchans) {
+            const int4 o0 = o[0], o1 = o[1], o2 = o[2], o3 = o[3];
+            channel(st, 0, o0);
+            channel(st, 1, o1);
+            if (pending >= 0) try_produce(false);
+            channel(st, 2, o2);
+            channel(st, 3, o3);
+        } else {
+            for (int ch = 0; ch < p.nchans - g * kCH; ++ch) channel(st, ch, o[ch]);
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[st]);
+        const int c1 = (g + 1) * kCH;                                   // kFlush is a multiple of kCH
+        if ((c1 & (kFlush - 1)) == 0 && c1 < p.nchans) flush();
     }
     flush();
 }
