@@ -188,6 +188,7 @@ def run_ours(args, w):
     stream = torch.cuda.Stream()
     kern = plan.kernel_for(Xd, in_stride, w.nchans * in_stride, Dd, out_stride, w.ndm * out_stride, w.nsamp, nb)
 
+    lpe = plan.launches_per_execute()          # kernels per dd_execute (front end + main kernel)
     streamer = None
     if w.nchunks > 1:
         # config 5: fed through the streaming API: first push nsamp/nchunks + maxshift, then equal chunks
@@ -198,7 +199,7 @@ def run_ours(args, w):
         if streamer is None:
             plan.execute(Xd, in_stride, w.nchans * in_stride, Dd, out_stride, w.ndm * out_stride,
                          w.nsamp, nb, stream)
-            return 1
+            return lpe
         streamer.reset()
         pos = emitted = 0
         chunk = w.nsamp // w.nchunks
@@ -209,7 +210,7 @@ def run_ours(args, w):
             pos += n_new
             emitted += n
         assert emitted == w.nsamp
-        return w.nchunks
+        return w.nchunks * lpe
 
     def barrier():
         if dist is not None:
