@@ -171,7 +171,7 @@ def run_ours(args, w):
     odt = torch.float32 if w.dtype == "f32" else torch.int32
     plan = dd.Plan(dtype, w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
     if args.kernel:
-        plan.set_kernel({"generic": dd.DD_KERNEL_GENERIC, "tma": dd.DD_KERNEL_TMA}[args.kernel])
+        plan.set_kernel({"generic": dd.DD_KERNEL_GENERIC, "tma": dd.DD_KERNEL_TMA, "ps": dd.DD_KERNEL_PS}[args.kernel])
     ms = plan.max_shift()
     nb = w.nbeams
     in_stride = (w.nsamp + ms + 63) // 64 * 64
@@ -288,7 +288,7 @@ def run_ours(args, w):
             "data": "synthetic",
             "config": {"workload": w.name, "nbeams": nb, "nchans": w.nchans, "ndm": w.ndm,
                        "nsamp": w.nsamp, "maxshift": ms, "tsamp": w.tsamp, "fch1": w.fch1, "foff": w.foff,
-                       "kernel": {1: "generic", 2: "tma"}.get(kern, str(kern)),
+                       "kernel": {1: "generic", 2: "tma", 3: "ps"}.get(kern, str(kern)),
                        "parallelism": "beam-per-rank" if world > 1 else "single",
                        "l2": "X+D per step = %.0f MB > 126 MB L2 (no flush needed)" % (hbm_bytes / 1e6)},
             "real_time_factor": w.nsamp * w.tsamp / (ms_per_step * 1e-3),
@@ -321,7 +321,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); default 2 = configs[1]")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--kernel", default=None, choices=["generic", "tma"])
+    ap.add_argument("--kernel", default=None, choices=["generic", "tma", "ps"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -168,6 +168,7 @@ int dd_plan_create(dd_plan** out, int dtype, int nchans, double fch1, double fof
         }
     }
     rc = build_tma_plan(p);
+    if (rc == DD_OK) rc = build_ps_plan(p);
     if (rc != DD_OK) {
         dd_plan_destroy(p);
         return rc;
@@ -191,6 +192,7 @@ void dd_plan_destroy(dd_plan* p)
         delete w;
     }
     destroy_tma_plan(p);
+    destroy_ps_plan(p);
     if (p->d_shift) cudaFree(p->d_shift);
     if (p->d_order) cudaFree(p->d_order);
     delete p;
@@ -216,8 +218,11 @@ int dd_plan_shift_table(const dd_plan* p, int32_t* host_out)
 int dd_plan_set_kernel(dd_plan* p, int kernel)
 {
     if (!p) return fail(DD_ERR_BAD_ARG, "plan is null");
-    if (kernel != DD_KERNEL_AUTO && kernel != DD_KERNEL_GENERIC && kernel != DD_KERNEL_TMA)
+    if (kernel != DD_KERNEL_AUTO && kernel != DD_KERNEL_GENERIC && kernel != DD_KERNEL_TMA &&
+        kernel != DD_KERNEL_PS)
         return fail(DD_ERR_BAD_ARG, "unknown kernel id");
+    if (kernel == DD_KERNEL_PS && !ps_plan_usable(p))
+        return fail(DD_ERR_UNSUPPORTED, "the partial-sum kernel does not take this plan (dtype or per-trial delay steps)");
     if (kernel == DD_KERNEL_TMA && !tma_plan_usable(p))
         return fail(DD_ERR_UNSUPPORTED, "the TMA-staged kernel does not take this plan (dtype or per-trial delay steps)");
     p->kernel_pref = kernel;
@@ -247,6 +252,7 @@ static int kernel_for(const dd_plan* p, const ExecArgs& a)
 {
     if (p->kernel_pref == DD_KERNEL_GENERIC) return DD_KERNEL_GENERIC;
     if (tma_plan_usable(p) && tma_args_ok(p, a)) return DD_KERNEL_TMA;
+    if (ps_plan_usable(p) && ps_args_ok(p, a)) return DD_KERNEL_PS;
     return DD_KERNEL_GENERIC;
 }
 
@@ -265,7 +271,9 @@ int dd_plan_kernel_for(const dd_plan* p, const void* X, int64_t in_stride, int64
 int dd_plan_launches_per_execute(const dd_plan* p)
 {
     if (!p) return fail(DD_ERR_BAD_ARG, "plan is null");
-    // the TMA-staged path runs the byte-shift front end and the dedispersion kernel
+    // the TMA-staged uint8 path runs the byte-shift front end and the dedispersion kernel; the
+    // float32 partial-sum kernel reads 16-byte aligned input directly (one launch; two when the
+    // caller's buffer has to be re-pitched first)
     return (p->kernel_pref != DD_KERNEL_GENERIC && tma_plan_usable(p)) ? 2 : 1;
 }
 
@@ -294,7 +302,10 @@ int dd_execute(const dd_plan* p, const void* X, int64_t in_stride, int64_t in_be
     const int k = kernel_for(p, a);
     if (p->kernel_pref == DD_KERNEL_TMA && k != DD_KERNEL_TMA)
         return fail(DD_ERR_UNSUPPORTED, "TMA kernel forced but the output is not 16-byte aligned or the buffer is tiny");
+    if (p->kernel_pref == DD_KERNEL_PS && k != DD_KERNEL_PS)
+        return fail(DD_ERR_UNSUPPORTED, "partial-sum kernel forced but the grid does not fit");
     if (k == DD_KERNEL_TMA) return launch_tma(p, a);
+    if (k == DD_KERNEL_PS) return launch_ps(p, a);
     return launch_generic(p->dtype, p->generic_kb, p->generic_spread, a);
 }
 

@@ -54,6 +54,7 @@ int launch_generic(int dtype, int kb, int max_spread, const ExecArgs& a);
 struct dd_plan;
 struct dd_host_ws;
 struct dd_tma_plan;
+struct dd_ps_plan;
 
 namespace dd {
 // TMA-staged kernels (tma_u8.cu): plan-time tables, eligibility, launch
@@ -62,6 +63,13 @@ void destroy_tma_plan(dd_plan* p);
 bool tma_plan_usable(const dd_plan* p);
 bool tma_args_ok(const dd_plan* p, const ExecArgs& a);
 int launch_tma(const dd_plan* p, const ExecArgs& a);
+// float32 kernel with shared partial sums (ps_f32.cu)
+int build_ps_plan(dd_plan* p);
+void destroy_ps_plan(dd_plan* p);
+bool ps_plan_usable(const dd_plan* p);
+bool ps_args_ok(const dd_plan* p, const ExecArgs& a);
+int ps_launches(const dd_plan* p, const ExecArgs& a);
+int launch_ps(const dd_plan* p, const ExecArgs& a);
 }  // namespace dd
 
 struct dd_plan {
@@ -75,6 +83,7 @@ struct dd_plan {
     int kernel_pref = DD_KERNEL_AUTO;
     int generic_kb = 1;
     int generic_spread = 0;
-    dd_tma_plan* tma = nullptr;         // null: the TMA-staged kernels do not take this plan
+    dd_tma_plan* tma = nullptr;         // null: the TMA-staged uint8 kernel does not take this plan
+    dd_ps_plan* ps = nullptr;           // null: the float32 partial-sum kernel does not take this plan
     dd_host_ws* host_ws = nullptr;      // device buffers / streams cached by dd_execute_host
 };

@@ -1,0 +1,439 @@
+// float32 kernel with shared partial sums (SURVEY.md §8 rows a2, a4, a5, a6 for the float32 path).
+//
+// What is computed is eq 2.1 exactly: every output is the sum of the same
+// nchans operands.  How: a float32 word holds one sample, so the thesis' loop (Alg. 1,
+// one shared-memory read per add) is capped at 32 adds/clk/SM, a quarter of
+// the FP32 add rate.  Here the channels are taken in groups of kG = 4.  Within a tile of kKB
+// adjacent (sorted) trials the relative delays of a group,
+//     r_k(d) = s(d, c0+k) - s(d, c0),  k = 1..3,
+// take only a few distinct values ("patterns": 3-7 per tile on the BASELINE.json workloads,
+// because adjacent channels and adjacent trials differ by a fraction of a sample).  Per group a
+// block therefore
+//   1. has the four channel vectors (eq 2.14) in shared memory, copied there by the
+//      TMA engine (cp.async.bulk + mbarrier, three stages ahead);
+//   2. forms one row per pattern,  P[u] = ((x0[u] + x1[u+r1]) + x2[u+r2]) + x3[u+r3],  in shared
+//      memory (all warps, 32 consecutive u per warp step);
+//   3. adds, for every trial d and sample t of the tile, ONE word:  acc += P_{pattern(d)}[t + s(d,c0)].
+// Step 3 costs one shared-memory word per FOUR channel-adds; step 2 adds about (patterns / kKB)
+// * 5/4 words per channel-add.  Descriptors (windows, patterns, per-trial row offsets) are built on
+// the host at plan time from the exact delay table; nothing is approximated, and the order of
+// the additions depends only on the plan (groups in ascending channel order, inside a group the
+// expression above), never on the tile, so batch / streaming / one-shot results are identical.
+//
+// Layout of a block: 16 warps; warp w owns trials w*kKW .. w*kKW+kKW-1 of the tile, lane l owns
+// the output samples t0 + l + 32 i, i < kNK (accumulators acc[kKW][kNK] in registers,
+// PAPER.md:958).  D is written once with 128-byte coalesced warp stores.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <new>
+#include <vector>
+
+#include "dd_internal.h"
+
+struct dd_ps_plan {
+    bool ok = false;
+    int ntiles = 0, ngroups = 0;
+    int desc_ints = 0;             // ints per (tile, group) descriptor (multiple of 4)
+    int rmax = 0;                  // pattern rows per descriptor
+    int xw = 0;                    // words per staged channel vector
+    int psw = 0;                   // words of one partial-sum buffer
+    size_t smem = 0;
+    int32_t* d_desc = nullptr;     // device [ntiles][ngroups][desc_ints]
+};
+
+namespace dd {
+
+namespace {
+
+constexpr int kG = 4;                     // channels per group
+constexpr int kWarps = 16;
+constexpr int kThreads = 32 * kWarps;
+constexpr int kKW = 4;                    // trials per warp
+constexpr int kKB = kKW * kWarps;         // trials per block
+constexpr int kNK = 16;                   // output samples per lane
+constexpr int kTB = 32 * kNK;             // output samples per block
+constexpr int kXStages = 3;
+constexpr int kMaxSmem = 200 * 1024;
+
+// descriptor layout (ints)
+constexpr int kDNRows = 0, kDNChan = 1, kDNChunks = 2;
+constexpr int kDBase = 4;                 // [4]  first staged word of channel k, relative to t0 (multiple of 4)
+constexpr int kDLen = 8;                  // [4]  words to stage (multiple of 4)
+constexpr int kDRows = 12;                // per row: end (flat words, multiple of 32), qf[4]
+constexpr int kDRowInts = 5;
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+        ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+
+struct PsParams {
+    const float* X;
+    float* D;
+    const int32_t* desc;
+    const int32_t* order;
+    int nchans, ndm, ngroups, desc_ints, rmax, xw, psw;
+    int64_t nsamp, row_valid;      // row_valid: words of a channel row that may be read (multiple of 4)
+    int64_t in_stride, in_beam_stride, out_stride, out_beam_stride;
+};
+
+__global__ void __launch_bounds__(kThreads, 1)
+dd_ps_f32_kernel(const PsParams p)
+{
+    extern __shared__ __align__(128) uint8_t smem_raw[];
+    float* Xs = reinterpret_cast<float*>(smem_raw);                            // [kXStages][kG][xw]
+    float* Ps = Xs + kXStages * kG * p.xw;                                     // [2][psw]
+    int32_t* Ds = reinterpret_cast<int32_t*>(Ps + 2 * p.psw);                  // [kXStages][desc_ints]
+    uint64_t* full = reinterpret_cast<uint64_t*>(Ds + kXStages * p.desc_ints); // [kXStages]
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int tile = blockIdx.x;                          // trial tiles fastest: neighbours share L2 lines
+    const int64_t t0 = (int64_t)blockIdx.y * kTB;
+    const int beam = blockIdx.z;
+    const int ng = p.ngroups;
+    const int trial_off = kDRows + kDRowInts * p.rmax;    // per-trial flat offsets start here
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kXStages; ++s) mbar_init(&full[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+
+    const int32_t* gdesc = p.desc + (int64_t)tile * ng * p.desc_ints;
+    const float* Xb = p.X + (int64_t)beam * p.in_beam_stride + t0;
+
+    // Producer (warp 0): lane k < 4 stages channel k of the group, lane 4 the descriptor.
+    auto produce = [&](int g) {
+        const int st = g % kXStages;
+        const int32_t* dg = gdesc + (int64_t)g * p.desc_ints;
+        int base = 0, len = 0;
+        if (lane < kG) {
+            base = __ldg(dg + kDBase + lane);
+            len = __ldg(dg + kDLen + lane);
+            // the last time tile must not read past the row
+            const int64_t room = p.row_valid - (t0 + base);
+            len = (int)max((int64_t)0, min((int64_t)len, room));
+        }
+        uint32_t bytes = lane < kG ? (uint32_t)len * 4u : (lane == kG ? (uint32_t)p.desc_ints * 4u : 0u);
+        uint32_t total = bytes;
+#pragma unroll
+        for (int o = 4; o >= 1; o >>= 1) total += __shfl_xor_sync(0xffffffffu, total, o);   // lanes 0..7
+        if (lane == 0) mbar_arrive_expect_tx(&full[st], total);
+        __syncwarp();
+        if (lane < kG) {
+            if (len > 0) {
+                const int c = g * kG + lane;
+                bulk_load(Xs + (st * kG + lane) * p.xw, Xb + (int64_t)c * p.in_stride + base, bytes, &full[st]);
+            }
+        } else if (lane == kG) {
+            bulk_load(Ds + st * p.desc_ints, dg, bytes, &full[st]);
+        }
+    };
+
+    // Step 2: the pattern rows of group g into partial-sum buffer `buf`.
+    auto pre = [&](int g, int buf) {
+        const int st = g % kXStages;
+        const int32_t* ds = Ds + st * p.desc_ints;
+        const float* xs = Xs + st * kG * p.xw;
+        float* ps = Ps + buf * p.psw;
+        const int nchunks = ds[kDNChunks], nk = ds[kDNChan];
+        int rho = 0;
+        const int32_t* rd = ds + kDRows;
+        for (int cidx = warp; cidx < nchunks; cidx += kWarps) {
+            const int pos = cidx * 32;
+            while (pos >= rd[0]) { rd += kDRowInts; ++rho; }         // rows are contiguous, 32-padded
+            const int e = pos + lane;
+            float v = xs[rd[1] + e];
+            if (nk > 1) v += xs[p.xw + rd[2] + e];
+            if (nk > 2) v += xs[2 * p.xw + rd[3] + e];
+            if (nk > 3) v += xs[3 * p.xw + rd[4] + e];
+            ps[e] = v;
+        }
+        (void)rho;
+    };
+
+    float acc[kKW][kNK];
+#pragma unroll
+    for (int j = 0; j < kKW; ++j)
+#pragma unroll
+        for (int i = 0; i < kNK; ++i) acc[j][i] = 0.0f;
+
+    if (warp == 0)
+        for (int g = 0; g < kXStages && g < ng; ++g) produce(g);
+    mbar_wait(&full[0], 0);
+    pre(0, 0);
+    __syncthreads();
+
+    for (int g = 0; g < ng; ++g) {
+        if (g + 1 < ng) {
+            mbar_wait(&full[(g + 1) % kXStages], ((g + 1) / kXStages) & 1);
+            pre(g + 1, (g + 1) & 1);
+        }
+        // Step 3
+        const int32_t* tr = Ds + (g % kXStages) * p.desc_ints + trial_off + warp * kKW;
+        const float* ps = Ps + (g & 1) * p.psw + lane;
+#pragma unroll
+        for (int j = 0; j < kKW; ++j) {
+            const float* r = ps + tr[j];
+#pragma unroll
+            for (int i = 0; i < kNK; ++i) acc[j][i] += r[32 * i];
+        }
+        __syncthreads();
+        if (warp == 0 && g + kXStages < ng) produce(g + kXStages);
+    }
+
+    float* Db = p.D + (int64_t)beam * p.out_beam_stride;
+#pragma unroll
+    for (int j = 0; j < kKW; ++j) {
+        const int d = tile * kKB + warp * kKW + j;
+        if (d < p.ndm) {
+            float* drow = Db + (int64_t)__ldg(p.order + d) * p.out_stride + t0 + lane;
+#pragma unroll
+            for (int i = 0; i < kNK; ++i)
+                if (t0 + lane + 32 * i < p.nsamp) drow[32 * i] = acc[j][i];
+        }
+    }
+}
+
+// 2-D copy of the valid part of every row into a 16-byte aligned, padded workspace (used when the
+// caller's X is not 16-byte aligned or its strides are not multiples of four elements)
+__global__ void __launch_bounds__(256)
+dd_repitch_f32(const float* __restrict__ X, float* __restrict__ W, int nchans, int64_t rowlen, int64_t in_stride,
+               int64_t in_beam_stride, int64_t wpitch)
+{
+    const int64_t row = blockIdx.y;
+    const float* src = X + (row / nchans) * in_beam_stride + (row % nchans) * in_stride;
+    float* dst = W + row * wpitch;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < wpitch; i += (int64_t)gridDim.x * blockDim.x)
+        dst[i] = i < rowlen ? src[i] : 0.0f;
+}
+
+}  // namespace
+
+int build_ps_plan(dd_plan* p)
+{
+    p->ps = nullptr;
+    if (p->ndm == 0 || p->dtype != DD_F32) return DD_OK;
+    const HostTable& h = p->host;
+    const int nch = p->nchans, ndm = p->ndm;
+    const int ntiles = (ndm + kKB - 1) / kKB, ngroups = (nch + kG - 1) / kG;
+    const int64_t spread = max_tile_spread(h, kKB);
+    const int64_t xw64 = (kTB + spread + 3 + 3) / 4 * 4 + 32;
+    if (xw64 > 16384) return DD_OK;                      // per-trial steps too large: generic kernel
+
+    struct Row { int key[kG - 1]; int umin, umax; };
+    // pass 1: the largest number of pattern rows and partial-sum words of any (tile, group)
+    // pass 2: fill.  Both passes run the same classification.
+    std::vector<Row> rows;
+    std::vector<int> slot(kKB);
+    auto classify = [&](int tile, int g) {
+        rows.clear();
+        const int c0 = g * kG, nk = std::min(kG, nch - c0);
+        for (int j = 0; j < kKB; ++j) {
+            const int d = std::min(tile * kKB + j, ndm - 1);
+            const int32_t* s = &h.shift[(size_t)d * nch + c0];
+            int key[kG - 1] = {0, 0, 0};
+            for (int k = 1; k < nk; ++k) key[k - 1] = s[k] - s[0];
+            int r = 0;
+            for (; r < (int)rows.size(); ++r)
+                if (rows[r].key[0] == key[0] && rows[r].key[1] == key[1] && rows[r].key[2] == key[2]) break;
+            if (r == (int)rows.size()) rows.push_back(Row{{key[0], key[1], key[2]}, s[0], s[0]});
+            rows[r].umin = std::min(rows[r].umin, s[0]);
+            rows[r].umax = std::max(rows[r].umax, s[0]);
+            slot[j] = r;
+        }
+    };
+    int rmax = 1;
+    int64_t psw = 0;
+    for (int tile = 0; tile < ntiles; ++tile)
+        for (int g = 0; g < ngroups; ++g) {
+            classify(tile, g);
+            rmax = std::max(rmax, (int)rows.size());
+            int64_t w = 0;
+            for (const Row& r : rows) w += ((int64_t)r.umax - r.umin + kTB + 31) / 32 * 32;
+            psw = std::max(psw, w);
+        }
+    const int desc_ints = (kDRows + kDRowInts * rmax + kKB + 3) / 4 * 4;
+    const size_t smem = (size_t)kXStages * kG * xw64 * 4 + (size_t)2 * psw * 4 + (size_t)kXStages * desc_ints * 4 +
+                        kXStages * 8;
+    if (smem > (size_t)kMaxSmem) return DD_OK;            // too many patterns for shared memory: generic kernel
+
+    dd_ps_plan* t = new (std::nothrow) dd_ps_plan;
+    if (!t) return fail(DD_ERR_NOMEM, "ps plan allocation failed");
+    p->ps = t;
+    t->ntiles = ntiles;
+    t->ngroups = ngroups;
+    t->desc_ints = desc_ints;
+    t->rmax = rmax;
+    t->xw = (int)xw64;
+    t->psw = (int)psw;
+    t->smem = smem;
+
+    std::vector<int32_t> desc;
+    try {
+        desc.assign((size_t)ntiles * ngroups * desc_ints, 0);
+    } catch (const std::bad_alloc&) {
+        destroy_ps_plan(p);
+        return fail(DD_ERR_NOMEM, "ps descriptor allocation failed");
+    }
+    for (int tile = 0; tile < ntiles; ++tile)
+        for (int g = 0; g < ngroups; ++g) {
+            classify(tile, g);
+            int32_t* ds = &desc[((size_t)tile * ngroups + g) * desc_ints];
+            const int c0 = g * kG, nk = std::min(kG, nch - c0);
+            const int dfirst = tile * kKB, dlast = std::min(tile * kKB + kKB, ndm) - 1;
+            int base[kG] = {0, 0, 0, 0};
+            for (int k = 0; k < nk; ++k) {
+                const int smin = h.shift[(size_t)dfirst * nch + c0 + k], smax = h.shift[(size_t)dlast * nch + c0 + k];
+                base[k] = smin & ~3;
+                ds[kDBase + k] = base[k];
+                ds[kDLen + k] = (smax + kTB - base[k] + 3) / 4 * 4;
+            }
+            ds[kDNRows] = (int)rows.size();
+            ds[kDNChan] = nk;
+            int flat = 0;
+            std::vector<int> rowbase(rows.size());
+            for (size_t r = 0; r < rows.size(); ++r) {
+                rowbase[r] = flat;
+                const int ulen = rows[r].umax - rows[r].umin + kTB;
+                int32_t* rd = ds + kDRows + kDRowInts * r;
+                // element e of the flat buffer (rowbase <= e < end) is u = umin + (e - rowbase); channel k
+                // supplies x_k[u + r_k], staged at word (u + r_k - base_k) of its vector
+                for (int k = 0; k < kG; ++k) {
+                    const int rk = k == 0 ? 0 : rows[r].key[k - 1];
+                    rd[1 + k] = k < nk ? rows[r].umin + rk - base[k] - flat : 0;
+                }
+                flat += (ulen + 31) / 32 * 32;
+                rd[0] = flat;
+            }
+            for (size_t r = rows.size(); r < (size_t)rmax; ++r) ds[kDRows + kDRowInts * r] = 0x7fffffff;
+            ds[kDNChunks] = flat / 32;
+            for (int j = 0; j < kKB; ++j) {
+                const int d = std::min(tile * kKB + j, ndm - 1);
+                const int s0 = h.shift[(size_t)d * nch + c0];
+                ds[kDRows + kDRowInts * rmax + j] = rowbase[slot[j]] + (s0 - rows[slot[j]].umin);
+            }
+        }
+    cudaError_t e = cudaMalloc(&t->d_desc, desc.size() * sizeof(int32_t));
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        destroy_ps_plan(p);
+        return fail(DD_ERR_NOMEM, std::string("ps descriptor table: ") + cudaGetErrorString(e));
+    }
+    e = cudaMemcpy(t->d_desc, desc.data(), desc.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        destroy_ps_plan(p);
+        return fail(DD_ERR_CUDA, std::string("ps descriptor upload: ") + cudaGetErrorString(e));
+    }
+    e = cudaFuncSetAttribute(dd_ps_f32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return DD_OK;                                     // stays unusable; generic kernel serves
+    }
+    t->ok = true;
+    return DD_OK;
+}
+
+void destroy_ps_plan(dd_plan* p)
+{
+    if (!p->ps) return;
+    if (p->ps->d_desc) cudaFree(p->ps->d_desc);
+    delete p->ps;
+    p->ps = nullptr;
+}
+
+bool ps_plan_usable(const dd_plan* p) { return p->ps && p->ps->ok; }
+
+bool ps_args_ok(const dd_plan* p, const ExecArgs& a)
+{
+    if (!ps_plan_usable(p)) return false;
+    if ((a.nsamp_out + kTB - 1) / kTB > 65535 || a.nbeams > 65535) return false;
+    if ((int64_t)a.nbeams * p->nchans > 65535) return false;          // grid.y of the re-pitch copy
+    return true;
+}
+
+static bool ps_direct(const ExecArgs& a)
+{
+    return (((uintptr_t)a.X & 15) == 0) && (a.in_stride & 3) == 0 && (a.nbeams == 1 || (a.in_beam_stride & 3) == 0);
+}
+
+int ps_launches(const dd_plan* p, const ExecArgs& a) { return ps_direct(a) ? 1 : 2; }
+
+int launch_ps(const dd_plan* p, const ExecArgs& a)
+{
+    const dd_ps_plan* t = p->ps;
+    cudaStream_t st = (cudaStream_t)a.stream;
+    const int64_t rowlen = a.nsamp_out + p->host.maxshift;
+    PsParams q;
+    q.X = (const float*)a.X;
+    q.in_stride = a.in_stride;
+    q.in_beam_stride = a.in_beam_stride;
+    q.row_valid = (rowlen + 3) / 4 * 4;
+    float* W = nullptr;
+    if (!ps_direct(a)) {
+        const int64_t wpitch = (rowlen + 3) / 4 * 4;
+        const int64_t nrows = (int64_t)a.nbeams * p->nchans;
+        cudaError_t e = cudaMallocAsync((void**)&W, (size_t)(nrows * wpitch) * sizeof(float), st);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            return fail(DD_ERR_NOMEM, std::string("re-pitch workspace: ") + cudaGetErrorString(e));
+        }
+        dim3 grid((unsigned)std::min<int64_t>((wpitch + 255) / 256, 64), (unsigned)nrows);
+        dd_repitch_f32<<<grid, 256, 0, st>>>((const float*)a.X, W, p->nchans, rowlen, a.in_stride, a.in_beam_stride,
+                                             wpitch);
+        q.X = W;
+        q.in_stride = wpitch;
+        q.in_beam_stride = (int64_t)p->nchans * wpitch;
+    }
+    q.D = (float*)a.D;
+    q.desc = t->d_desc;
+    q.order = a.d_order;
+    q.nchans = p->nchans;
+    q.ndm = p->ndm;
+    q.ngroups = t->ngroups;
+    q.desc_ints = t->desc_ints;
+    q.rmax = t->rmax;
+    q.xw = t->xw;
+    q.psw = t->psw;
+    q.nsamp = a.nsamp_out;
+    q.out_stride = a.out_stride;
+    q.out_beam_stride = a.out_beam_stride;
+    dim3 grid((unsigned)t->ntiles, (unsigned)((a.nsamp_out + kTB - 1) / kTB), (unsigned)a.nbeams);
+    dd_ps_f32_kernel<<<grid, kThreads, t->smem, st>>>(q);
+    cudaError_t e = cudaGetLastError();
+    if (W) cudaFreeAsync(W, st);
+    if (e != cudaSuccess) return fail(DD_ERR_CUDA, std::string("ps f32 launch: ") + cudaGetErrorString(e));
+    return DD_OK;
+}
+
+}  // namespace dd

@@ -14,7 +14,8 @@ from _util import (assert_parity, assert_row_checksums, assert_sampled_parity, d
 pytestmark = pytest.mark.gpu
 
 KERNELS = [pytest.param(dd.DD_KERNEL_GENERIC, id="generic"), pytest.param(dd.DD_KERNEL_AUTO, id="auto")]
-# AUTO takes the TMA-staged kernel whenever the plan and the buffers allow it (uint8, 16-byte aligned D)
+# AUTO takes the TMA-staged kernel for uint8 whenever the plan and the buffers allow it (16-byte aligned D)
+# and the partial-sum kernel for float32 (through a re-pitched copy when X is not 16-byte aligned)
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -264,6 +265,58 @@ def test_one_shot_and_host_calls(dtype):
         plan.execute_host(Xp, X.shape[1], Dp, w.nsamp, w.nsamp)
         assert np.array_equal(Dp.numpy(), D1)
     plan.destroy()
+
+
+# ------------------------------------------------------------------ float32 partial-sum kernel, direct (aligned) path
+
+@pytest.mark.parametrize("idx,nchans,ndm,nsamp", [(3, 517, 130, 2000), (4, 64, 200, 1500), (1, 64, 32, 8192)])
+def test_ps_kernel_reads_aligned_input_directly(idx, nchans, ndm, nsamp):
+    """16-byte aligned X with strides that are multiples of four elements is staged by TMA straight from
+    the caller's buffer (no re-pitch copy): several DM tiles, several time tiles, ragged tails, a
+    channel count that is not a multiple of the group size."""
+    import torch
+    w = small(idx, nchans, ndm, nsamp, dtype="f32")
+    X, ms = make_case(w, pulses=2)
+    stride = (w.nsamp + ms + 63) // 64 * 64
+    plan = dd.Plan(dd.DD_F32, w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    Xd = torch.zeros((w.nchans, stride), dtype=torch.float32, device="cuda")
+    Xd[:, :w.nsamp + ms] = torch.from_numpy(X).cuda()
+    Dd = torch.full((w.ndm, w.nsamp), -7.0, dtype=torch.float32, device="cuda")
+    assert plan.kernel_for(Xd, stride, 0, Dd, w.nsamp, 0, w.nsamp, 1) == dd.DD_KERNEL_PS
+    plan.execute(Xd, stride, 0, Dd, w.nsamp, 0, w.nsamp, 1)
+    torch.cuda.synchronize()
+    D = Dd.cpu().numpy()
+    assert_parity(w, X, D)
+    # forced generic kernel on the same plan: both within tolerance of the oracle, and the
+    # partial-sum result does not depend on the path the input took (re-pitched copy vs direct)
+    D2 = gpu_dedisperse(w, X, dd.DD_KERNEL_PS)
+    assert np.array_equal(D, D2)
+    plan.destroy()
+
+
+def test_config3_channels_and_trials_full_time_cut():
+    # BASELINE.json configs[2] in the launch configuration bench.py times (4096 ch x 4096 DMs, float32,
+    # partial-sum kernel, aligned direct path), cut to 8192 samples: sampled elements + whole rows
+    import torch
+    w = synth.scaled(synth.WORKLOADS[3], nsamp=8192)
+    tab = oracle.shift_table(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    ms = int(tab.max())
+    X = synth.make_input(w, w.nsamp + ms)
+    for d, t0, width in synth.pulse_plan(w, 5):
+        synth.inject_pulse(X, t0, width, 0.25, tab[d])
+    stride = (w.nsamp + ms + 63) // 64 * 64
+    plan = dd.Plan(dd.DD_F32, w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    Xd = torch.zeros((w.nchans, stride), dtype=torch.float32, device="cuda")
+    Xd[:, :w.nsamp + ms] = torch.from_numpy(X).cuda()
+    Dd = torch.empty((w.ndm, w.nsamp), dtype=torch.float32, device="cuda")
+    assert plan.kernel_for(Xd, stride, 0, Dd, w.nsamp, 0, w.nsamp, 1) == dd.DD_KERNEL_PS
+    plan.execute(Xd, stride, 0, Dd, w.nsamp, 0, w.nsamp, 1)
+    torch.cuda.synchronize()
+    D = Dd.cpu().numpy()
+    plan.destroy()
+    assert_sampled_parity(w, X, D, n=100000, seed=3)
+    rows = sorted({0, w.ndm - 1, w.ndm // 2, 63, 64} | {d for d, _, _ in synth.pulse_plan(w, 5)})
+    assert_parity(w, X, D, rows=rows)
 
 
 # ------------------------------------------------------------------ full sizes, bench configuration
