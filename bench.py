@@ -323,9 +323,13 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--kernel", default=None, choices=["generic", "tma", "ps"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--nsamp", type=int, default=0,
+                    help="profiling aid: cut the workload to this many output samples (the line then names it)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     w = synth.WORKLOADS[args.config]
+    if args.nsamp:
+        w = synth.scaled(w, nsamp=args.nsamp, name="%s_cut_to_%d_samples" % (w.name, args.nsamp))
     if args.impl == "reference":
         run_reference(args, w)
     else:

@@ -3,7 +3,8 @@
 // What is computed is eq 2.1 exactly: every output is the sum of the same
 // nchans operands.  How: a float32 word holds one sample, so the thesis' loop (Alg. 1,
 // one shared-memory read per add) is capped at 32 adds/clk/SM, a quarter of
-// the FP32 add rate.  Here the channels are taken in groups of kG = 4.  Within a tile of kKB
+// the FP32 add rate.  Here the channels are taken in groups of G = 4 or 8 (chosen per plan by a
+// cost model; the text below writes G = 4).  Within a tile of kKB
 // adjacent (sorted) trials the relative delays of a group,
 //     r_k(d) = s(d, c0+k) - s(d, c0),  k = 1..3,
 // take only a few distinct values ("patterns": 3-7 per tile on the BASELINE.json workloads,
@@ -12,7 +13,7 @@
 //   1. has the four channel vectors (eq 2.14) in shared memory, copied there by the
 //      TMA engine (cp.async.bulk + mbarrier, three stages ahead);
 //   2. forms one row per pattern,  P[u] = ((x0[u] + x1[u+r1]) + x2[u+r2]) + x3[u+r3],  in shared
-//      memory (all warps, 32 consecutive u per warp step);
+//      memory (all warps, 64 consecutive u per warp step);
 //   3. adds, for every trial d and sample t of the tile, ONE word:  acc += P_{pattern(d)}[t + s(d,c0)].
 // Step 3 costs one shared-memory word per FOUR channel-adds; step 2 adds about (patterns / kKB)
 // * 5/4 words per channel-add.  Descriptors (windows, patterns, per-trial row offsets) are built on
@@ -34,8 +35,8 @@
 struct dd_ps_plan {
     bool ok = false;
     int ntiles = 0, ngroups = 0;
+    int G = 4;                     // channels per group
     int desc_ints = 0;             // ints per (tile, group) descriptor (multiple of 4)
-    int rmax = 0;                  // pattern rows per descriptor
     int xw = 0;                    // words per staged channel vector
     int psw = 0;                   // words of one partial-sum buffer
     size_t smem = 0;
@@ -46,7 +47,7 @@ namespace dd {
 
 namespace {
 
-constexpr int kG = 4;                     // channels per group
+constexpr int kGMax = 8;                  // channels per group: 4 or 8
 constexpr int kWarps = 16;
 constexpr int kThreads = 32 * kWarps;
 constexpr int kKW = 4;                    // trials per warp
@@ -56,17 +57,24 @@ constexpr int kTB = 32 * kNK;             // output samples per block
 constexpr int kXStages = 3;
 constexpr int kMaxSmem = 200 * 1024;
 
-// descriptor layout (ints)
-constexpr int kDNRows = 0, kDNChan = 1, kDNChunks = 2;
-constexpr int kDBase = 4;                 // [4]  first staged word of channel k, relative to t0 (multiple of 4)
-constexpr int kDLen = 8;                  // [4]  words to stage (multiple of 4)
-constexpr int kDRows = 12;                // per row: end (flat words, multiple of 32), qf[4]
-constexpr int kDRowInts = 5;
+// descriptor layout (ints), one per (trial tile, channel group)
+constexpr int kChunk = 64;                // words of a partial-sum row formed per warp step
+constexpr int kDNChunks = 0;              // kChunk-word steps of the partial-sum phase
+constexpr int kDBytes = 1;                // bytes of this descriptor that are in use (multiple of 16)
+constexpr int kDBase = 4;                 // [8]  first staged word of channel k, relative to t0 (multiple of 4)
+constexpr int kDLen = 12;                 // [8]  words to stage (multiple of 4; 0 for a missing channel)
+constexpr int kDTrial = 20;               // [kKB] flat word offset of trial j's first operand in the partial sums
+constexpr int kDChunk = kDTrial + kKB;    // [nchunks][G] byte offset, from the stage's first staged word, of
+                                          //      the operand of lane 0 in channel k (zero pad if missing)
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
 {
@@ -95,91 +103,119 @@ __device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t b
         ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar))
         : "memory");
 }
+__device__ __forceinline__ void consumer_barrier()
+{
+    asm volatile("bar.sync 1, %0;" ::"n"(kThreads) : "memory");
+}
+__device__ __forceinline__ float lds_f32(uint32_t addr)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
 
 struct PsParams {
     const float* X;
     float* D;
     const int32_t* desc;
     const int32_t* order;
-    int nchans, ndm, ngroups, desc_ints, rmax, xw, psw;
+    int nchans, ndm, ngroups, desc_ints, xw, psw;
     int64_t nsamp, row_valid;      // row_valid: words of a channel row that may be read (multiple of 4)
     int64_t in_stride, in_beam_stride, out_stride, out_beam_stride;
 };
 
-__global__ void __launch_bounds__(kThreads, 1)
+template <int G>
+__global__ void __launch_bounds__(kThreads + 32, 1)
 dd_ps_f32_kernel(const PsParams p)
 {
     extern __shared__ __align__(128) uint8_t smem_raw[];
-    float* Xs = reinterpret_cast<float*>(smem_raw);                            // [kXStages][kG][xw]
-    float* Ps = Xs + kXStages * kG * p.xw;                                     // [2][psw]
+    const int xstage = G * p.xw + kChunk;                                      // words; the last kChunk stay zero
+    float* Xs = reinterpret_cast<float*>(smem_raw);                            // [kXStages][xstage]
+    float* Ps = Xs + kXStages * xstage;                                        // [2][psw]
     int32_t* Ds = reinterpret_cast<int32_t*>(Ps + 2 * p.psw);                  // [kXStages][desc_ints]
     uint64_t* full = reinterpret_cast<uint64_t*>(Ds + kXStages * p.desc_ints); // [kXStages]
+    uint64_t* empty = full + kXStages;                                         // [kXStages]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int tile = blockIdx.x;                          // trial tiles fastest: neighbours share L2 lines
     const int64_t t0 = (int64_t)blockIdx.y * kTB;
     const int beam = blockIdx.z;
     const int ng = p.ngroups;
-    const int trial_off = kDRows + kDRowInts * p.rmax;    // per-trial flat offsets start here
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < kXStages; ++s) mbar_init(&full[s], 1);
+        for (int s = 0; s < kXStages; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], kWarps);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
+    if (threadIdx.x < kXStages * kChunk)
+        Xs[(threadIdx.x / kChunk) * xstage + G * p.xw + (threadIdx.x % kChunk)] = 0.0f;
     __syncthreads();
 
-    const int32_t* gdesc = p.desc + (int64_t)tile * ng * p.desc_ints;
-    const float* Xb = p.X + (int64_t)beam * p.in_beam_stride + t0;
-
-    // Producer (warp 0): lane k < 4 stages channel k of the group, lane 4 the descriptor.
-    auto produce = [&](int g) {
-        const int st = g % kXStages;
-        const int32_t* dg = gdesc + (int64_t)g * p.desc_ints;
-        int base = 0, len = 0;
-        if (lane < kG) {
-            base = __ldg(dg + kDBase + lane);
-            len = __ldg(dg + kDLen + lane);
+    if (warp == kWarps) {
+        // ---------------------------------------------------------------- producer warp
+        // lane k < G stages channel k of the group, lane G the descriptor; a stage is refilled as
+        // soon as all 16 consumer warps have released it.
+        const int32_t* gdesc = p.desc + (int64_t)tile * ng * p.desc_ints;
+        const float* Xb = p.X + (int64_t)beam * p.in_beam_stride + t0;
+        for (int g = 0; g < ng; ++g) {
+            const int st = g % kXStages;
+            const int32_t* dg = gdesc + (int64_t)g * p.desc_ints;
+            const int hv = lane < kDTrial ? __ldg(dg + lane) : 0;           // header words
+            const int base = __shfl_sync(0xffffffffu, hv, kDBase + (lane & 7));
+            int len = __shfl_sync(0xffffffffu, hv, kDLen + (lane & 7));
+            const int dbytes = __shfl_sync(0xffffffffu, hv, kDBytes);
             // the last time tile must not read past the row
-            const int64_t room = p.row_valid - (t0 + base);
-            len = (int)max((int64_t)0, min((int64_t)len, room));
-        }
-        uint32_t bytes = lane < kG ? (uint32_t)len * 4u : (lane == kG ? (uint32_t)p.desc_ints * 4u : 0u);
-        uint32_t total = bytes;
+            len = (int)max((int64_t)0, min((int64_t)len, p.row_valid - (t0 + base)));
+            const uint32_t bytes = lane < G ? (uint32_t)len * 4u : (lane == G ? (uint32_t)dbytes : 0u);
+            uint32_t total = bytes;
 #pragma unroll
-        for (int o = 4; o >= 1; o >>= 1) total += __shfl_xor_sync(0xffffffffu, total, o);   // lanes 0..7
-        if (lane == 0) mbar_arrive_expect_tx(&full[st], total);
-        __syncwarp();
-        if (lane < kG) {
-            if (len > 0) {
-                const int c = g * kG + lane;
-                bulk_load(Xs + (st * kG + lane) * p.xw, Xb + (int64_t)c * p.in_stride + base, bytes, &full[st]);
+            for (int o = 8; o >= 1; o >>= 1) total += __shfl_xor_sync(0xffffffffu, total, o);   // lanes 0..15
+            if (g >= kXStages) mbar_wait(&empty[st], ((g / kXStages) - 1) & 1);
+            if (lane == 0) mbar_arrive_expect_tx(&full[st], total);
+            __syncwarp();
+            if (lane < G) {
+                if (len > 0)
+                    bulk_load(Xs + st * xstage + lane * p.xw, Xb + (int64_t)(g * G + lane) * p.in_stride + base,
+                              bytes, &full[st]);
+            } else if (lane == G) {
+                bulk_load(Ds + st * p.desc_ints, dg, bytes, &full[st]);
             }
-        } else if (lane == kG) {
-            bulk_load(Ds + st * p.desc_ints, dg, bytes, &full[st]);
         }
-    };
+        return;
+    }
 
-    // Step 2: the pattern rows of group g into partial-sum buffer `buf`.
+    // -------------------------------------------------------------------- consumer warps
+    // Step 2: the pattern rows of group g into partial-sum buffer `buf`; a warp step forms kChunk
+    // consecutive words (lane l: words l and l + 32) from one descriptor entry of G byte offsets.
     auto pre = [&](int g, int buf) {
         const int st = g % kXStages;
         const int32_t* ds = Ds + st * p.desc_ints;
-        const float* xs = Xs + st * kG * p.xw;
-        float* ps = Ps + buf * p.psw;
-        const int nchunks = ds[kDNChunks], nk = ds[kDNChan];
-        int rho = 0;
-        const int32_t* rd = ds + kDRows;
-        for (int cidx = warp; cidx < nchunks; cidx += kWarps) {
-            const int pos = cidx * 32;
-            while (pos >= rd[0]) { rd += kDRowInts; ++rho; }         // rows are contiguous, 32-padded
-            const int e = pos + lane;
-            float v = xs[rd[1] + e];
-            if (nk > 1) v += xs[p.xw + rd[2] + e];
-            if (nk > 2) v += xs[2 * p.xw + rd[3] + e];
-            if (nk > 3) v += xs[3 * p.xw + rd[4] + e];
-            ps[e] = v;
+        const uint32_t xa = smem_u32(Xs + st * xstage) + lane * 4;
+        float* ps = Ps + buf * p.psw + lane;
+        const int nchunks = ds[kDNChunks];
+        const int4* ct = reinterpret_cast<const int4*>(ds + kDChunk);
+        for (int c = warp; c < nchunks; c += kWarps) {
+            int o[G];
+#pragma unroll
+            for (int q = 0; q < G / 4; ++q) {
+                const int4 v = ct[c * (G / 4) + q];
+                o[4 * q] = v.x; o[4 * q + 1] = v.y; o[4 * q + 2] = v.z; o[4 * q + 3] = v.w;
+            }
+            float lo[G], hi[G];
+#pragma unroll
+            for (int k = 0; k < G; ++k) {
+                lo[k] = lds_f32(xa + o[k]);
+                hi[k] = lds_f32(xa + o[k] + 128);
+            }
+            float slo = lo[0], shi = hi[0];
+#pragma unroll
+            for (int k = 1; k < G; ++k) { slo += lo[k]; shi += hi[k]; }
+            ps[c * kChunk] = slo;
+            ps[c * kChunk + 32] = shi;
         }
-        (void)rho;
     };
 
     float acc[kKW][kNK];
@@ -188,28 +224,29 @@ dd_ps_f32_kernel(const PsParams p)
 #pragma unroll
         for (int i = 0; i < kNK; ++i) acc[j][i] = 0.0f;
 
-    if (warp == 0)
-        for (int g = 0; g < kXStages && g < ng; ++g) produce(g);
     mbar_wait(&full[0], 0);
     pre(0, 0);
-    __syncthreads();
+    consumer_barrier();
 
     for (int g = 0; g < ng; ++g) {
+        const int st = g % kXStages;
         if (g + 1 < ng) {
             mbar_wait(&full[(g + 1) % kXStages], ((g + 1) / kXStages) & 1);
             pre(g + 1, (g + 1) & 1);
         }
-        // Step 3
-        const int32_t* tr = Ds + (g % kXStages) * p.desc_ints + trial_off + warp * kKW;
+        // Step 3: one word per trial, sample and group
+        const int4 tr = *reinterpret_cast<const int4*>(Ds + st * p.desc_ints + kDTrial + warp * kKW);
+        const int tro[kKW] = {tr.x, tr.y, tr.z, tr.w};
         const float* ps = Ps + (g & 1) * p.psw + lane;
 #pragma unroll
         for (int j = 0; j < kKW; ++j) {
-            const float* r = ps + tr[j];
+            const float* r = ps + tro[j];
 #pragma unroll
             for (int i = 0; i < kNK; ++i) acc[j][i] += r[32 * i];
         }
-        __syncthreads();
-        if (warp == 0 && g + kXStages < ng) produce(g + kXStages);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[st]);          // stage st (vectors and descriptor) may be refilled
+        consumer_barrier();                              // partial sums of g+1 complete, those of g consumed
     }
 
     float* Db = p.D + (int64_t)beam * p.out_beam_stride;
@@ -240,64 +277,102 @@ dd_repitch_f32(const float* __restrict__ X, float* __restrict__ W, int nchans, i
 
 }  // namespace
 
+namespace {
+
+struct PsRow { int key[kGMax - 1]; int umin, umax; };
+
+// The distinct relative-delay patterns of channel group g (G channels) among the trials of `tile`,
+// in order of first appearance; slot[j] = pattern of the tile's j-th trial.
+void classify(const HostTable& h, int G, int tile, int g, std::vector<PsRow>& rows, int* slot)
+{
+    rows.clear();
+    const int nch = h.nchans, ndm = h.ndm;
+    const int c0 = g * G, nk = std::min(G, nch - c0);
+    for (int j = 0; j < kKB; ++j) {
+        const int d = std::min(tile * kKB + j, ndm - 1);
+        const int32_t* s = &h.shift[(size_t)d * nch + c0];
+        int key[kGMax - 1] = {0, 0, 0, 0, 0, 0, 0};
+        for (int k = 1; k < nk; ++k) key[k - 1] = s[k] - s[0];
+        int r = 0;
+        for (; r < (int)rows.size(); ++r) {
+            bool same = true;
+            for (int k = 0; k < kGMax - 1; ++k) same = same && rows[r].key[k] == key[k];
+            if (same) break;
+        }
+        if (r == (int)rows.size()) {
+            PsRow nr;
+            for (int k = 0; k < kGMax - 1; ++k) nr.key[k] = key[k];
+            nr.umin = nr.umax = s[0];
+            rows.push_back(nr);
+        }
+        rows[r].umin = std::min(rows[r].umin, s[0]);
+        rows[r].umax = std::max(rows[r].umax, s[0]);
+        slot[j] = r;
+    }
+}
+
+struct PsShape { bool fits = false; int64_t psw = 0, xw = 0; int desc_ints = 0; size_t smem = 0; double cost = 0; };
+
+// Shared-memory need and modelled shared-memory wavefronts per output tile for group size G:
+// step 3 costs kKB * kNK per group, step 2 (2 G + 2 + G / 4) per kChunk words of pattern rows.
+PsShape shape_for(const HostTable& h, int G)
+{
+    PsShape o;
+    const int ntiles = (h.ndm + kKB - 1) / kKB, ngroups = (h.nchans + G - 1) / G;
+    const int64_t spread = max_tile_spread(h, kKB);
+    o.xw = (kTB + spread + 3 + 3) / 4 * 4 + kChunk;
+    std::vector<PsRow> rows;
+    int slot[kKB];
+    int64_t chunks = 0;
+    for (int tile = 0; tile < ntiles; ++tile)
+        for (int g = 0; g < ngroups; ++g) {
+            classify(h, G, tile, g, rows, slot);
+            int64_t w = 0;
+            for (const PsRow& r : rows) w += ((int64_t)r.umax - r.umin + kTB + kChunk - 1) / kChunk * kChunk;
+            o.psw = std::max(o.psw, w);
+            chunks += w / kChunk;
+        }
+    o.desc_ints = kDChunk + G * (int)(o.psw / kChunk);
+    o.smem = (size_t)kXStages * (G * o.xw + kChunk) * 4 + (size_t)2 * o.psw * 4 +
+             (size_t)kXStages * o.desc_ints * 4 + 2 * kXStages * 8;
+    o.fits = o.xw <= 16384 && o.smem <= (size_t)kMaxSmem;
+    o.cost = (double)ntiles * ngroups * kKB * kNK + (double)chunks * (2 * G + 2 + G / 4);
+    return o;
+}
+
+}  // namespace
+
 int build_ps_plan(dd_plan* p)
 {
     p->ps = nullptr;
     if (p->ndm == 0 || p->dtype != DD_F32) return DD_OK;
     const HostTable& h = p->host;
     const int nch = p->nchans, ndm = p->ndm;
-    const int ntiles = (ndm + kKB - 1) / kKB, ngroups = (nch + kG - 1) / kG;
-    const int64_t spread = max_tile_spread(h, kKB);
-    const int64_t xw64 = (kTB + spread + 3 + 3) / 4 * 4 + 32;
-    if (xw64 > 16384) return DD_OK;                      // per-trial steps too large: generic kernel
-
-    struct Row { int key[kG - 1]; int umin, umax; };
-    // pass 1: the largest number of pattern rows and partial-sum words of any (tile, group)
-    // pass 2: fill.  Both passes run the same classification.
-    std::vector<Row> rows;
-    std::vector<int> slot(kKB);
-    auto classify = [&](int tile, int g) {
-        rows.clear();
-        const int c0 = g * kG, nk = std::min(kG, nch - c0);
-        for (int j = 0; j < kKB; ++j) {
-            const int d = std::min(tile * kKB + j, ndm - 1);
-            const int32_t* s = &h.shift[(size_t)d * nch + c0];
-            int key[kG - 1] = {0, 0, 0};
-            for (int k = 1; k < nk; ++k) key[k - 1] = s[k] - s[0];
-            int r = 0;
-            for (; r < (int)rows.size(); ++r)
-                if (rows[r].key[0] == key[0] && rows[r].key[1] == key[1] && rows[r].key[2] == key[2]) break;
-            if (r == (int)rows.size()) rows.push_back(Row{{key[0], key[1], key[2]}, s[0], s[0]});
-            rows[r].umin = std::min(rows[r].umin, s[0]);
-            rows[r].umax = std::max(rows[r].umax, s[0]);
-            slot[j] = r;
+    // group size: the cheaper of 8 and 4 by the wavefront model, among those that fit
+    int G = 0;
+    PsShape sh;
+    for (int cand : {8, 4}) {
+        if (cand == 8 && nch < 16) continue;
+        PsShape c = shape_for(h, cand);
+        if (c.fits && (G == 0 || c.cost < sh.cost)) {
+            G = cand;
+            sh = c;
         }
-    };
-    int rmax = 1;
-    int64_t psw = 0;
-    for (int tile = 0; tile < ntiles; ++tile)
-        for (int g = 0; g < ngroups; ++g) {
-            classify(tile, g);
-            rmax = std::max(rmax, (int)rows.size());
-            int64_t w = 0;
-            for (const Row& r : rows) w += ((int64_t)r.umax - r.umin + kTB + 31) / 32 * 32;
-            psw = std::max(psw, w);
-        }
-    const int desc_ints = (kDRows + kDRowInts * rmax + kKB + 3) / 4 * 4;
-    const size_t smem = (size_t)kXStages * kG * xw64 * 4 + (size_t)2 * psw * 4 + (size_t)kXStages * desc_ints * 4 +
-                        kXStages * 8;
-    if (smem > (size_t)kMaxSmem) return DD_OK;            // too many patterns for shared memory: generic kernel
+    }
+    if (G == 0) return DD_OK;        // per-trial delay steps too large / too many patterns: generic kernel
+    const int ntiles = (ndm + kKB - 1) / kKB, ngroups = (nch + G - 1) / G;
+    const int desc_ints = sh.desc_ints;
 
     dd_ps_plan* t = new (std::nothrow) dd_ps_plan;
     if (!t) return fail(DD_ERR_NOMEM, "ps plan allocation failed");
     p->ps = t;
+    t->G = G;
     t->ntiles = ntiles;
     t->ngroups = ngroups;
     t->desc_ints = desc_ints;
-    t->rmax = rmax;
-    t->xw = (int)xw64;
-    t->psw = (int)psw;
-    t->smem = smem;
+    t->xw = (int)sh.xw;
+    t->psw = (int)sh.psw;
+    t->smem = sh.smem;
 
     std::vector<int32_t> desc;
     try {
@@ -306,42 +381,46 @@ int build_ps_plan(dd_plan* p)
         destroy_ps_plan(p);
         return fail(DD_ERR_NOMEM, "ps descriptor allocation failed");
     }
+    const int zero_pad = G * t->xw * 4;                   // byte offset of the stage's kChunk zero words
+    std::vector<PsRow> rows;
+    int slot[kKB];
+    std::vector<int> rowbase;
     for (int tile = 0; tile < ntiles; ++tile)
         for (int g = 0; g < ngroups; ++g) {
-            classify(tile, g);
+            classify(h, G, tile, g, rows, slot);
             int32_t* ds = &desc[((size_t)tile * ngroups + g) * desc_ints];
-            const int c0 = g * kG, nk = std::min(kG, nch - c0);
+            const int c0 = g * G, nk = std::min(G, nch - c0);
             const int dfirst = tile * kKB, dlast = std::min(tile * kKB + kKB, ndm) - 1;
-            int base[kG] = {0, 0, 0, 0};
+            int base[kGMax] = {0, 0, 0, 0, 0, 0, 0, 0};
             for (int k = 0; k < nk; ++k) {
                 const int smin = h.shift[(size_t)dfirst * nch + c0 + k], smax = h.shift[(size_t)dlast * nch + c0 + k];
                 base[k] = smin & ~3;
                 ds[kDBase + k] = base[k];
                 ds[kDLen + k] = (smax + kTB - base[k] + 3) / 4 * 4;
             }
-            ds[kDNRows] = (int)rows.size();
-            ds[kDNChan] = nk;
             int flat = 0;
-            std::vector<int> rowbase(rows.size());
+            rowbase.assign(rows.size(), 0);
             for (size_t r = 0; r < rows.size(); ++r) {
                 rowbase[r] = flat;
                 const int ulen = rows[r].umax - rows[r].umin + kTB;
-                int32_t* rd = ds + kDRows + kDRowInts * r;
-                // element e of the flat buffer (rowbase <= e < end) is u = umin + (e - rowbase); channel k
-                // supplies x_k[u + r_k], staged at word (u + r_k - base_k) of its vector
-                for (int k = 0; k < kG; ++k) {
-                    const int rk = k == 0 ? 0 : rows[r].key[k - 1];
-                    rd[1 + k] = k < nk ? rows[r].umin + rk - base[k] - flat : 0;
+                // word e of the flat partial-sum buffer (rowbase <= e < rowbase + ulen) is
+                // u = umin + (e - rowbase); channel k supplies x_k[u + r_k], staged at word
+                // (u + r_k - base_k) of its vector
+                for (int c = 0; c < (ulen + kChunk - 1) / kChunk; ++c) {
+                    int32_t* ce = ds + kDChunk + G * (flat / kChunk + c);
+                    for (int k = 0; k < G; ++k) {
+                        const int rk = k == 0 ? 0 : rows[r].key[k - 1];
+                        ce[k] = k < nk ? 4 * (k * t->xw + rows[r].umin + kChunk * c + rk - base[k]) : zero_pad;
+                    }
                 }
-                flat += (ulen + 31) / 32 * 32;
-                rd[0] = flat;
+                flat += (ulen + kChunk - 1) / kChunk * kChunk;
             }
-            for (size_t r = rows.size(); r < (size_t)rmax; ++r) ds[kDRows + kDRowInts * r] = 0x7fffffff;
-            ds[kDNChunks] = flat / 32;
+            ds[kDNChunks] = flat / kChunk;
+            ds[kDBytes] = 4 * (kDChunk + G * (flat / kChunk));
             for (int j = 0; j < kKB; ++j) {
                 const int d = std::min(tile * kKB + j, ndm - 1);
                 const int s0 = h.shift[(size_t)d * nch + c0];
-                ds[kDRows + kDRowInts * rmax + j] = rowbase[slot[j]] + (s0 - rows[slot[j]].umin);
+                ds[kDTrial + j] = rowbase[slot[j]] + (s0 - rows[slot[j]].umin);
             }
         }
     cudaError_t e = cudaMalloc(&t->d_desc, desc.size() * sizeof(int32_t));
@@ -355,7 +434,8 @@ int build_ps_plan(dd_plan* p)
         destroy_ps_plan(p);
         return fail(DD_ERR_CUDA, std::string("ps descriptor upload: ") + cudaGetErrorString(e));
     }
-    e = cudaFuncSetAttribute(dd_ps_f32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    e = G == 8 ? cudaFuncSetAttribute(dd_ps_f32_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->smem)
+               : cudaFuncSetAttribute(dd_ps_f32_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->smem);
     if (e != cudaSuccess) {
         cudaGetLastError();
         return DD_OK;                                     // stays unusable; generic kernel serves
@@ -422,14 +502,14 @@ int launch_ps(const dd_plan* p, const ExecArgs& a)
     q.ndm = p->ndm;
     q.ngroups = t->ngroups;
     q.desc_ints = t->desc_ints;
-    q.rmax = t->rmax;
     q.xw = t->xw;
     q.psw = t->psw;
     q.nsamp = a.nsamp_out;
     q.out_stride = a.out_stride;
     q.out_beam_stride = a.out_beam_stride;
     dim3 grid((unsigned)t->ntiles, (unsigned)((a.nsamp_out + kTB - 1) / kTB), (unsigned)a.nbeams);
-    dd_ps_f32_kernel<<<grid, kThreads, t->smem, st>>>(q);
+    if (t->G == 8) dd_ps_f32_kernel<8><<<grid, kThreads + 32, t->smem, st>>>(q);
+    else dd_ps_f32_kernel<4><<<grid, kThreads + 32, t->smem, st>>>(q);
     cudaError_t e = cudaGetLastError();
     if (W) cudaFreeAsync(W, st);
     if (e != cudaSuccess) return fail(DD_ERR_CUDA, std::string("ps f32 launch: ") + cudaGetErrorString(e));

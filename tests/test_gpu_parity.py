@@ -269,7 +269,7 @@ def test_one_shot_and_host_calls(dtype):
 
 # ------------------------------------------------------------------ float32 partial-sum kernel, direct (aligned) path
 
-@pytest.mark.parametrize("idx,nchans,ndm,nsamp", [(3, 517, 130, 2000), (4, 64, 200, 1500), (1, 64, 32, 8192)])
+@pytest.mark.parametrize("idx,nchans,ndm,nsamp", [(3, 517, 130, 2000), (4, 256, 200, 1500), (3, 64, 40, 5000), (3, 130, 70, 600)])
 def test_ps_kernel_reads_aligned_input_directly(idx, nchans, ndm, nsamp):
     """16-byte aligned X with strides that are multiples of four elements is staged by TMA straight from
     the caller's buffer (no re-pitch copy): several DM tiles, several time tiles, ragged tails, a
