@@ -169,6 +169,7 @@ int dd_plan_create(dd_plan** out, int dtype, int nchans, double fch1, double fof
     }
     rc = build_tma_plan(p);
     if (rc == DD_OK) rc = build_ps_plan(p);
+    if (rc == DD_OK) rc = build_psu8_plan(p);
     if (rc != DD_OK) {
         dd_plan_destroy(p);
         return rc;
@@ -193,6 +194,7 @@ void dd_plan_destroy(dd_plan* p)
     }
     destroy_tma_plan(p);
     destroy_ps_plan(p);
+    destroy_psu8_plan(p);
     if (p->d_shift) cudaFree(p->d_shift);
     if (p->d_order) cudaFree(p->d_order);
     delete p;
@@ -221,7 +223,7 @@ int dd_plan_set_kernel(dd_plan* p, int kernel)
     if (kernel != DD_KERNEL_AUTO && kernel != DD_KERNEL_GENERIC && kernel != DD_KERNEL_TMA &&
         kernel != DD_KERNEL_PS)
         return fail(DD_ERR_BAD_ARG, "unknown kernel id");
-    if (kernel == DD_KERNEL_PS && !ps_plan_usable(p))
+    if (kernel == DD_KERNEL_PS && !ps_plan_usable(p) && !psu8_plan_usable(p))
         return fail(DD_ERR_UNSUPPORTED, "the partial-sum kernel does not take this plan (dtype or per-trial delay steps)");
     if (kernel == DD_KERNEL_TMA && !tma_plan_usable(p))
         return fail(DD_ERR_UNSUPPORTED, "the TMA-staged kernel does not take this plan (dtype or per-trial delay steps)");
@@ -251,7 +253,8 @@ static void fill_args(const dd_plan* p, ExecArgs* a, const void* X, int64_t in_s
 static int kernel_for(const dd_plan* p, const ExecArgs& a)
 {
     if (p->kernel_pref == DD_KERNEL_GENERIC) return DD_KERNEL_GENERIC;
-    if (tma_plan_usable(p) && tma_args_ok(p, a)) return DD_KERNEL_TMA;
+    if (p->kernel_pref != DD_KERNEL_TMA && psu8_plan_usable(p) && psu8_args_ok(p, a)) return DD_KERNEL_PS;
+    if (p->kernel_pref != DD_KERNEL_PS && tma_plan_usable(p) && tma_args_ok(p, a)) return DD_KERNEL_TMA;
     if (ps_plan_usable(p) && ps_args_ok(p, a)) return DD_KERNEL_PS;
     return DD_KERNEL_GENERIC;
 }
@@ -274,7 +277,7 @@ int dd_plan_launches_per_execute(const dd_plan* p)
     // the TMA-staged uint8 path runs the byte-shift front end and the dedispersion kernel; the
     // float32 partial-sum kernel reads 16-byte aligned input directly (one launch; two when the
     // caller's buffer has to be re-pitched first)
-    return (p->kernel_pref != DD_KERNEL_GENERIC && tma_plan_usable(p)) ? 2 : 1;
+    return (p->kernel_pref != DD_KERNEL_GENERIC && (tma_plan_usable(p) || psu8_plan_usable(p))) ? 2 : 1;
 }
 
 int dd_execute(const dd_plan* p, const void* X, int64_t in_stride, int64_t in_beam_stride, void* D,
@@ -305,7 +308,7 @@ int dd_execute(const dd_plan* p, const void* X, int64_t in_stride, int64_t in_be
     if (p->kernel_pref == DD_KERNEL_PS && k != DD_KERNEL_PS)
         return fail(DD_ERR_UNSUPPORTED, "partial-sum kernel forced but the grid does not fit");
     if (k == DD_KERNEL_TMA) return launch_tma(p, a);
-    if (k == DD_KERNEL_PS) return launch_ps(p, a);
+    if (k == DD_KERNEL_PS) return p->dtype == DD_U8 ? launch_psu8(p, a) : launch_ps(p, a);
     return launch_generic(p->dtype, p->generic_kb, p->generic_spread, a);
 }
 

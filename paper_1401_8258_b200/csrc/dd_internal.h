@@ -55,6 +55,7 @@ struct dd_plan;
 struct dd_host_ws;
 struct dd_tma_plan;
 struct dd_ps_plan;
+struct dd_psu8_plan;
 
 namespace dd {
 // TMA-staged kernels (tma_u8.cu): plan-time tables, eligibility, launch
@@ -63,6 +64,8 @@ void destroy_tma_plan(dd_plan* p);
 bool tma_plan_usable(const dd_plan* p);
 bool tma_args_ok(const dd_plan* p, const ExecArgs& a);
 int launch_tma(const dd_plan* p, const ExecArgs& a);
+int make_shift_copies_u8(const dd_plan* p, const ExecArgs& a, uint8_t** W_out, int64_t* wcopy_out,
+                         int64_t* wpitch_out);
 // float32 kernel with shared partial sums (ps_f32.cu)
 int build_ps_plan(dd_plan* p);
 void destroy_ps_plan(dd_plan* p);
@@ -70,6 +73,12 @@ bool ps_plan_usable(const dd_plan* p);
 bool ps_args_ok(const dd_plan* p, const ExecArgs& a);
 int ps_launches(const dd_plan* p, const ExecArgs& a);
 int launch_ps(const dd_plan* p, const ExecArgs& a);
+// uint8 kernel with shared partial sums (ps_u8.cu)
+int build_psu8_plan(dd_plan* p);
+void destroy_psu8_plan(dd_plan* p);
+bool psu8_plan_usable(const dd_plan* p);
+bool psu8_args_ok(const dd_plan* p, const ExecArgs& a);
+int launch_psu8(const dd_plan* p, const ExecArgs& a);
 }  // namespace dd
 
 struct dd_plan {
@@ -85,5 +94,6 @@ struct dd_plan {
     int generic_spread = 0;
     dd_tma_plan* tma = nullptr;         // null: the TMA-staged uint8 kernel does not take this plan
     dd_ps_plan* ps = nullptr;           // null: the float32 partial-sum kernel does not take this plan
+    dd_psu8_plan* psu8 = nullptr;       // null: the uint8 partial-sum kernel does not take this plan
     dd_host_ws* host_ws = nullptr;      // device buffers / streams cached by dd_execute_host
 };

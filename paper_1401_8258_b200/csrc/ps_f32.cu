@@ -31,6 +31,7 @@
 #include <vector>
 
 #include "dd_internal.h"
+#include "ps_host.h"
 
 struct dd_ps_plan {
     bool ok = false;
@@ -47,7 +48,7 @@ namespace dd {
 
 namespace {
 
-constexpr int kGMax = 8;                  // channels per group: 4 or 8
+constexpr int kGMax = kPsGMax;            // channels per group: 4 or 8
 constexpr int kWarps = 16;
 constexpr int kThreads = 32 * kWarps;
 constexpr int kKW = 4;                    // trials per warp
@@ -279,38 +280,6 @@ dd_repitch_f32(const float* __restrict__ X, float* __restrict__ W, int nchans, i
 
 namespace {
 
-struct PsRow { int key[kGMax - 1]; int umin, umax; };
-
-// The distinct relative-delay patterns of channel group g (G channels) among the trials of `tile`,
-// in order of first appearance; slot[j] = pattern of the tile's j-th trial.
-void classify(const HostTable& h, int G, int tile, int g, std::vector<PsRow>& rows, int* slot)
-{
-    rows.clear();
-    const int nch = h.nchans, ndm = h.ndm;
-    const int c0 = g * G, nk = std::min(G, nch - c0);
-    for (int j = 0; j < kKB; ++j) {
-        const int d = std::min(tile * kKB + j, ndm - 1);
-        const int32_t* s = &h.shift[(size_t)d * nch + c0];
-        int key[kGMax - 1] = {0, 0, 0, 0, 0, 0, 0};
-        for (int k = 1; k < nk; ++k) key[k - 1] = s[k] - s[0];
-        int r = 0;
-        for (; r < (int)rows.size(); ++r) {
-            bool same = true;
-            for (int k = 0; k < kGMax - 1; ++k) same = same && rows[r].key[k] == key[k];
-            if (same) break;
-        }
-        if (r == (int)rows.size()) {
-            PsRow nr;
-            for (int k = 0; k < kGMax - 1; ++k) nr.key[k] = key[k];
-            nr.umin = nr.umax = s[0];
-            rows.push_back(nr);
-        }
-        rows[r].umin = std::min(rows[r].umin, s[0]);
-        rows[r].umax = std::max(rows[r].umax, s[0]);
-        slot[j] = r;
-    }
-}
-
 struct PsShape { bool fits = false; int64_t psw = 0, xw = 0; int desc_ints = 0; size_t smem = 0; double cost = 0; };
 
 // Shared-memory need and modelled shared-memory wavefronts per output tile for group size G:
@@ -326,7 +295,7 @@ PsShape shape_for(const HostTable& h, int G)
     int64_t chunks = 0;
     for (int tile = 0; tile < ntiles; ++tile)
         for (int g = 0; g < ngroups; ++g) {
-            classify(h, G, tile, g, rows, slot);
+            ps_classify(h, G, kKB, tile, g, rows, slot);
             int64_t w = 0;
             for (const PsRow& r : rows) w += ((int64_t)r.umax - r.umin + kTB + kChunk - 1) / kChunk * kChunk;
             o.psw = std::max(o.psw, w);
@@ -387,7 +356,7 @@ int build_ps_plan(dd_plan* p)
     std::vector<int> rowbase;
     for (int tile = 0; tile < ntiles; ++tile)
         for (int g = 0; g < ngroups; ++g) {
-            classify(h, G, tile, g, rows, slot);
+            ps_classify(h, G, kKB, tile, g, rows, slot);
             int32_t* ds = &desc[((size_t)tile * ngroups + g) * desc_ints];
             const int c0 = g * G, nk = std::min(G, nch - c0);
             const int dfirst = tile * kKB, dlast = std::min(tile * kKB + kKB, ndm) - 1;

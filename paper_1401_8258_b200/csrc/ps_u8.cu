@@ -1,0 +1,446 @@
+// uint8 -> int32 kernel with shared partial sums (SURVEY.md §8 rows a2-a6 for the uint8 path).
+//
+// Same idea as ps_f32.cu, same result as eq 2.1, exact integer arithmetic:
+// channels are taken in groups of G = 4; within a tile of kKB adjacent (sorted) trials the relative
+// delays r_k(d) = s(d,c0+k) - s(d,c0) take a handful of distinct values ("patterns"), so a block
+//   1. has the channel vectors of the group in shared memory (eq 2.14): for every
+//      channel the 16-byte aligned window of each of the four byte-shifted copies W_r[i] = X[i+r]
+//      that the front end of tma_u8.cu writes (bulk copies need aligned sources, the window start
+//      t0 + s(d0,c) is arbitrary), copied by the TMA engine three groups ahead;
+//   2. forms, per pattern, the row of partial sums P[u] = x0[u] + x1[u+r1] + x2[u+r2] + x3[u+r3]
+//      (<= 4*255, so 16 bits) TWICE, as 32-bit words holding (P[u], P[u+1]) for even and for odd u:
+//      one aligned LDS gives four consecutive samples of a channel, two PRMT widen them into two
+//      words of 16-bit lanes, three adds per word sum the channels;
+//   3. adds ONE word per trial, per PAIR of output samples and per group:
+//      acc(16-bit lanes) += P^{parity}_{pattern(d)}[(t + s(d,c0)) / 2].
+// Step 3 is one shared-memory word and one integer add per EIGHT channel-sample adds (Alg. 1,
+// PAPER.md:960-988, spends one word and two instructions per ONE).  The packed accumulators are
+// flushed into the int32 output every kFlushGroups groups (64 * 4 * 255 < 65536) by a 16-byte
+// read-modify-write that stays in L2 (plain store the first time).
+//
+// Layout of a block: 16 consumer warps + 1 producer warp; consumer warp w owns trials
+// w*kKW .. w*kKW+kKW-1, lane l owns output samples t0 + 2 (l + 32 i) + {0,1}, i < kNK.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <new>
+#include <vector>
+
+#include "dd_internal.h"
+#include "ps_host.h"
+
+struct dd_psu8_plan {
+    bool ok = false;
+    int ntiles = 0, ngroups = 0;
+    int desc_ints = 0;             // ints per (tile, group) descriptor (multiple of 4)
+    int xwb = 0;                   // bytes staged per byte-shifted copy of a channel (multiple of 16)
+    int psw = 0;                   // words of one partial-sum buffer
+    size_t smem = 0;
+    int32_t* d_desc = nullptr;     // device [ntiles][ngroups][desc_ints]
+};
+
+namespace dd {
+
+namespace {
+
+constexpr int kG = 4;                     // channels per group
+constexpr int kWarps = 16;
+constexpr int kThreads = 32 * kWarps;
+constexpr int kKW = 4;                    // trials per warp
+constexpr int kKB = kKW * kWarps;         // trials per block
+constexpr int kNK = 16;                   // output sample PAIRS per lane
+constexpr int kTB = 2 * 32 * kNK;         // output samples per block
+constexpr int kXStages = 3;
+constexpr int kMaxSmem = 200 * 1024;
+constexpr int kFlushGroups = 64;          // 64 groups * 4 channels * 255 = 65280 < 65536
+constexpr int kChunk = 64;                // words (= 128 samples) of a partial-sum row per warp step
+
+// descriptor layout (ints), one per (trial tile, channel group)
+constexpr int kDNChunks = 0;
+constexpr int kDBytes = 1;                // bytes of this descriptor that are in use (multiple of 16)
+constexpr int kDBase = 4;                 // [4]  first staged byte of channel k, relative to t0 (multiple of 16)
+constexpr int kDLen = 8;                  // [4]  bytes to stage per copy (multiple of 16; 0 for a missing channel)
+constexpr int kDTrial = 12;               // [kKB] word offset of trial j's first operand in the partial sums
+constexpr int kDChunk = kDTrial + kKB;    // [nchunks][4] byte offset, from the stage's first byte, of the
+                                          //      aligned word lane 0 reads in channel k (zero pad if missing)
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+        ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+__device__ __forceinline__ void consumer_barrier()
+{
+    asm volatile("bar.sync 1, %0;" ::"n"(kThreads) : "memory");
+}
+__device__ __forceinline__ uint32_t lds_u32(uint32_t addr)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+
+struct PsU8Params {
+    const uint8_t* W;              // workspace: four byte-shifted copies, [4][nbeams*nchans][wpitch]
+    int64_t wcopy, wpitch;         // bytes between the copies / between channel rows of a copy
+    int32_t* D;
+    const int32_t* desc;
+    const int32_t* order;
+    int nchans, ndm, ngroups, desc_ints, xwb, psw;
+    int64_t nsamp, out_stride, out_beam_stride;
+};
+
+__global__ void __launch_bounds__(kThreads + 32, 1)
+dd_ps_u8_kernel(const PsU8Params p)
+{
+    extern __shared__ __align__(128) uint8_t smem_raw[];
+    const int xstage = kG * 4 * p.xwb + 4 * kChunk;                            // bytes; the last 256 stay zero
+    uint8_t* Xs = smem_raw;                                                    // [kXStages][xstage]
+    uint32_t* Ps = reinterpret_cast<uint32_t*>(Xs + kXStages * xstage);        // [2][psw]
+    int32_t* Ds = reinterpret_cast<int32_t*>(Ps + 2 * p.psw);                  // [kXStages][desc_ints]
+    uint64_t* full = reinterpret_cast<uint64_t*>(Ds + kXStages * p.desc_ints); // [kXStages]
+    uint64_t* empty = full + kXStages;                                         // [kXStages]
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int tile = blockIdx.x;                          // trial tiles fastest: neighbours share L2 lines
+    const int64_t t0 = (int64_t)blockIdx.y * kTB;
+    const int beam = blockIdx.z;
+    const int ng = p.ngroups;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kXStages; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], kWarps);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    if (threadIdx.x < kXStages * kChunk)
+        reinterpret_cast<uint32_t*>(Xs + (threadIdx.x / kChunk) * xstage + kG * 4 * p.xwb)[threadIdx.x % kChunk] = 0u;
+    __syncthreads();
+
+    if (warp == kWarps) {
+        // ---------------------------------------------------------------- producer warp
+        // lane 4 k + r stages copy r of channel k, lane 16 the descriptor; a stage is refilled as
+        // soon as all 16 consumer warps have released it.
+        const int32_t* gdesc = p.desc + (int64_t)tile * ng * p.desc_ints;
+        const uint8_t* Wb = p.W + (int64_t)beam * p.nchans * p.wpitch + t0;
+        for (int g = 0; g < ng; ++g) {
+            const int st = g % kXStages;
+            const int32_t* dg = gdesc + (int64_t)g * p.desc_ints;
+            const int hv = lane < kDTrial ? __ldg(dg + lane) : 0;           // header words
+            const int base = __shfl_sync(0xffffffffu, hv, kDBase + ((lane >> 2) & 3));
+            const int len = __shfl_sync(0xffffffffu, hv, kDLen + ((lane >> 2) & 3));
+            const int dbytes = __shfl_sync(0xffffffffu, hv, kDBytes);
+            const uint32_t bytes = lane < 4 * kG ? (uint32_t)len : (lane == 4 * kG ? (uint32_t)dbytes : 0u);
+            uint32_t total = bytes;
+#pragma unroll
+            for (int o = 16; o >= 1; o >>= 1) total += __shfl_xor_sync(0xffffffffu, total, o);
+            if (g >= kXStages) mbar_wait(&empty[st], ((g / kXStages) - 1) & 1);
+            if (lane == 0) mbar_arrive_expect_tx(&full[st], total);
+            __syncwarp();
+            if (lane < 4 * kG) {
+                if (len > 0)
+                    bulk_load(Xs + st * xstage + lane * p.xwb,
+                              Wb + (lane & 3) * p.wcopy + (int64_t)(g * kG + (lane >> 2)) * p.wpitch + base, bytes,
+                              &full[st]);
+            } else if (lane == 4 * kG) {
+                bulk_load(Ds + st * p.desc_ints, dg, bytes, &full[st]);
+            }
+        }
+        return;
+    }
+
+    // -------------------------------------------------------------------- consumer warps
+    // Step 2: a warp step forms kChunk consecutive words (128 samples) of one pattern row and parity:
+    // lane l reads the aligned word with samples 4l..4l+3 of every channel and writes words 2l, 2l+1.
+    auto pre = [&](int g, int buf) {
+        const int st = g % kXStages;
+        const int32_t* ds = Ds + st * p.desc_ints;
+        const uint32_t xa = smem_u32(Xs + st * xstage) + lane * 4;
+        uint2* ps = reinterpret_cast<uint2*>(Ps + buf * p.psw) + lane;
+        const int nchunks = ds[kDNChunks];
+        const int4* ct = reinterpret_cast<const int4*>(ds + kDChunk);
+        for (int c = warp; c < nchunks; c += kWarps) {
+            const int4 o = ct[c];
+            const uint32_t w0 = lds_u32(xa + o.x), w1 = lds_u32(xa + o.y), w2 = lds_u32(xa + o.z),
+                           w3 = lds_u32(xa + o.w);
+            // (b0 | b1 << 16) and (b2 | b3 << 16) of each channel word, summed over the channels
+            const uint32_t lo = (__byte_perm(w0, 0, 0x4140) + __byte_perm(w1, 0, 0x4140)) +
+                                (__byte_perm(w2, 0, 0x4140) + __byte_perm(w3, 0, 0x4140));
+            const uint32_t hi = (__byte_perm(w0, 0, 0x4342) + __byte_perm(w1, 0, 0x4342)) +
+                                (__byte_perm(w2, 0, 0x4342) + __byte_perm(w3, 0, 0x4342));
+            ps[c * (kChunk / 2)] = make_uint2(lo, hi);
+        }
+    };
+
+    uint32_t acc[kKW][kNK];
+#pragma unroll
+    for (int j = 0; j < kKW; ++j)
+#pragma unroll
+        for (int i = 0; i < kNK; ++i) acc[j][i] = 0u;
+
+    int32_t* Db = p.D + (int64_t)beam * p.out_beam_stride;
+    int nflush = 0;
+    // lanes 2m, 2m+1 exchange halves so that every lane writes four consecutive samples
+    auto flush = [&]() {
+#pragma unroll
+        for (int j = 0; j < kKW; ++j) {
+            const int d = tile * kKB + warp * kKW + j;
+            int32_t* drow = Db + (int64_t)(d < p.ndm ? __ldg(p.order + d) : 0) * p.out_stride;
+#pragma unroll
+            for (int i = 0; i < kNK; i += 2) {
+                // this lane holds samples 2l+64i+{0,1} (acc[j][i]) and 2l+64(i+1)+{0,1} (acc[j][i+1]);
+                // even lanes take both pairs of block i, odd lanes both pairs of block i+1
+                const uint32_t mine = (lane & 1) ? acc[j][i + 1] : acc[j][i];
+                const uint32_t give = (lane & 1) ? acc[j][i] : acc[j][i + 1];
+                const uint32_t got = __shfl_xor_sync(0xffffffffu, give, 1);
+                const uint32_t first = (lane & 1) ? got : mine, second = (lane & 1) ? mine : got;
+                const int64_t t = t0 + 2 * (lane & ~1) + 64 * (i + (lane & 1));
+                int4 v = make_int4((int)(first & 0xffffu), (int)(first >> 16), (int)(second & 0xffffu),
+                                   (int)(second >> 16));
+                if (d < p.ndm) {
+                    if (t + 3 < p.nsamp) {
+                        int4* q = reinterpret_cast<int4*>(drow + t);
+                        if (nflush) {
+                            const int4 old = __ldcg(q);
+                            v.x += old.x; v.y += old.y; v.z += old.z; v.w += old.w;
+                        }
+                        *q = v;
+                    } else {
+                        const int vv[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                        for (int e = 0; e < 4; ++e)
+                            if (t + e < p.nsamp) drow[t + e] = (nflush ? __ldcg(drow + t + e) : 0) + vv[e];
+                    }
+                }
+                acc[j][i] = acc[j][i + 1] = 0u;
+            }
+        }
+        ++nflush;
+    };
+
+    mbar_wait(&full[0], 0);
+    pre(0, 0);
+    consumer_barrier();
+
+    for (int g = 0; g < ng; ++g) {
+        const int st = g % kXStages;
+        if (g + 1 < ng) {
+            mbar_wait(&full[(g + 1) % kXStages], ((g + 1) / kXStages) & 1);
+            pre(g + 1, (g + 1) & 1);
+        }
+        // Step 3: one word per trial, sample pair and group
+        const int4 tr = *reinterpret_cast<const int4*>(Ds + st * p.desc_ints + kDTrial + warp * kKW);
+        const int tro[kKW] = {tr.x, tr.y, tr.z, tr.w};
+        const uint32_t* ps = Ps + (g & 1) * p.psw + lane;
+#pragma unroll
+        for (int j = 0; j < kKW; ++j) {
+            const uint32_t* r = ps + tro[j];
+#pragma unroll
+            for (int i = 0; i < kNK; ++i) acc[j][i] += r[32 * i];
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[st]);          // stage st (vectors and descriptor) may be refilled
+        consumer_barrier();                              // partial sums of g+1 complete, those of g consumed
+        if (((g + 1) % kFlushGroups) == 0 && g + 1 < ng) flush();
+    }
+    flush();
+}
+
+}  // namespace
+
+int build_psu8_plan(dd_plan* p)
+{
+    p->psu8 = nullptr;
+    if (p->ndm == 0 || p->dtype != DD_U8) return DD_OK;
+    const HostTable& h = p->host;
+    const int nch = p->nchans, ndm = p->ndm;
+    const int ntiles = (ndm + kKB - 1) / kKB, ngroups = (nch + kG - 1) / kG;
+    const int64_t spread = max_tile_spread(h, kKB);
+    const int64_t xwb = (kTB + spread + 16 + 2 * kChunk + 128 + 16 + 15) / 16 * 16;
+    if (xwb > 8192) return DD_OK;                         // per-trial steps too large: other kernels
+
+    // words of one parity copy of a pattern row: the largest offset of a trial in it, halved, plus
+    // the kTB / 2 words every trial reads, in whole warp steps
+    auto row_words = [](const PsRow& r) { return ((r.umax - r.umin) / 2 + kTB / 2 + kChunk - 1) / kChunk * kChunk; };
+    std::vector<PsRow> rows;
+    int slot[kKB];
+    int64_t psw = 0;
+    for (int tile = 0; tile < ntiles; ++tile)
+        for (int g = 0; g < ngroups; ++g) {
+            ps_classify(h, kG, kKB, tile, g, rows, slot);
+            int64_t w = 0;
+            for (const PsRow& r : rows) w += 2 * row_words(r);
+            psw = std::max(psw, w);
+        }
+    const int desc_ints = kDChunk + 4 * (int)(psw / kChunk);
+    const size_t smem = (size_t)kXStages * (kG * 4 * xwb + 4 * kChunk) + (size_t)2 * psw * 4 +
+                        (size_t)kXStages * desc_ints * 4 + 2 * kXStages * 8;
+    if (smem > (size_t)kMaxSmem) return DD_OK;            // too many patterns for shared memory
+
+    dd_psu8_plan* t = new (std::nothrow) dd_psu8_plan;
+    if (!t) return fail(DD_ERR_NOMEM, "ps u8 plan allocation failed");
+    p->psu8 = t;
+    t->ntiles = ntiles;
+    t->ngroups = ngroups;
+    t->desc_ints = desc_ints;
+    t->xwb = (int)xwb;
+    t->psw = (int)psw;
+    t->smem = smem;
+
+    std::vector<int32_t> desc;
+    try {
+        desc.assign((size_t)ntiles * ngroups * desc_ints, 0);
+    } catch (const std::bad_alloc&) {
+        destroy_psu8_plan(p);
+        return fail(DD_ERR_NOMEM, "ps u8 descriptor allocation failed");
+    }
+    const int zero_pad = kG * 4 * t->xwb;                 // byte offset of the stage's zero words
+    std::vector<int> rowbase;
+    for (int tile = 0; tile < ntiles; ++tile)
+        for (int g = 0; g < ngroups; ++g) {
+            ps_classify(h, kG, kKB, tile, g, rows, slot);
+            int32_t* ds = &desc[((size_t)tile * ngroups + g) * desc_ints];
+            const int c0 = g * kG, nk = std::min(kG, nch - c0);
+            const int dfirst = tile * kKB, dlast = std::min(tile * kKB + kKB, ndm) - 1;
+            int base[kG] = {0, 0, 0, 0};
+            for (int k = 0; k < nk; ++k) {
+                const int smin = h.shift[(size_t)dfirst * nch + c0 + k], smax = h.shift[(size_t)dlast * nch + c0 + k];
+                base[k] = smin & ~15;
+                ds[kDBase + k] = base[k];
+                ds[kDLen + k] = (smax + kTB - base[k] + 15) / 16 * 16;
+            }
+            int flat = 0;                                 // words
+            rowbase.assign(2 * rows.size(), 0);
+            for (size_t r = 0; r < rows.size(); ++r)
+                for (int par = 0; par < 2; ++par) {
+                    rowbase[2 * r + par] = flat;
+                    const int nw = row_words(rows[r]);
+                    // word w of this copy holds the partial sums of u = umin + par + 2 w and u + 1;
+                    // a warp step makes words [kChunk c, kChunk c + kChunk): lane l reads, per channel
+                    // k, the aligned word with samples x_k[u0 + r_k + 4 l ..+3], u0 = umin + par + 128 c,
+                    // i.e. byte a0 + 4 l of the staged window, a0 = u0 + r_k - base_k: copy (a0 & 3),
+                    // word (a0 >> 2) + l
+                    for (int c = 0; c < nw / kChunk; ++c) {
+                        int32_t* ce = ds + kDChunk + 4 * (flat / kChunk + c);
+                        for (int k = 0; k < kG; ++k) {
+                            const int rk = k == 0 ? 0 : rows[r].key[k - 1];
+                            const int a0 = rows[r].umin + par + 2 * kChunk * c + rk - base[k];
+                            ce[k] = k < nk ? (4 * k + (a0 & 3)) * t->xwb + (a0 & ~3) : zero_pad;
+                        }
+                    }
+                    flat += nw;
+                }
+            ds[kDNChunks] = flat / kChunk;
+            ds[kDBytes] = 4 * (kDChunk + 4 * (flat / kChunk));
+            for (int j = 0; j < kKB; ++j) {
+                const int d = std::min(tile * kKB + j, ndm - 1);
+                const int o = h.shift[(size_t)d * nch + c0] - rows[slot[j]].umin;
+                ds[kDTrial + j] = rowbase[2 * slot[j] + (o & 1)] + (o >> 1);
+            }
+        }
+    cudaError_t e = cudaMalloc(&t->d_desc, desc.size() * sizeof(int32_t));
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        destroy_psu8_plan(p);
+        return fail(DD_ERR_NOMEM, std::string("ps u8 descriptor table: ") + cudaGetErrorString(e));
+    }
+    e = cudaMemcpy(t->d_desc, desc.data(), desc.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        destroy_psu8_plan(p);
+        return fail(DD_ERR_CUDA, std::string("ps u8 descriptor upload: ") + cudaGetErrorString(e));
+    }
+    e = cudaFuncSetAttribute(dd_ps_u8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->smem);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return DD_OK;                                     // stays unusable; the other kernels serve
+    }
+    t->ok = true;
+    return DD_OK;
+}
+
+void destroy_psu8_plan(dd_plan* p)
+{
+    if (!p->psu8) return;
+    if (p->psu8->d_desc) cudaFree(p->psu8->d_desc);
+    delete p->psu8;
+    p->psu8 = nullptr;
+}
+
+bool psu8_plan_usable(const dd_plan* p) { return p->psu8 && p->psu8->ok; }
+
+bool psu8_args_ok(const dd_plan* p, const ExecArgs& a)
+{
+    if (!psu8_plan_usable(p)) return false;
+    // 16-byte read-modify-write of D
+    if (((uintptr_t)a.D & 15) || (a.out_stride & 3) || (a.nbeams > 1 && (a.out_beam_stride & 3))) return false;
+    if ((a.nsamp_out + kTB - 1) / kTB > 65535 || a.nbeams > 65535) return false;
+    if ((int64_t)a.nbeams * p->nchans > 65535) return false;          // grid.y of the front end
+    return true;
+}
+
+int launch_psu8(const dd_plan* p, const ExecArgs& a)
+{
+    const dd_psu8_plan* t = p->psu8;
+    cudaStream_t st = (cudaStream_t)a.stream;
+    uint8_t* W = nullptr;
+    int64_t wcopy = 0, wpitch = 0;
+    int rc = make_shift_copies_u8(p, a, &W, &wcopy, &wpitch);
+    if (rc != DD_OK) return rc;
+    PsU8Params q;
+    q.W = W;
+    q.wcopy = wcopy;
+    q.wpitch = wpitch;
+    q.D = (int32_t*)a.D;
+    q.desc = t->d_desc;
+    q.order = a.d_order;
+    q.nchans = p->nchans;
+    q.ndm = p->ndm;
+    q.ngroups = t->ngroups;
+    q.desc_ints = t->desc_ints;
+    q.xwb = t->xwb;
+    q.psw = t->psw;
+    q.nsamp = a.nsamp_out;
+    q.out_stride = a.out_stride;
+    q.out_beam_stride = a.out_beam_stride;
+    dim3 grid((unsigned)t->ntiles, (unsigned)((a.nsamp_out + kTB - 1) / kTB), (unsigned)a.nbeams);
+    dd_ps_u8_kernel<<<grid, kThreads + 32, t->smem, st>>>(q);
+    cudaError_t e = cudaGetLastError();
+    cudaFreeAsync(W, st);
+    if (e != cudaSuccess) return fail(DD_ERR_CUDA, std::string("ps u8 launch: ") + cudaGetErrorString(e));
+    return DD_OK;
+}
+
+}  // namespace dd

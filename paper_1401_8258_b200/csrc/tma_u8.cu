@@ -405,13 +405,13 @@ bool tma_args_ok(const dd_plan* p, const ExecArgs& a)
     return true;
 }
 
-int launch_tma(const dd_plan* p, const ExecArgs& a)
+// Front end shared with ps_u8.cu: allocates (stream-ordered) and fills the four byte-shifted copies.
+// Rows are padded so that the last time tile may over-read its window (the excess only feeds
+// output samples >= nsamp_out, which are never stored).  The caller frees *W with cudaFreeAsync.
+int make_shift_copies_u8(const dd_plan* p, const ExecArgs& a, uint8_t** W_out, int64_t* wcopy_out, int64_t* wpitch_out)
 {
-    const dd_tma_plan* t = p->tma;
     cudaStream_t st = (cudaStream_t)a.stream;
     const int64_t rowlen = a.nsamp_out + p->host.maxshift;            // valid samples per channel row
-    // rows are padded so that the last time tile may over-read its window (the excess only feeds
-    // output samples >= nsamp_out, which are never stored)
     const int64_t wpitch = (rowlen + (int64_t)kMaxNY * kBoxW + 16 + 127) / 128 * 128;
     const int64_t nrows = (int64_t)a.nbeams * p->nchans;
     const int64_t wcopy = nrows * wpitch;
@@ -421,12 +421,25 @@ int launch_tma(const dd_plan* p, const ExecArgs& a)
         cudaGetLastError();
         return fail(DD_ERR_NOMEM, std::string("byte-shifted workspace: ") + cudaGetErrorString(e));
     }
-    {
-        const int64_t nwords = (rowlen + 3) / 4;
-        dim3 grid((unsigned)std::min<int64_t>((nwords + 255) / 256, 64), (unsigned)nrows);
-        dd_shift_copies_u8<<<grid, 256, 0, st>>>((const uint8_t*)a.X, W, wcopy, wpitch, p->nchans, rowlen,
-                                                 a.in_stride, a.in_beam_stride);
-    }
+    const int64_t nwords = (rowlen + 3) / 4;
+    dim3 grid((unsigned)std::min<int64_t>((nwords + 255) / 256, 64), (unsigned)nrows);
+    dd_shift_copies_u8<<<grid, 256, 0, st>>>((const uint8_t*)a.X, W, wcopy, wpitch, p->nchans, rowlen,
+                                             a.in_stride, a.in_beam_stride);
+    *W_out = W;
+    *wcopy_out = wcopy;
+    *wpitch_out = wpitch;
+    return DD_OK;
+}
+
+int launch_tma(const dd_plan* p, const ExecArgs& a)
+{
+    const dd_tma_plan* t = p->tma;
+    cudaStream_t st = (cudaStream_t)a.stream;
+    uint8_t* W = nullptr;
+    int64_t wcopy = 0, wpitch = 0;
+    int rc = make_shift_copies_u8(p, a, &W, &wcopy, &wpitch);
+    if (rc != DD_OK) return rc;
+    cudaError_t e;
     U8Params q;
     q.W = W;
     q.wcopy = wcopy;

@@ -267,6 +267,18 @@ def test_one_shot_and_host_calls(dtype):
     plan.destroy()
 
 
+# ------------------------------------------------------------------ the first-generation uint8 kernel, forced
+
+@pytest.mark.parametrize("idx,nchans,ndm,nsamp", [(2, 256, 70, 9036), (2, 1024, 40, 4100), (5, 300, 61, 7004)])
+def test_tma_u8_kernel_forced(idx, nchans, ndm, nsamp):
+    """AUTO prefers the partial-sum kernel for uint8; the byte-packed TMA kernel stays selectable and exact."""
+    w = small(idx, nchans, ndm, nsamp)
+    X, ms = make_case(w, pulses=3)
+    D = gpu_dedisperse(w, X, dd.DD_KERNEL_TMA)
+    assert_parity(w, X, D)
+    assert np.array_equal(D, gpu_dedisperse(w, X, dd.DD_KERNEL_AUTO))
+
+
 # ------------------------------------------------------------------ float32 partial-sum kernel, direct (aligned) path
 
 @pytest.mark.parametrize("idx,nchans,ndm,nsamp", [(3, 517, 130, 2000), (4, 256, 200, 1500), (3, 64, 40, 5000), (3, 130, 70, 600)])
