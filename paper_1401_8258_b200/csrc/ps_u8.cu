@@ -20,6 +20,7 @@
 //
 // Layout of a block: 16 consumer warps + 1 producer warp; consumer warp w owns trials
 // w*kKW .. w*kKW+kKW-1, lane l owns output samples t0 + 2 (l + 32 i) + {0,1}, i < kNK.
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -33,7 +34,8 @@ struct dd_psu8_plan {
     bool ok = false;
     int ntiles = 0, ngroups = 0;
     int desc_ints = 0;             // ints per (tile, group) descriptor (multiple of 4)
-    int xwb = 0;                   // bytes staged per byte-shifted copy of a channel (multiple of 16)
+    int xwb = 0;                   // bytes staged per row (one byte-shifted copy of one channel; multiple of 16)
+    int xstage = 0;                // bytes of one stage: 16 rows, 256 zero bytes, over-read slack
     int psw = 0;                   // words of one partial-sum buffer
     size_t smem = 0;
     int32_t* d_desc = nullptr;     // device [ntiles][ngroups][desc_ints]
@@ -58,8 +60,7 @@ constexpr int kChunk = 64;                // words (= 128 samples) of a partial-
 // descriptor layout (ints), one per (trial tile, channel group)
 constexpr int kDNChunks = 0;
 constexpr int kDBytes = 1;                // bytes of this descriptor that are in use (multiple of 16)
-constexpr int kDBase = 4;                 // [4]  first staged byte of channel k, relative to t0 (multiple of 16)
-constexpr int kDLen = 8;                  // [4]  bytes to stage per copy (multiple of 16; 0 for a missing channel)
+constexpr int kDBase = 4;                 // first staged sample of the group's rows, relative to t0 (multiple of 16)
 constexpr int kDTrial = 12;               // [kKB] word offset of trial j's first operand in the partial sums
 constexpr int kDChunk = kDTrial + kKB;    // [nchunks][4] byte offset, from the stage's first byte, of the
                                           //      aligned word lane 0 reads in channel k (zero pad if missing)
@@ -100,6 +101,14 @@ __device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t b
         ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar))
         : "memory");
 }
+// tile-mode tensor copy (SASS UTMALDG): box of the tensor map at (column c0, row c1) -> dense rows in smem
+__device__ __forceinline__ void tensor_load_2d(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar))
+        : "memory");
+}
 __device__ __forceinline__ void consumer_barrier()
 {
     asm volatile("bar.sync 1, %0;" ::"n"(kThreads) : "memory");
@@ -112,20 +121,18 @@ __device__ __forceinline__ uint32_t lds_u32(uint32_t addr)
 }
 
 struct PsU8Params {
-    const uint8_t* W;              // workspace: four byte-shifted copies, [4][nbeams*nchans][wpitch]
-    int64_t wcopy, wpitch;         // bytes between the copies / between channel rows of a copy
     int32_t* D;
     const int32_t* desc;
     const int32_t* order;
-    int nchans, ndm, ngroups, desc_ints, xwb, psw;
+    int nchans, ndm, ngroups, desc_ints, xwb, xstage, psw;
     int64_t nsamp, out_stride, out_beam_stride;
 };
 
 __global__ void __launch_bounds__(kThreads + 32, 1)
-dd_ps_u8_kernel(const PsU8Params p)
+dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
 {
     extern __shared__ __align__(128) uint8_t smem_raw[];
-    const int xstage = kG * 4 * p.xwb + 4 * kChunk;                            // bytes; the last 256 stay zero
+    const int xstage = p.xstage;                                               // bytes: 16 rows of xwb, 256 zero bytes, slack
     uint8_t* Xs = smem_raw;                                                    // [kXStages][xstage]
     uint32_t* Ps = reinterpret_cast<uint32_t*>(Xs + kXStages * xstage);        // [2][psw]
     int32_t* Ds = reinterpret_cast<int32_t*>(Ps + 2 * p.psw);                  // [kXStages][desc_ints]
@@ -133,6 +140,7 @@ dd_ps_u8_kernel(const PsU8Params p)
     uint64_t* empty = full + kXStages;                                         // [kXStages]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t xs0 = smem_u32(Xs);
     const int tile = blockIdx.x;                          // trial tiles fastest: neighbours share L2 lines
     const int64_t t0 = (int64_t)blockIdx.y * kTB;
     const int beam = blockIdx.z;
@@ -152,32 +160,25 @@ dd_ps_u8_kernel(const PsU8Params p)
 
     if (warp == kWarps) {
         // ---------------------------------------------------------------- producer warp
-        // lane 4 k + r stages copy r of channel k, lane 16 the descriptor; a stage is refilled as
-        // soon as all 16 consumer warps have released it.
+        // lane 0 stages the group's channel vectors and its descriptor; a stage is refilled as soon
+        // as all 16 consumer warps have released it.
         const int32_t* gdesc = p.desc + (int64_t)tile * ng * p.desc_ints;
-        const uint8_t* Wb = p.W + (int64_t)beam * p.nchans * p.wpitch + t0;
         for (int g = 0; g < ng; ++g) {
             const int st = g % kXStages;
             const int32_t* dg = gdesc + (int64_t)g * p.desc_ints;
             const int hv = lane < kDTrial ? __ldg(dg + lane) : 0;           // header words
-            const int base = __shfl_sync(0xffffffffu, hv, kDBase + ((lane >> 2) & 3));
-            const int len = __shfl_sync(0xffffffffu, hv, kDLen + ((lane >> 2) & 3));
+            const int base = __shfl_sync(0xffffffffu, hv, kDBase);
             const int dbytes = __shfl_sync(0xffffffffu, hv, kDBytes);
-            const uint32_t bytes = lane < 4 * kG ? (uint32_t)len : (lane == 4 * kG ? (uint32_t)dbytes : 0u);
-            uint32_t total = bytes;
-#pragma unroll
-            for (int o = 16; o >= 1; o >>= 1) total += __shfl_xor_sync(0xffffffffu, total, o);
             if (g >= kXStages) mbar_wait(&empty[st], ((g / kXStages) - 1) & 1);
-            if (lane == 0) mbar_arrive_expect_tx(&full[st], total);
-            __syncwarp();
-            if (lane < 4 * kG) {
-                if (len > 0)
-                    bulk_load(Xs + st * xstage + lane * p.xwb,
-                              Wb + (lane & 3) * p.wcopy + (int64_t)(g * kG + (lane >> 2)) * p.wpitch + base, bytes,
-                              &full[st]);
-            } else if (lane == 4 * kG) {
-                bulk_load(Ds + st * p.desc_ints, dg, bytes, &full[st]);
+            if (lane == 0) {
+                mbar_arrive_expect_tx(&full[st], (uint32_t)(4 * kG * p.xwb + dbytes));
+                // one tensor copy: 16 rows (4 channels x 4 byte-shifted copies) x xwb bytes, starting at
+                // sample t0 + base of every row (columns are counted in 8-byte elements)
+                tensor_load_2d(Xs + st * xstage, &tmap, (int)((t0 + base) >> 3), (beam * p.nchans + g * kG) * 4,
+                               &full[st]);
+                bulk_load(Ds + st * p.desc_ints, dg, (uint32_t)dbytes, &full[st]);
             }
+            __syncwarp();
         }
         return;
     }
@@ -185,24 +186,37 @@ dd_ps_u8_kernel(const PsU8Params p)
     // -------------------------------------------------------------------- consumer warps
     // Step 2: a warp step forms kChunk consecutive words (128 samples) of one pattern row and parity:
     // lane l reads the aligned word with samples 4l..4l+3 of every channel and writes words 2l, 2l+1.
-    auto pre = [&](int g, int buf) {
-        const int st = g % kXStages;
+    // The steps of group g+1 are interleaved with step 3 of group g (below) so that their
+    // shared-memory latency is covered by independent work.
+    struct Words { uint32_t w0, w1, w2, w3; };
+    auto pre_load = [&](uint32_t xa, const int4 o) {
+        Words r;
+        r.w0 = lds_u32(xa + o.x); r.w1 = lds_u32(xa + o.y); r.w2 = lds_u32(xa + o.z); r.w3 = lds_u32(xa + o.w);
+        return r;
+    };
+    auto pre_store = [&](uint2* ps, int c, const Words& r) {
+        // (b0 | b1 << 16) and (b2 | b3 << 16) of each channel word, summed over the channels
+        const uint32_t lo = __byte_perm(r.w0, 0, 0x4140) + __byte_perm(r.w1, 0, 0x4140) +
+                            __byte_perm(r.w2, 0, 0x4140) + __byte_perm(r.w3, 0, 0x4140);
+        const uint32_t hi = __byte_perm(r.w0, 0, 0x4342) + __byte_perm(r.w1, 0, 0x4342) +
+                            __byte_perm(r.w2, 0, 0x4342) + __byte_perm(r.w3, 0, 0x4342);
+        ps[c * (kChunk / 2)] = make_uint2(lo, hi);
+    };
+    // all steps of the group staged in stage `st`, two in flight per warp
+    auto pre = [&](int st, int buf) {
         const int32_t* ds = Ds + st * p.desc_ints;
-        const uint32_t xa = smem_u32(Xs + st * xstage) + lane * 4;
+        const uint32_t xa = xs0 + st * xstage + lane * 4;
         uint2* ps = reinterpret_cast<uint2*>(Ps + buf * p.psw) + lane;
         const int nchunks = ds[kDNChunks];
         const int4* ct = reinterpret_cast<const int4*>(ds + kDChunk);
-        for (int c = warp; c < nchunks; c += kWarps) {
-            const int4 o = ct[c];
-            const uint32_t w0 = lds_u32(xa + o.x), w1 = lds_u32(xa + o.y), w2 = lds_u32(xa + o.z),
-                           w3 = lds_u32(xa + o.w);
-            // (b0 | b1 << 16) and (b2 | b3 << 16) of each channel word, summed over the channels
-            const uint32_t lo = (__byte_perm(w0, 0, 0x4140) + __byte_perm(w1, 0, 0x4140)) +
-                                (__byte_perm(w2, 0, 0x4140) + __byte_perm(w3, 0, 0x4140));
-            const uint32_t hi = (__byte_perm(w0, 0, 0x4342) + __byte_perm(w1, 0, 0x4342)) +
-                                (__byte_perm(w2, 0, 0x4342) + __byte_perm(w3, 0, 0x4342));
-            ps[c * (kChunk / 2)] = make_uint2(lo, hi);
+        int c = warp;
+        for (; c + kWarps < nchunks; c += 2 * kWarps) {
+            const int4 ea = ct[c], eb = ct[c + kWarps];
+            const Words a = pre_load(xa, ea), b = pre_load(xa, eb);
+            pre_store(ps, c, a);
+            pre_store(ps, c + kWarps, b);
         }
+        if (c < nchunks) pre_store(ps, c, pre_load(xa, ct[c]));
     };
 
     uint32_t acc[kKW][kNK];
@@ -255,11 +269,12 @@ dd_ps_u8_kernel(const PsU8Params p)
     pre(0, 0);
     consumer_barrier();
 
+    // st: stage of group g; sn / phn: stage and phase parity of group g + 1
+    int st = 0, sn = 1 % kXStages, phn = kXStages == 1 ? 1 : 0, flush_in = kFlushGroups;
     for (int g = 0; g < ng; ++g) {
-        const int st = g % kXStages;
         if (g + 1 < ng) {
-            mbar_wait(&full[(g + 1) % kXStages], ((g + 1) / kXStages) & 1);
-            pre(g + 1, (g + 1) & 1);
+            mbar_wait(&full[sn], phn);
+            pre(sn, (g + 1) & 1);
         }
         // Step 3: one word per trial, sample pair and group
         const int4 tr = *reinterpret_cast<const int4*>(Ds + st * p.desc_ints + kDTrial + warp * kKW);
@@ -274,7 +289,9 @@ dd_ps_u8_kernel(const PsU8Params p)
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[st]);          // stage st (vectors and descriptor) may be refilled
         consumer_barrier();                              // partial sums of g+1 complete, those of g consumed
-        if (((g + 1) % kFlushGroups) == 0 && g + 1 < ng) flush();
+        st = sn;
+        if (++sn == kXStages) { sn = 0; phn ^= 1; }
+        if (--flush_in == 0 && g + 1 < ng) { flush(); flush_in = kFlushGroups; }
     }
     flush();
 }
@@ -288,9 +305,21 @@ int build_psu8_plan(dd_plan* p)
     const HostTable& h = p->host;
     const int nch = p->nchans, ndm = p->ndm;
     const int ntiles = (ndm + kKB - 1) / kKB, ngroups = (nch + kG - 1) / kG;
-    const int64_t spread = max_tile_spread(h, kKB);
-    const int64_t xwb = (kTB + spread + 16 + 2 * kChunk + 128 + 16 + 15) / 16 * 16;
-    if (xwb > 8192) return DD_OK;                         // per-trial steps too large: other kernels
+    // staged bytes per row: from the 16-byte aligned start of the group's first channel at the tile's
+    // first trial to the end of the window of its last channel at the tile's last trial
+    int64_t xwb = 0;
+    for (int tile = 0; tile < ntiles; ++tile) {
+        const int dfirst = tile * kKB, dlast = std::min(tile * kKB + kKB, ndm) - 1;
+        for (int g = 0; g < ngroups; ++g) {
+            const int c0 = g * kG, c1 = std::min(c0 + kG, nch) - 1;
+            const int64_t b = h.shift[(size_t)dfirst * nch + c0] & ~15;
+            xwb = std::max<int64_t>(xwb, h.shift[(size_t)dlast * nch + c1] + kTB - b);
+        }
+    }
+    xwb = (xwb + 15) / 16 * 16;
+    if (xwb > 2048) return DD_OK;                         // wider than a tensor-copy box (256 x 8 bytes)
+    // a warp step of step 2 may read up to 2 * kChunk + 128 bytes past a row's window
+    const int64_t xstage = (kG * 4 * xwb + 4 * kChunk + 2 * kChunk + 128 + 127) / 128 * 128;
 
     // words of one parity copy of a pattern row: the largest offset of a trial in it, halved, plus
     // the kTB / 2 words every trial reads, in whole warp steps
@@ -306,7 +335,7 @@ int build_psu8_plan(dd_plan* p)
             psw = std::max(psw, w);
         }
     const int desc_ints = kDChunk + 4 * (int)(psw / kChunk);
-    const size_t smem = (size_t)kXStages * (kG * 4 * xwb + 4 * kChunk) + (size_t)2 * psw * 4 +
+    const size_t smem = (size_t)kXStages * xstage + (size_t)2 * psw * 4 +
                         (size_t)kXStages * desc_ints * 4 + 2 * kXStages * 8;
     if (smem > (size_t)kMaxSmem) return DD_OK;            // too many patterns for shared memory
 
@@ -317,6 +346,7 @@ int build_psu8_plan(dd_plan* p)
     t->ngroups = ngroups;
     t->desc_ints = desc_ints;
     t->xwb = (int)xwb;
+    t->xstage = (int)xstage;
     t->psw = (int)psw;
     t->smem = smem;
 
@@ -335,13 +365,9 @@ int build_psu8_plan(dd_plan* p)
             int32_t* ds = &desc[((size_t)tile * ngroups + g) * desc_ints];
             const int c0 = g * kG, nk = std::min(kG, nch - c0);
             const int dfirst = tile * kKB, dlast = std::min(tile * kKB + kKB, ndm) - 1;
-            int base[kG] = {0, 0, 0, 0};
-            for (int k = 0; k < nk; ++k) {
-                const int smin = h.shift[(size_t)dfirst * nch + c0 + k], smax = h.shift[(size_t)dlast * nch + c0 + k];
-                base[k] = smin & ~15;
-                ds[kDBase + k] = base[k];
-                ds[kDLen + k] = (smax + kTB - base[k] + 15) / 16 * 16;
-            }
+            const int base = h.shift[(size_t)dfirst * nch + c0] & ~15;   // channel c0 has the smallest delay
+            ds[kDBase] = base;
+            (void)dlast;
             int flat = 0;                                 // words
             rowbase.assign(2 * rows.size(), 0);
             for (size_t r = 0; r < rows.size(); ++r)
@@ -351,13 +377,13 @@ int build_psu8_plan(dd_plan* p)
                     // word w of this copy holds the partial sums of u = umin + par + 2 w and u + 1;
                     // a warp step makes words [kChunk c, kChunk c + kChunk): lane l reads, per channel
                     // k, the aligned word with samples x_k[u0 + r_k + 4 l ..+3], u0 = umin + par + 128 c,
-                    // i.e. byte a0 + 4 l of the staged window, a0 = u0 + r_k - base_k: copy (a0 & 3),
+                    // i.e. byte a0 + 4 l of the staged rows, a0 = u0 + r_k - base: copy (a0 & 3),
                     // word (a0 >> 2) + l
                     for (int c = 0; c < nw / kChunk; ++c) {
                         int32_t* ce = ds + kDChunk + 4 * (flat / kChunk + c);
                         for (int k = 0; k < kG; ++k) {
                             const int rk = k == 0 ? 0 : rows[r].key[k - 1];
-                            const int a0 = rows[r].umin + par + 2 * kChunk * c + rk - base[k];
+                            const int a0 = rows[r].umin + par + 2 * kChunk * c + rk - base;
                             ce[k] = k < nk ? (4 * k + (a0 & 3)) * t->xwb + (a0 & ~3) : zero_pad;
                         }
                     }
@@ -408,21 +434,53 @@ bool psu8_args_ok(const dd_plan* p, const ExecArgs& a)
     if (((uintptr_t)a.D & 15) || (a.out_stride & 3) || (a.nbeams > 1 && (a.out_beam_stride & 3))) return false;
     if ((a.nsamp_out + kTB - 1) / kTB > 65535 || a.nbeams > 65535) return false;
     if ((int64_t)a.nbeams * p->nchans > 65535) return false;          // grid.y of the front end
+    if ((a.nsamp_out + p->host.maxshift + 4096) / 8 >= ((int64_t)1 << 31)) return false;   // tensor coordinates
     return true;
+}
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_tiled()
+{
+    static EncodeTiledFn fn = [] {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &qr) != cudaSuccess ||
+            qr != cudaDriverEntryPointSuccess) {
+            cudaGetLastError();
+            f = nullptr;
+        }
+        return (EncodeTiledFn)f;
+    }();
+    return fn;
 }
 
 int launch_psu8(const dd_plan* p, const ExecArgs& a)
 {
     const dd_psu8_plan* t = p->psu8;
     cudaStream_t st = (cudaStream_t)a.stream;
+    EncodeTiledFn enc = encode_tiled();
+    if (!enc) return fail(DD_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
     uint8_t* W = nullptr;
     int64_t wcopy = 0, wpitch = 0;
     int rc = make_shift_copies_u8(p, a, &W, &wcopy, &wpitch);
     if (rc != DD_OK) return rc;
+    // the workspace as a 2-D tensor of 8-byte elements: rows = (beam, channel, copy), wcopy bytes apart
+    CUtensorMap tmap;
+    const cuuint64_t dims[2] = {(cuuint64_t)(wcopy / 8), (cuuint64_t)a.nbeams * p->nchans * 4};
+    const cuuint64_t strides[1] = {(cuuint64_t)wcopy};
+    const cuuint32_t box[2] = {(cuuint32_t)(t->xwb / 8), 4 * kG};
+    const cuuint32_t estr[2] = {1, 1};
+    CUresult cr = enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT64, 2, W, dims, strides, box, estr,
+                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (cr != CUDA_SUCCESS) {
+        cudaFreeAsync(W, st);
+        return fail(DD_ERR_CUDA, "cuTensorMapEncodeTiled failed (" + std::to_string((int)cr) + ")");
+    }
     PsU8Params q;
-    q.W = W;
-    q.wcopy = wcopy;
-    q.wpitch = wpitch;
     q.D = (int32_t*)a.D;
     q.desc = t->d_desc;
     q.order = a.d_order;
@@ -431,12 +489,13 @@ int launch_psu8(const dd_plan* p, const ExecArgs& a)
     q.ngroups = t->ngroups;
     q.desc_ints = t->desc_ints;
     q.xwb = t->xwb;
+    q.xstage = t->xstage;
     q.psw = t->psw;
     q.nsamp = a.nsamp_out;
     q.out_stride = a.out_stride;
     q.out_beam_stride = a.out_beam_stride;
     dim3 grid((unsigned)t->ntiles, (unsigned)((a.nsamp_out + kTB - 1) / kTB), (unsigned)a.nbeams);
-    dd_ps_u8_kernel<<<grid, kThreads + 32, t->smem, st>>>(q);
+    dd_ps_u8_kernel<<<grid, kThreads + 32, t->smem, st>>>(q, tmap);
     cudaError_t e = cudaGetLastError();
     cudaFreeAsync(W, st);
     if (e != cudaSuccess) return fail(DD_ERR_CUDA, std::string("ps u8 launch: ") + cudaGetErrorString(e));

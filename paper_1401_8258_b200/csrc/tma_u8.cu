@@ -412,11 +412,13 @@ int make_shift_copies_u8(const dd_plan* p, const ExecArgs& a, uint8_t** W_out, i
 {
     cudaStream_t st = (cudaStream_t)a.stream;
     const int64_t rowlen = a.nsamp_out + p->host.maxshift;            // valid samples per channel row
-    const int64_t wpitch = (rowlen + (int64_t)kMaxNY * kBoxW + 16 + 127) / 128 * 128;
+    // layout [beam * nchans + channel][copy r][wcopy bytes]: the four copies of a channel are adjacent
+    // rows (ps_u8.cu fetches the 16 rows of a four-channel group with one tensor copy)
+    const int64_t wcopy = (rowlen + (int64_t)kMaxNY * kBoxW + 16 + 127) / 128 * 128;
+    const int64_t wpitch = 4 * wcopy;
     const int64_t nrows = (int64_t)a.nbeams * p->nchans;
-    const int64_t wcopy = nrows * wpitch;
     uint8_t* W = nullptr;
-    cudaError_t e = cudaMallocAsync((void**)&W, (size_t)(4 * wcopy), st);
+    cudaError_t e = cudaMallocAsync((void**)&W, (size_t)(nrows * wpitch), st);
     if (e != cudaSuccess) {
         cudaGetLastError();
         return fail(DD_ERR_NOMEM, std::string("byte-shifted workspace: ") + cudaGetErrorString(e));
