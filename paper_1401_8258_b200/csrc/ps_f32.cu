@@ -104,10 +104,6 @@ __device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t b
         ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar))
         : "memory");
 }
-__device__ __forceinline__ void consumer_barrier()
-{
-    asm volatile("bar.sync 1, %0;" ::"n"(kThreads) : "memory");
-}
 __device__ __forceinline__ float lds_f32(uint32_t addr)
 {
     float v;
@@ -136,6 +132,8 @@ dd_ps_f32_kernel(const PsParams p)
     int32_t* Ds = reinterpret_cast<int32_t*>(Ps + 2 * p.psw);                  // [kXStages][desc_ints]
     uint64_t* full = reinterpret_cast<uint64_t*>(Ds + kXStages * p.desc_ints); // [kXStages]
     uint64_t* empty = full + kXStages;                                         // [kXStages]
+    uint64_t* ready = empty + kXStages;                                        // [2] partial sums complete
+    uint64_t* freeb = ready + 2;                                               // [2] partial sums consumed
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int tile = blockIdx.x;                          // trial tiles fastest: neighbours share L2 lines
@@ -147,6 +145,10 @@ dd_ps_f32_kernel(const PsParams p)
         for (int s = 0; s < kXStages; ++s) {
             mbar_init(&full[s], 1);
             mbar_init(&empty[s], kWarps);
+        }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(&ready[b], kWarps);
+            mbar_init(&freeb[b], kWarps);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -191,8 +193,7 @@ dd_ps_f32_kernel(const PsParams p)
     // -------------------------------------------------------------------- consumer warps
     // Step 2: the pattern rows of group g into partial-sum buffer `buf`; a warp step forms kChunk
     // consecutive words (lane l: words l and l + 32) from one descriptor entry of G byte offsets.
-    auto pre = [&](int g, int buf) {
-        const int st = g % kXStages;
+    auto pre = [&](int st, int buf) {
         const int32_t* ds = Ds + st * p.desc_ints;
         const uint32_t xa = smem_u32(Xs + st * xstage) + lane * 4;
         float* ps = Ps + buf * p.psw + lane;
@@ -225,20 +226,29 @@ dd_ps_f32_kernel(const PsParams p)
 #pragma unroll
         for (int i = 0; i < kNK; ++i) acc[j][i] = 0.0f;
 
+    // Warps synchronise through split-phase barriers instead of a block barrier: ready[b] completes
+    // when all 16 warps have written their part of partial-sum buffer b, freeb[b] when all have
+    // consumed it; a warp only waits if another one is a whole phase behind.
     mbar_wait(&full[0], 0);
     pre(0, 0);
-    consumer_barrier();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&ready[0]);
 
+    int st = 0, sn = 1 % kXStages, phn = kXStages == 1 ? 1 : 0;
     for (int g = 0; g < ng; ++g) {
-        const int st = g % kXStages;
+        const int b = g & 1;
         if (g + 1 < ng) {
-            mbar_wait(&full[(g + 1) % kXStages], ((g + 1) / kXStages) & 1);
-            pre(g + 1, (g + 1) & 1);
+            mbar_wait(&full[sn], phn);
+            if (g >= 1) mbar_wait(&freeb[b ^ 1], ((g - 1) >> 1) & 1);      // step 3 of g-1 is done everywhere
+            pre(sn, b ^ 1);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&ready[b ^ 1]);
         }
         // Step 3: one word per trial, sample and group
         const int4 tr = *reinterpret_cast<const int4*>(Ds + st * p.desc_ints + kDTrial + warp * kKW);
         const int tro[kKW] = {tr.x, tr.y, tr.z, tr.w};
-        const float* ps = Ps + (g & 1) * p.psw + lane;
+        const float* ps = Ps + b * p.psw + lane;
+        mbar_wait(&ready[b], (g >> 1) & 1);                                // step 2 of g is done everywhere
 #pragma unroll
         for (int j = 0; j < kKW; ++j) {
             const float* r = ps + tro[j];
@@ -246,8 +256,12 @@ dd_ps_f32_kernel(const PsParams p)
             for (int i = 0; i < kNK; ++i) acc[j][i] += r[32 * i];
         }
         __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[st]);          // stage st (vectors and descriptor) may be refilled
-        consumer_barrier();                              // partial sums of g+1 complete, those of g consumed
+        if (lane == 0) {
+            mbar_arrive(&freeb[b]);
+            mbar_arrive(&empty[st]);                     // stage st (vectors and descriptor) may be refilled
+        }
+        st = sn;
+        if (++sn == kXStages) { sn = 0; phn ^= 1; }
     }
 
     float* Db = p.D + (int64_t)beam * p.out_beam_stride;
@@ -303,7 +317,7 @@ PsShape shape_for(const HostTable& h, int G)
         }
     o.desc_ints = kDChunk + G * (int)(o.psw / kChunk);
     o.smem = (size_t)kXStages * (G * o.xw + kChunk) * 4 + (size_t)2 * o.psw * 4 +
-             (size_t)kXStages * o.desc_ints * 4 + 2 * kXStages * 8;
+             (size_t)kXStages * o.desc_ints * 4 + (2 * kXStages + 4) * 8;
     o.fits = o.xw <= 16384 && o.smem <= (size_t)kMaxSmem;
     o.cost = (double)ntiles * ngroups * kKB * kNK + (double)chunks * (2 * G + 2 + G / 4);
     return o;
