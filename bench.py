@@ -24,7 +24,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_1401_8258_b200 import synth  # noqa: E402
+from paper_1401_8258_b200 import sharding, synth  # noqa: E402
 
 METRIC = "dedispersed DM·channel·samples/s"
 UNIT = "G/s"
@@ -180,9 +180,9 @@ def run_ours(args, w):
     # host input: pinned, one beam per rank-beam (rank r uses beam seeds r*nb .. r*nb+nb-1)
     Xh = torch.empty((nb, w.nchans, in_stride), dtype=tdt).pin_memory()
     Xh.zero_()
-    for b in range(nb):
-        wb = synth.scaled(w, nbeams=max(2, nb * world))       # per-beam seeds
-        Xh[b, :, :w.nsamp + ms] = torch.from_numpy(synth.make_input(wb, w.nsamp + ms, beam=rank * nb + b))
+    wb = synth.scaled(w, nbeams=max(2, nb * world))           # per-beam seeds
+    for b, beam in enumerate(sharding.beams_of_rank(rank, world, nb)):
+        Xh[b, :, :w.nsamp + ms] = torch.from_numpy(synth.make_input(wb, w.nsamp + ms, beam=beam))
     Xd = Xh.cuda()
     Dd = torch.empty((nb, w.ndm, out_stride), dtype=odt, device="cuda")
     stream = torch.cuda.Stream()
@@ -234,13 +234,10 @@ def run_ours(args, w):
     clocks = sampler.result()
     total_ms = ev[0].elapsed_time(ev[-1])
     per_step = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
-    if dist is not None:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = sharding.max_over_ranks(total_ms, dist, "cuda")
     ms_per_step = total_ms / args.steps
     adds_rank = w.adds
-    value = adds_rank * world / (ms_per_step * 1e-3) / 1e9
+    value = sharding.whole_job_rate(adds_rank, world, ms_per_step * 1e-3) / 1e9
 
     # ---- end to end through the host-buffer C-ABI call (pinned host X and D; copies inside)
     e2e = None
@@ -255,12 +252,9 @@ def run_ours(args, w):
             plan.execute_host(Xh[0], in_stride, Dh, out_stride, w.nsamp)
         torch.cuda.synchronize()
         dt = (time.perf_counter() - t0) / n_e2e
-        if dist is not None:
-            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = sharding.max_over_ranks(dt, dist, "cuda")
         es = 4 if w.dtype == "f32" else 1
-        e2e = {"value": adds_rank * world / dt / 1e9, "unit": UNIT,
+        e2e = {"value": sharding.whole_job_rate(adds_rank, world, dt) / 1e9, "unit": UNIT,
                "h2d_bytes_per_step": int(w.nchans * (w.nsamp + ms) * es),
                "d2h_bytes_per_step": int(w.ndm * w.nsamp * 4), "ms_per_step": dt * 1e3,
                "timer": "host wall clock around the synchronous dd_execute_host call, pinned buffers"}
@@ -273,6 +267,11 @@ def run_ours(args, w):
         kernel_ms = float(np.mean(per_step))
         achieved = adds_rank / (kernel_ms * 1e-3) / 1e12
         hbm_bytes = nb * (w.nchans * (w.nsamp + ms) * (4 if w.dtype == "f32" else 1) + w.ndm * w.nsamp * 4)
+        hbm_peak = None
+        try:
+            hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs")
+        except (OSError, ValueError):
+            pass
         traffic = None
         try:
             for ln in open(os.path.join(ROOT, "profiles", "dram_traffic.txt")):
@@ -298,8 +297,14 @@ def run_ours(args, w):
                          "kernel_ms": kernel_ms,
                          "frac_at_sampled_clock": (achieved / (SM_COUNT * LANES_PER_SM * clocks["sm_mhz"] * 1e6 / 1e12)
                                                    if clocks["sm_mhz"] else None),
+                         "algorithmic_adds_per_launch": adds_rank,
+                         "work_note": ("achieved = nbeams*nchans*ndm*nsamp adds (one per DM-channel-sample, SURVEY "
+                                       "8(d)) / CUDA-event time of the step; the ps kernels form each output from the "
+                                       "same operands but share partial sums of 4-8 channels between trials "
+                                       "(DESIGN.md 5.3), so fewer add instructions are issued"),
                          "hbm_algorithmic_bytes": hbm_bytes,
-                         "hbm_achieved_gbs": hbm_bytes / (kernel_ms * 1e-3) / 1e9},
+                         "hbm_achieved_gbs": hbm_bytes / (kernel_ms * 1e-3) / 1e9,
+                         "hbm_peak_gbs_measured": hbm_peak},
             "clocks": clocks, "gpu_launches": launches,
         }
         if e2e is not None:
