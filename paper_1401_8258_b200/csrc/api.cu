@@ -51,6 +51,40 @@ static int require_sm100(int* device_out)
 
 static size_t elem_size(int dtype) { return dtype == DD_F32 ? 4 : 1; }
 
+// Per-call workspaces (byte-shifted copies, re-pitched input) come from a stream-ordered pool of the
+// library's own that keeps its memory between calls (release threshold = max): the default pool
+// would return the memory at the next synchronisation and the following call would pay for a
+// fresh physical allocation.
+int workspace_alloc(void** out, size_t bytes, void* stream)
+{
+    static cudaMemPool_t pools[64] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess && dev >= 0 && dev < 64 && !pools[dev]) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t pool = nullptr;
+        e = cudaMemPoolCreate(&pool, &props);
+        if (e == cudaSuccess) {
+            uint64_t keep = UINT64_MAX;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+            pools[dev] = pool;
+        }
+    }
+    if (e == cudaSuccess && dev >= 0 && dev < 64 && pools[dev])
+        e = cudaMallocFromPoolAsync(out, bytes, pools[dev], (cudaStream_t)stream);
+    else if (e == cudaSuccess)
+        e = cudaMallocAsync(out, bytes, (cudaStream_t)stream);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(DD_ERR_NOMEM, std::string("workspace allocation: ") + cudaGetErrorString(e));
+    }
+    return DD_OK;
+}
+
 }  // namespace dd
 
 using namespace dd;

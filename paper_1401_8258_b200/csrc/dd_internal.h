@@ -14,6 +14,9 @@ namespace dd {
 void set_error(const std::string& msg);
 int fail(int code, const std::string& msg);
 
+// stream-ordered workspace from the library's own pool (api.cu); free with cudaFreeAsync
+int workspace_alloc(void** out, size_t bytes, void* stream);
+
 // ---- host delay table (plan.cpp; eq 2.2/2.3) ------------------------------
 struct HostTable {
     int nchans = 0;

@@ -466,11 +466,8 @@ int launch_ps(const dd_plan* p, const ExecArgs& a)
     if (!ps_direct(a)) {
         const int64_t wpitch = (rowlen + 3) / 4 * 4;
         const int64_t nrows = (int64_t)a.nbeams * p->nchans;
-        cudaError_t e = cudaMallocAsync((void**)&W, (size_t)(nrows * wpitch) * sizeof(float), st);
-        if (e != cudaSuccess) {
-            cudaGetLastError();
-            return fail(DD_ERR_NOMEM, std::string("re-pitch workspace: ") + cudaGetErrorString(e));
-        }
+        int rc = workspace_alloc((void**)&W, (size_t)(nrows * wpitch) * sizeof(float), a.stream);
+        if (rc != DD_OK) return rc;
         dim3 grid((unsigned)std::min<int64_t>((wpitch + 255) / 256, 64), (unsigned)nrows);
         dd_repitch_f32<<<grid, 256, 0, st>>>((const float*)a.X, W, p->nchans, rowlen, a.in_stride, a.in_beam_stride,
                                              wpitch);

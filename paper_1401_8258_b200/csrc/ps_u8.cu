@@ -10,7 +10,9 @@
 //   2. forms, per pattern, the row of partial sums P[u] = x0[u] + x1[u+r1] + x2[u+r2] + x3[u+r3]
 //      (<= 4*255, so 16 bits) TWICE, as 32-bit words holding (P[u], P[u+1]) for even and for odd u:
 //      one aligned LDS gives four consecutive samples of a channel, two PRMT widen them into two
-//      words of 16-bit lanes, three adds per word sum the channels;
+//      words of 16-bit lanes, adds sum the channels -> the even-u words; the odd-u words are cut
+//      from those and the neighbouring lane's (one SHFL, two PRMT); warp steps overlap by one
+//      lane (124 new samples per step) so that no step needs its successor;
 //   3. adds ONE word per trial, per PAIR of output samples and per group:
 //      acc(16-bit lanes) += P^{parity}_{pattern(d)}[(t + s(d,c0)) / 2].
 // Step 3 is one shared-memory word and one integer add per EIGHT channel-sample adds (Alg. 1,
@@ -55,15 +57,18 @@ constexpr int kTB = 2 * 32 * kNK;         // output samples per block
 constexpr int kXStages = 3;
 constexpr int kMaxSmem = 200 * 1024;
 constexpr int kFlushGroups = 64;          // 64 groups * 4 channels * 255 = 65280 < 65536
-constexpr int kChunk = 64;                // words (= 128 samples) of a partial-sum row per warp step
+constexpr int kChunk = 64;                // even-u words (= 128 samples) a warp step writes ...
+constexpr int kStepW = 62;                // ... of which the last two are rewritten by the next step
+constexpr int kCE = 8;                    // ints per step entry of the descriptor
 
 // descriptor layout (ints), one per (trial tile, channel group)
 constexpr int kDNChunks = 0;
 constexpr int kDBytes = 1;                // bytes of this descriptor that are in use (multiple of 16)
 constexpr int kDBase = 4;                 // first staged sample of the group's rows, relative to t0 (multiple of 16)
 constexpr int kDTrial = 12;               // [kKB] word offset of trial j's first operand in the partial sums
-constexpr int kDChunk = kDTrial + kKB;    // [nchunks][4] byte offset, from the stage's first byte, of the
-                                          //      aligned word lane 0 reads in channel k (zero pad if missing)
+constexpr int kDChunk = kDTrial + kKB;    // [nchunks][kCE]: [0..3] byte offset, from the stage's first byte, of the
+                                          //      aligned word lane 0 reads in channel k (zero pad if missing);
+                                          //      [4], [5] first even-u / odd-u word the step writes (even numbers)
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
@@ -194,29 +199,35 @@ dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
         r.w0 = lds_u32(xa + o.x); r.w1 = lds_u32(xa + o.y); r.w2 = lds_u32(xa + o.z); r.w3 = lds_u32(xa + o.w);
         return r;
     };
-    auto pre_store = [&](uint2* ps, int c, const Words& r) {
-        // (b0 | b1 << 16) and (b2 | b3 << 16) of each channel word, summed over the channels
+    auto pre_store = [&](uint32_t* ps, const int4 dst, const Words& r) {
+        // (b0 | b1 << 16) and (b2 | b3 << 16) of each channel word, summed over the channels:
+        // partial sums S0..S3 of this lane's four samples
         const uint32_t lo = __byte_perm(r.w0, 0, 0x4140) + __byte_perm(r.w1, 0, 0x4140) +
                             __byte_perm(r.w2, 0, 0x4140) + __byte_perm(r.w3, 0, 0x4140);
         const uint32_t hi = __byte_perm(r.w0, 0, 0x4342) + __byte_perm(r.w1, 0, 0x4342) +
                             __byte_perm(r.w2, 0, 0x4342) + __byte_perm(r.w3, 0, 0x4342);
-        ps[c * (kChunk / 2)] = make_uint2(lo, hi);
+        *reinterpret_cast<uint2*>(ps + dst.x + 2 * lane) = make_uint2(lo, hi);             // (S0,S1) (S2,S3)
+        const uint32_t nlo = __shfl_down_sync(0xffffffffu, lo, 1);                        // next lane's (S0,S1)
+        if (lane < 31)                                                                    // (S1,S2) (S3,S4)
+            *reinterpret_cast<uint2*>(ps + dst.y + 2 * lane) =
+                make_uint2(__byte_perm(lo, hi, 0x5432), __byte_perm(hi, nlo, 0x5432));
     };
     // all steps of the group staged in stage `st`, two in flight per warp
     auto pre = [&](int st, int buf) {
         const int32_t* ds = Ds + st * p.desc_ints;
         const uint32_t xa = xs0 + st * xstage + lane * 4;
-        uint2* ps = reinterpret_cast<uint2*>(Ps + buf * p.psw) + lane;
+        uint32_t* ps = Ps + buf * p.psw;
         const int nchunks = ds[kDNChunks];
         const int4* ct = reinterpret_cast<const int4*>(ds + kDChunk);
         int c = warp;
         for (; c + kWarps < nchunks; c += 2 * kWarps) {
-            const int4 ea = ct[c], eb = ct[c + kWarps];
+            const int4 ea = ct[2 * c], eb = ct[2 * (c + kWarps)];
+            const int4 da = ct[2 * c + 1], db = ct[2 * (c + kWarps) + 1];
             const Words a = pre_load(xa, ea), b = pre_load(xa, eb);
-            pre_store(ps, c, a);
-            pre_store(ps, c + kWarps, b);
+            pre_store(ps, da, a);
+            pre_store(ps, db, b);
         }
-        if (c < nchunks) pre_store(ps, c, pre_load(xa, ct[c]));
+        if (c < nchunks) pre_store(ps, ct[2 * c + 1], pre_load(xa, ct[2 * c]));
     };
 
     uint32_t acc[kKW][kNK];
@@ -319,22 +330,27 @@ int build_psu8_plan(dd_plan* p)
     xwb = (xwb + 15) / 16 * 16;
     if (xwb > 2048) return DD_OK;                         // wider than a tensor-copy box (256 x 8 bytes)
     // a warp step of step 2 may read up to 2 * kChunk + 128 bytes past a row's window
-    const int64_t xstage = (kG * 4 * xwb + 4 * kChunk + 2 * kChunk + 128 + 127) / 128 * 128;
+    const int64_t xstage = (kG * 4 * xwb + 4 * kChunk + 384 + 127) / 128 * 128;
 
     // words of one parity copy of a pattern row: the largest offset of a trial in it, halved, plus
     // the kTB / 2 words every trial reads, in whole warp steps
-    auto row_words = [](const PsRow& r) { return ((r.umax - r.umin) / 2 + kTB / 2 + kChunk - 1) / kChunk * kChunk; };
+    // warp steps of a pattern row: step c writes even-u words [62 c, 62 c + 64) and odd-u words [62 c, 62 c + 62)
+    auto row_steps = [](const PsRow& r) { return ((r.umax - r.umin) / 2 + kTB / 2 + kStepW - 1) / kStepW; };
     std::vector<PsRow> rows;
     int slot[kKB];
-    int64_t psw = 0;
+    int64_t psw = 0, max_steps = 0;
     for (int tile = 0; tile < ntiles; ++tile)
         for (int g = 0; g < ngroups; ++g) {
             ps_classify(h, kG, kKB, tile, g, rows, slot);
-            int64_t w = 0;
-            for (const PsRow& r : rows) w += 2 * row_words(r);
+            int64_t w = 0, n = 0;
+            for (const PsRow& r : rows) {
+                n += row_steps(r);
+                w += 2 * (kStepW * row_steps(r) + 2);
+            }
             psw = std::max(psw, w);
+            max_steps = std::max(max_steps, n);
         }
-    const int desc_ints = kDChunk + 4 * (int)(psw / kChunk);
+    const int desc_ints = kDChunk + kCE * (int)max_steps;
     const size_t smem = (size_t)kXStages * xstage + (size_t)2 * psw * 4 +
                         (size_t)kXStages * desc_ints * 4 + 2 * kXStages * 8;
     if (smem > (size_t)kMaxSmem) return DD_OK;            // too many patterns for shared memory
@@ -368,29 +384,29 @@ int build_psu8_plan(dd_plan* p)
             const int base = h.shift[(size_t)dfirst * nch + c0] & ~15;   // channel c0 has the smallest delay
             ds[kDBase] = base;
             (void)dlast;
-            int flat = 0;                                 // words
+            int flat = 0, step = 0;                       // words, warp steps
             rowbase.assign(2 * rows.size(), 0);
-            for (size_t r = 0; r < rows.size(); ++r)
-                for (int par = 0; par < 2; ++par) {
-                    rowbase[2 * r + par] = flat;
-                    const int nw = row_words(rows[r]);
-                    // word w of this copy holds the partial sums of u = umin + par + 2 w and u + 1;
-                    // a warp step makes words [kChunk c, kChunk c + kChunk): lane l reads, per channel
-                    // k, the aligned word with samples x_k[u0 + r_k + 4 l ..+3], u0 = umin + par + 128 c,
-                    // i.e. byte a0 + 4 l of the staged rows, a0 = u0 + r_k - base: copy (a0 & 3),
-                    // word (a0 >> 2) + l
-                    for (int c = 0; c < nw / kChunk; ++c) {
-                        int32_t* ce = ds + kDChunk + 4 * (flat / kChunk + c);
-                        for (int k = 0; k < kG; ++k) {
-                            const int rk = k == 0 ? 0 : rows[r].key[k - 1];
-                            const int a0 = rows[r].umin + par + 2 * kChunk * c + rk - base;
-                            ce[k] = k < nk ? (4 * k + (a0 & 3)) * t->xwb + (a0 & ~3) : zero_pad;
-                        }
+            for (size_t r = 0; r < rows.size(); ++r) {
+                const int ns = row_steps(rows[r]);
+                rowbase[2 * r] = flat;                                // even-u words: (P[umin + 2 w], P[umin + 2 w + 1])
+                rowbase[2 * r + 1] = flat + kStepW * ns + 2;          // odd-u words:  (P[umin + 2 w + 1], P[umin + 2 w + 2])
+                // step c: lane l reads, per channel k, the aligned word with samples
+                // x_k[u0 + r_k + 4 l ..+3], u0 = umin + 124 c, i.e. byte a0 + 4 l of the staged rows,
+                // a0 = u0 + r_k - base: copy (a0 & 3), word (a0 >> 2) + l
+                for (int c = 0; c < ns; ++c, ++step) {
+                    int32_t* ce = ds + kDChunk + kCE * step;
+                    for (int k = 0; k < kG; ++k) {
+                        const int rk = k == 0 ? 0 : rows[r].key[k - 1];
+                        const int a0 = rows[r].umin + 2 * kStepW * c + rk - base;
+                        ce[k] = k < nk ? (4 * k + (a0 & 3)) * t->xwb + (a0 & ~3) : zero_pad;
                     }
-                    flat += nw;
+                    ce[4] = rowbase[2 * r] + kStepW * c;
+                    ce[5] = rowbase[2 * r + 1] + kStepW * c;
                 }
-            ds[kDNChunks] = flat / kChunk;
-            ds[kDBytes] = 4 * (kDChunk + 4 * (flat / kChunk));
+                flat += 2 * (kStepW * ns + 2);
+            }
+            ds[kDNChunks] = step;
+            ds[kDBytes] = 4 * (kDChunk + kCE * step);
             for (int j = 0; j < kKB; ++j) {
                 const int d = std::min(tile * kKB + j, ndm - 1);
                 const int o = h.shift[(size_t)d * nch + c0] - rows[slot[j]].umin;

@@ -418,11 +418,8 @@ int make_shift_copies_u8(const dd_plan* p, const ExecArgs& a, uint8_t** W_out, i
     const int64_t wpitch = 4 * wcopy;
     const int64_t nrows = (int64_t)a.nbeams * p->nchans;
     uint8_t* W = nullptr;
-    cudaError_t e = cudaMallocAsync((void**)&W, (size_t)(nrows * wpitch), st);
-    if (e != cudaSuccess) {
-        cudaGetLastError();
-        return fail(DD_ERR_NOMEM, std::string("byte-shifted workspace: ") + cudaGetErrorString(e));
-    }
+    int rc = workspace_alloc((void**)&W, (size_t)(nrows * wpitch), a.stream);
+    if (rc != DD_OK) return rc;
     const int64_t nwords = (rowlen + 3) / 4;
     dim3 grid((unsigned)std::min<int64_t>((nwords + 255) / 256, 64), (unsigned)nrows);
     dd_shift_copies_u8<<<grid, 256, 0, st>>>((const uint8_t*)a.X, W, wcopy, wpitch, p->nchans, rowlen,
