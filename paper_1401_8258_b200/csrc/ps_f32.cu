@@ -65,8 +65,9 @@ constexpr int kDBytes = 1;                // bytes of this descriptor that are i
 constexpr int kDBase = 4;                 // [8]  first staged word of channel k, relative to t0 (multiple of 4)
 constexpr int kDLen = 12;                 // [8]  words to stage (multiple of 4; 0 for a missing channel)
 constexpr int kDTrial = 20;               // [kKB] flat word offset of trial j's first operand in the partial sums
-constexpr int kDChunk = kDTrial + kKB;    // [nchunks][G] byte offset, from the stage's first staged word, of
-                                          //      the operand of lane 0 in channel k (zero pad if missing)
+constexpr int kDChunk = kDTrial + kKB;    // [nchunks][G] uint16 word offset, from the stage's first staged word, of
+                                          //      the operand of lane 0 in channel k (zero pad if missing); 16-bit
+                                          //      entries because a warp-uniform LDS.128 still costs four data cycles
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
@@ -198,13 +199,21 @@ dd_ps_f32_kernel(const PsParams p)
         const uint32_t xa = smem_u32(Xs + st * xstage) + lane * 4;
         float* ps = Ps + buf * p.psw + lane;
         const int nchunks = ds[kDNChunks];
-        const int4* ct = reinterpret_cast<const int4*>(ds + kDChunk);
+        const uint32_t* ct = reinterpret_cast<const uint32_t*>(ds + kDChunk);
         for (int c = warp; c < nchunks; c += kWarps) {
+            uint32_t pk[G / 2];
+            if (G == 4) {
+                const uint2 v = *reinterpret_cast<const uint2*>(ct + c * 2);
+                pk[0] = v.x; pk[1] = v.y;
+            } else {
+                const uint4 v = *reinterpret_cast<const uint4*>(ct + c * 4);
+                pk[0] = v.x; pk[1] = v.y; pk[G / 2 - 2] = v.z; pk[G / 2 - 1] = v.w;
+            }
             int o[G];
 #pragma unroll
-            for (int q = 0; q < G / 4; ++q) {
-                const int4 v = ct[c * (G / 4) + q];
-                o[4 * q] = v.x; o[4 * q + 1] = v.y; o[4 * q + 2] = v.z; o[4 * q + 3] = v.w;
+            for (int q = 0; q < G / 2; ++q) {
+                o[2 * q] = (int)(pk[q] & 0xffffu) * 4;
+                o[2 * q + 1] = (int)(pk[q] >> 16) * 4;
             }
             float lo[G], hi[G];
 #pragma unroll
@@ -297,7 +306,7 @@ namespace {
 struct PsShape { bool fits = false; int64_t psw = 0, xw = 0; int desc_ints = 0; size_t smem = 0; double cost = 0; };
 
 // Shared-memory need and modelled shared-memory wavefronts per output tile for group size G:
-// step 3 costs kKB * kNK per group, step 2 (2 G + 2 + G / 4) per kChunk words of pattern rows.
+// step 3 costs kKB * kNK per group, step 2 (2 G + 2 + G / 2) per kChunk words of pattern rows.
 PsShape shape_for(const HostTable& h, int G)
 {
     PsShape o;
@@ -315,11 +324,11 @@ PsShape shape_for(const HostTable& h, int G)
             o.psw = std::max(o.psw, w);
             chunks += w / kChunk;
         }
-    o.desc_ints = kDChunk + G * (int)(o.psw / kChunk);
+    o.desc_ints = (kDChunk + (G / 2) * (int)(o.psw / kChunk) + 3) / 4 * 4;
     o.smem = (size_t)kXStages * (G * o.xw + kChunk) * 4 + (size_t)2 * o.psw * 4 +
              (size_t)kXStages * o.desc_ints * 4 + (2 * kXStages + 4) * 8;
-    o.fits = o.xw <= 16384 && o.smem <= (size_t)kMaxSmem;
-    o.cost = (double)ntiles * ngroups * kKB * kNK + (double)chunks * (2 * G + 2 + G / 4);
+    o.fits = G * o.xw + kChunk < 65536 && o.smem <= (size_t)kMaxSmem;
+    o.cost = (double)ntiles * ngroups * kKB * kNK + (double)chunks * (2 * G + 2 + G / 2);
     return o;
 }
 
@@ -364,7 +373,7 @@ int build_ps_plan(dd_plan* p)
         destroy_ps_plan(p);
         return fail(DD_ERR_NOMEM, "ps descriptor allocation failed");
     }
-    const int zero_pad = G * t->xw * 4;                   // byte offset of the stage's kChunk zero words
+    const int zero_pad = G * t->xw;                       // word offset of the stage's kChunk zero words
     std::vector<PsRow> rows;
     int slot[kKB];
     std::vector<int> rowbase;
@@ -390,16 +399,16 @@ int build_ps_plan(dd_plan* p)
                 // u = umin + (e - rowbase); channel k supplies x_k[u + r_k], staged at word
                 // (u + r_k - base_k) of its vector
                 for (int c = 0; c < (ulen + kChunk - 1) / kChunk; ++c) {
-                    int32_t* ce = ds + kDChunk + G * (flat / kChunk + c);
+                    uint16_t* ce = reinterpret_cast<uint16_t*>(ds + kDChunk) + G * (flat / kChunk + c);
                     for (int k = 0; k < G; ++k) {
                         const int rk = k == 0 ? 0 : rows[r].key[k - 1];
-                        ce[k] = k < nk ? 4 * (k * t->xw + rows[r].umin + kChunk * c + rk - base[k]) : zero_pad;
+                        ce[k] = (uint16_t)(k < nk ? k * t->xw + rows[r].umin + kChunk * c + rk - base[k] : zero_pad);
                     }
                 }
                 flat += (ulen + kChunk - 1) / kChunk * kChunk;
             }
             ds[kDNChunks] = flat / kChunk;
-            ds[kDBytes] = 4 * (kDChunk + G * (flat / kChunk));
+            ds[kDBytes] = (4 * kDChunk + 2 * G * (flat / kChunk) + 15) / 16 * 16;
             for (int j = 0; j < kKB; ++j) {
                 const int d = std::min(tile * kKB + j, ndm - 1);
                 const int s0 = h.shift[(size_t)d * nch + c0];
