@@ -353,3 +353,109 @@ def test_config2_full_size_sampled_rows_and_checksums():
     # BASELINE.json configs[1] as benchmarked: 1024 ch x 1024 DMs x 2^17 samples, uint8 -> int32
     w, X, D, tab = _full_size(2)
     assert np.array_equal(D[0], X[:, :w.nsamp].sum(axis=0, dtype=np.int64).astype(np.int32))   # DM = 0 row
+
+
+# ------------------------------------------------------------------ configs 3-5 at full size, as bench.py launches them
+
+def _sampled(w, X, d_idx, t_idx, got):
+    if w.dtype == "u8":
+        want = oracle.elements(X, w.fch1, w.foff, w.tsamp, w.dm_list, d_idx, t_idx)
+        assert np.array_equal(got.astype(np.int64), want)
+    else:
+        want, A = oracle.elements(X, w.fch1, w.foff, w.tsamp, w.dm_list, d_idx, t_idx)
+        err = np.abs(got.astype(np.float64) - want)
+        assert np.all(err <= 1e-5 * A), (err / (1e-5 * A)).max()
+
+
+def _sample_points(w, n, seed):
+    g = np.random.default_rng(seed)
+    di = g.integers(0, w.ndm, n)
+    ti = g.integers(0, w.nsamp, n)
+    # corners and the seams of the 64-trial x 512/1024-sample tiles
+    di[:8] = [0, 0, w.ndm - 1, w.ndm - 1, 63, 64, min(w.ndm - 1, 127), min(w.ndm - 1, 128)]
+    ti[:8] = [0, w.nsamp - 1, 0, w.nsamp - 1, 511, 512, 1023, 1024]
+    return di, ti
+
+
+def test_config3_full_size_sampled():
+    # BASELINE.json configs[2] exactly as bench.py times it: 4096 ch x 4096 DMs x 2^18 samples, float32,
+    # one dd_execute on 16-byte aligned input (partial-sum kernel, G = 8)
+    import torch
+    w = synth.WORKLOADS[3]
+    tab = oracle.shift_table(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    ms = int(tab.max())
+    X = synth.make_input(w, w.nsamp + ms)
+    for d, t0, width in synth.pulse_plan(w, 5):
+        synth.inject_pulse(X, t0, width, 0.25, tab[d])
+    stride = (w.nsamp + ms + 63) // 64 * 64
+    plan = dd.Plan(dd.DD_F32, w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    Xd = torch.zeros((w.nchans, stride), dtype=torch.float32, device="cuda")
+    Xd[:, :w.nsamp + ms] = torch.from_numpy(X).cuda()
+    Dd = torch.empty((w.ndm, w.nsamp), dtype=torch.float32, device="cuda")
+    assert plan.kernel_for(Xd, stride, 0, Dd, w.nsamp, 0, w.nsamp, 1) == dd.DD_KERNEL_PS
+    plan.execute(Xd, stride, 0, Dd, w.nsamp, 0, w.nsamp, 1)
+    torch.cuda.synchronize()
+    di, ti = _sample_points(w, 40000, 33)
+    got = Dd[torch.from_numpy(di).cuda(), torch.from_numpy(ti).cuda()].cpu().numpy()
+    _sampled(w, X, di, ti, got)
+    # the injected pulses peak at their trial and start sample (S/N ~ A sqrt(nchans) = 16 per sample)
+    for d, t0, width in synth.pulse_plan(w, 5):
+        row = Dd[d].cpu().numpy()
+        assert abs(int(np.argmax(np.convolve(row, np.ones(width), "valid"))) - t0) <= 1
+    plan.destroy()
+
+
+def test_config4_full_size_sampled_batch():
+    # BASELINE.json configs[3] as bench.py times it: 32 beams x 512 ch x 2048 DMs x 2^16 samples in ONE
+    # dd_execute (grid.z = beam); sampled elements of three beams against the oracle
+    import torch
+    w = synth.WORKLOADS[4]
+    plan = dd.Plan(dd.DD_F32, w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    ms = plan.max_shift()
+    stride = (w.nsamp + ms + 63) // 64 * 64
+    Xd = torch.zeros((w.nbeams, w.nchans, stride), dtype=torch.float32, device="cuda")
+    keep = {}
+    for b in range(w.nbeams):
+        X = synth.make_input(w, w.nsamp + ms, beam=b)
+        Xd[b, :, :w.nsamp + ms] = torch.from_numpy(X).cuda()
+        if b in (0, 13, 31):
+            keep[b] = X
+    Dd = torch.empty((w.nbeams, w.ndm, w.nsamp), dtype=torch.float32, device="cuda")
+    assert plan.kernel_for(Xd, stride, w.nchans * stride, Dd, w.nsamp, w.ndm * w.nsamp, w.nsamp, w.nbeams) == dd.DD_KERNEL_PS
+    plan.execute(Xd, stride, w.nchans * stride, Dd, w.nsamp, w.ndm * w.nsamp, w.nsamp, w.nbeams)
+    torch.cuda.synchronize()
+    for b, X in keep.items():
+        di, ti = _sample_points(w, 30000, 40 + b)
+        got = Dd[b][torch.from_numpy(di).cuda(), torch.from_numpy(ti).cuda()].cpu().numpy()
+        _sampled(w, X, di, ti, got)
+    plan.destroy()
+
+
+def test_config5_full_size_streamed_in_four_pushes():
+    # BASELINE.json configs[4] as bench.py times it: 2048 ch uint8, 10000 DMs, 2^18 samples fed through
+    # dd_stream_push in 4 chunks (the first carries maxshift extra samples); bit-exact sampled elements
+    import torch
+    w = synth.WORKLOADS[5]
+    plan = dd.Plan(dd.DD_U8, w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    ms = plan.max_shift()
+    assert ms == 37599                                               # golden maxshift of config 5
+    X = synth.make_input(w, w.nsamp + ms)
+    Xd = torch.from_numpy(X).cuda()
+    Dd = torch.full((w.ndm, w.nsamp), -7, dtype=torch.int32, device="cuda")
+    chunk = w.nsamp // w.nchunks
+    st = dd.Stream(plan, chunk + ms, 1)
+    pos = emitted = 0
+    for k in range(w.nchunks):
+        n_new = chunk + (ms if k == 0 else 0)
+        n = st.push(Xd[:, pos:], X.shape[1], 0, n_new, Dd[:, emitted:], w.nsamp, 0)
+        assert n == chunk
+        pos += n_new
+        emitted += n
+    torch.cuda.synchronize()
+    assert emitted == w.nsamp
+    di, ti = _sample_points(w, 40000, 55)
+    ti[8:16] = [chunk - 1, chunk, 2 * chunk - 1, 2 * chunk, 3 * chunk - 1, 3 * chunk, chunk + 1, 3 * chunk + 1]
+    got = Dd[torch.from_numpy(di).cuda(), torch.from_numpy(ti).cuda()].cpu().numpy()
+    _sampled(w, X, di, ti, got)
+    assert np.array_equal(Dd[0].cpu().numpy().astype(np.int64), X[:, :w.nsamp].sum(axis=0, dtype=np.int64))   # DM = 0 row
+    st.destroy(); plan.destroy()
