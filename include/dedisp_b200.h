@@ -62,8 +62,8 @@ enum { DD_KERNEL_AUTO    = 0,
        DD_KERNEL_GENERIC = 1,   /* shared-memory channel-vector kernel, any DM list        */
        DD_KERNEL_TMA     = 2,   /* TMA-staged kernel (byte-shifted copies, packed 16-bit lanes);
                                    uint8 plans whose 64-trial tiles spread <= 1024 samples       */
-       DD_KERNEL_PS      = 3 }; /* TMA-staged float32 kernel with partial sums of four adjacent
-                                   channels shared between the trials of a 64-trial tile         */
+       DD_KERNEL_PS      = 3 }; /* TMA-staged kernels (float32 and uint8) with partial sums of 4-8
+                                   adjacent channels shared between the trials of a 64-trial tile */
 
 const char* dd_strerror(int code);   /* static string for an error code */
 const char* dd_last_error(void);     /* thread-local detail of the last failure ("" if none) */
@@ -111,9 +111,9 @@ int     dd_plan_nchans(const dd_plan* plan);
  * with the oracle's independently built table) */
 int     dd_plan_shift_table(const dd_plan* plan, int32_t* host_out);
 int     dd_plan_set_kernel(dd_plan* plan, int kernel);          /* DD_KERNEL_* */
-/* which kernel dd_execute would launch for these arguments: DD_KERNEL_GENERIC, DD_KERNEL_TMA
- * (uint8; needs a 16-byte aligned D and out strides that are multiples of 4) or DD_KERNEL_PS
- * (float32) */
+/* which kernel dd_execute would launch for these arguments: DD_KERNEL_PS (both dtypes, whenever the
+ * plan's delay steps are fine enough for shared partial sums), DD_KERNEL_TMA (uint8; needs a 16-byte
+ * aligned D and out strides that are multiples of 4) or DD_KERNEL_GENERIC */
 int     dd_plan_kernel_for(const dd_plan* plan, const void* X, int64_t in_stride,
                            int64_t in_beam_stride, const void* D, int64_t out_stride,
                            int64_t out_beam_stride, int64_t nsamp_out, int nbeams);

@@ -130,6 +130,7 @@ struct PsU8Params {
     const int32_t* desc;
     const int32_t* order;
     int nchans, ndm, ngroups, desc_ints, xwb, xstage, psw;
+    int vec_ok;                    // D rows are 16-byte aligned: 16-byte read-modify-write, else element by element
     int64_t nsamp, out_stride, out_beam_stride;
 };
 
@@ -256,7 +257,7 @@ dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
                 int4 v = make_int4((int)(first & 0xffffu), (int)(first >> 16), (int)(second & 0xffffu),
                                    (int)(second >> 16));
                 if (d < p.ndm) {
-                    if (t + 3 < p.nsamp) {
+                    if (p.vec_ok && t + 3 < p.nsamp) {
                         int4* q = reinterpret_cast<int4*>(drow + t);
                         if (nflush) {
                             const int4 old = __ldcg(q);
@@ -446,8 +447,6 @@ bool psu8_plan_usable(const dd_plan* p) { return p->psu8 && p->psu8->ok; }
 bool psu8_args_ok(const dd_plan* p, const ExecArgs& a)
 {
     if (!psu8_plan_usable(p)) return false;
-    // 16-byte read-modify-write of D
-    if (((uintptr_t)a.D & 15) || (a.out_stride & 3) || (a.nbeams > 1 && (a.out_beam_stride & 3))) return false;
     if ((a.nsamp_out + kTB - 1) / kTB > 65535 || a.nbeams > 65535) return false;
     if ((int64_t)a.nbeams * p->nchans > 65535) return false;          // grid.y of the front end
     if ((a.nsamp_out + p->host.maxshift + 4096) / 8 >= ((int64_t)1 << 31)) return false;   // tensor coordinates
@@ -510,6 +509,7 @@ int launch_psu8(const dd_plan* p, const ExecArgs& a)
     q.nsamp = a.nsamp_out;
     q.out_stride = a.out_stride;
     q.out_beam_stride = a.out_beam_stride;
+    q.vec_ok = !(((uintptr_t)a.D & 15) || (a.out_stride & 3) || (a.nbeams > 1 && (a.out_beam_stride & 3)));
     dim3 grid((unsigned)t->ntiles, (unsigned)((a.nsamp_out + kTB - 1) / kTB), (unsigned)a.nbeams);
     dd_ps_u8_kernel<<<grid, kThreads + 32, t->smem, st>>>(q, tmap);
     cudaError_t e = cudaGetLastError();

@@ -459,3 +459,21 @@ def test_config5_full_size_streamed_in_four_pushes():
     _sampled(w, X, di, ti, got)
     assert np.array_equal(Dd[0].cpu().numpy().astype(np.int64), X[:, :w.nsamp].sum(axis=0, dtype=np.int64))   # DM = 0 row
     st.destroy(); plan.destroy()
+
+
+def test_uint8_partial_sum_kernel_takes_unaligned_output():
+    # D rows that are not 16-byte aligned (odd row length, offset base): the partial-sum kernel flushes
+    # element by element instead of falling back to the generic kernel; results stay bit-exact
+    import torch
+    w = small(2, 256, 70, 9000 + 37)
+    X, ms = make_case(w, pulses=3)
+    plan = dd.Plan(dd.DD_U8, w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    Xd = torch.from_numpy(X).cuda()
+    buf = torch.full((1 + w.ndm * w.nsamp,), -7, dtype=torch.int32, device="cuda")
+    Dd = buf[1:]
+    assert plan.kernel_for(Xd, X.shape[1], 0, Dd, w.nsamp, 0, w.nsamp, 1) == dd.DD_KERNEL_PS
+    plan.execute(Xd, X.shape[1], 0, Dd, w.nsamp, 0, w.nsamp, 1)
+    torch.cuda.synchronize()
+    assert int(buf[0]) == -7
+    assert_parity(w, X, Dd.view(w.ndm, w.nsamp).cpu().numpy())
+    plan.destroy()
