@@ -374,6 +374,7 @@ int build_ps_plan(dd_plan* p)
         return fail(DD_ERR_NOMEM, "ps descriptor allocation failed");
     }
     const int zero_pad = G * t->xw;                       // word offset of the stage's kChunk zero words
+    bool bounds_ok = true;                                // every shared-memory offset written below is in range
     std::vector<PsRow> rows;
     int slot[kKB];
     std::vector<int> rowbase;
@@ -402,7 +403,10 @@ int build_ps_plan(dd_plan* p)
                     uint16_t* ce = reinterpret_cast<uint16_t*>(ds + kDChunk) + G * (flat / kChunk + c);
                     for (int k = 0; k < G; ++k) {
                         const int rk = k == 0 ? 0 : rows[r].key[k - 1];
-                        ce[k] = (uint16_t)(k < nk ? k * t->xw + rows[r].umin + kChunk * c + rk - base[k] : zero_pad);
+                        const int off = k < nk ? k * t->xw + rows[r].umin + kChunk * c + rk - base[k] : zero_pad;
+                        // every lane's two reads (words off + l and off + l + 32) stay inside the stage
+                        bounds_ok = bounds_ok && off >= 0 && off + kChunk <= G * t->xw + kChunk;
+                        ce[k] = (uint16_t)off;
                     }
                 }
                 flat += (ulen + kChunk - 1) / kChunk * kChunk;
@@ -413,8 +417,10 @@ int build_ps_plan(dd_plan* p)
                 const int d = std::min(tile * kKB + j, ndm - 1);
                 const int s0 = h.shift[(size_t)d * nch + c0];
                 ds[kDTrial + j] = rowbase[slot[j]] + (s0 - rows[slot[j]].umin);
+                bounds_ok = bounds_ok && ds[kDTrial + j] >= 0 && ds[kDTrial + j] + kTB <= t->psw;
             }
         }
+    if (!bounds_ok) return DD_OK;                         // never expected; the plan stays unusable (generic kernel)
     cudaError_t e = cudaMalloc(&t->d_desc, desc.size() * sizeof(int32_t));
     if (e != cudaSuccess) {
         cudaGetLastError();

@@ -375,6 +375,7 @@ int build_psu8_plan(dd_plan* p)
         return fail(DD_ERR_NOMEM, "ps u8 descriptor allocation failed");
     }
     const int zero_pad = kG * 4 * t->xwb;                 // byte offset of the stage's zero words
+    bool bounds_ok = true;                                // every shared-memory offset written below is in range
     std::vector<int> rowbase;
     for (int tile = 0; tile < ntiles; ++tile)
         for (int g = 0; g < ngroups; ++g) {
@@ -400,9 +401,12 @@ int build_psu8_plan(dd_plan* p)
                         const int rk = k == 0 ? 0 : rows[r].key[k - 1];
                         const int a0 = rows[r].umin + 2 * kStepW * c + rk - base;
                         ce[k] = k < nk ? (4 * k + (a0 & 3)) * t->xwb + (a0 & ~3) : zero_pad;
+                        // every lane's read (4 bytes at ce[k] + 4 l) stays inside the stage
+                        bounds_ok = bounds_ok && a0 >= 0 && ce[k] + 128 <= t->xstage;
                     }
                     ce[4] = rowbase[2 * r] + kStepW * c;
                     ce[5] = rowbase[2 * r + 1] + kStepW * c;
+                    bounds_ok = bounds_ok && ce[4] + kChunk <= t->psw && ce[5] + kStepW <= t->psw;
                 }
                 flat += 2 * (kStepW * ns + 2);
             }
@@ -412,8 +416,10 @@ int build_psu8_plan(dd_plan* p)
                 const int d = std::min(tile * kKB + j, ndm - 1);
                 const int o = h.shift[(size_t)d * nch + c0] - rows[slot[j]].umin;
                 ds[kDTrial + j] = rowbase[2 * slot[j] + (o & 1)] + (o >> 1);
+                bounds_ok = bounds_ok && o >= 0 && ds[kDTrial + j] + kTB / 2 <= t->psw;
             }
         }
+    if (!bounds_ok) return DD_OK;                         // never expected; the plan stays unusable (other kernels)
     cudaError_t e = cudaMalloc(&t->d_desc, desc.size() * sizeof(int32_t));
     if (e != cudaSuccess) {
         cudaGetLastError();
