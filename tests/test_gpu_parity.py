@@ -477,3 +477,37 @@ def test_uint8_partial_sum_kernel_takes_unaligned_output():
     assert int(buf[0]) == -7
     assert_parity(w, X, Dd.view(w.ndm, w.nsamp).cpu().numpy())
     plan.destroy()
+
+
+# ------------------------------------------------------------------ seeded random shapes (all kernels through AUTO)
+
+def _random_case(g, dtype):
+    nchans = int(g.choice([1, 2, 3, 5, 8, 13, 31, 64, 100, 257, 300]))
+    ndm = int(g.integers(1, 140))
+    nsamp = int(g.integers(1, 2600))
+    fch1 = float(g.uniform(150.0, 1600.0))
+    band = float(g.uniform(0.01, 0.2)) * fch1                 # 1 % .. 20 % fractional bandwidth
+    tsamp = float(g.choice([51.2e-6, 64e-6, 1e-4, 1e-3]))
+    dm_step = float(g.choice([0.01, 0.05, 0.1, 0.25, 1.0]))
+    return synth.scaled(synth.WORKLOADS[2], dtype=dtype, nchans=nchans, ndm=ndm, nsamp=nsamp, fch1=fch1,
+                        foff=-band / nchans, tsamp=tsamp, dm_step=dm_step, nbeams=1)
+
+
+@pytest.mark.parametrize("dtype", ["f32", "u8"])
+def test_random_shapes_against_the_oracle(dtype):
+    g = np.random.default_rng(20140128 + (dtype == "u8"))
+    kinds = set()
+    done = 0
+    while done < 24:
+        w = _random_case(g, dtype)
+        ms = oracle.max_shift(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+        if ms > 60000 or (w.nsamp + ms) * w.nchans > 3e7:
+            continue                                             # keep the oracle pass in seconds
+        X = synth.make_input(synth.scaled(w, seed=int(g.integers(1, 1 << 30))), w.nsamp + ms)
+        plan = dd.Plan(dd_dtype(w), w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+        kinds.add(plan.kernel_for(0x1000, w.nsamp + ms, 0, 0x2000, w.nsamp, 0, w.nsamp, 1))
+        plan.destroy()
+        D = gpu_dedisperse(w, X, dd.DD_KERNEL_AUTO)
+        assert_parity(w, X, D)
+        done += 1
+    assert dd.DD_KERNEL_PS in kinds and len(kinds) >= 2            # the draw exercises fast and fallback kernels
