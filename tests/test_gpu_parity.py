@@ -355,6 +355,18 @@ def test_config2_full_size_sampled_rows_and_checksums():
     assert np.array_equal(D[0], X[:, :w.nsamp].sum(axis=0, dtype=np.int64).astype(np.int32))   # DM = 0 row
 
 
+def test_config2_full_size_every_element():
+    # the metric's workload, complete: all 1024 x 131072 outputs of the launch bench.py times against a full
+    # pass of the oracle (1.4e11 adds on the host cores), bit for bit
+    w = synth.WORKLOADS[2]
+    ms = oracle.max_shift(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    X = synth.make_input(w, w.nsamp + ms)
+    D = gpu_dedisperse(w, X, dd.DD_KERNEL_AUTO)
+    want = oracle.dedisperse_u8(X, w.nsamp, w.fch1, w.foff, w.tsamp, w.dm_list)
+    assert D.dtype == np.int32 and D.shape == want.shape
+    assert np.array_equal(D, want)
+
+
 # ------------------------------------------------------------------ configs 3-5 at full size, as bench.py launches them
 
 def _sampled(w, X, d_idx, t_idx, got):
