@@ -313,17 +313,25 @@ PsShape shape_for(const HostTable& h, int G)
     const int ntiles = (h.ndm + kKB - 1) / kKB, ngroups = (h.nchans + G - 1) / G;
     const int64_t spread = max_tile_spread(h, kKB);
     o.xw = (kTB + spread + 3 + 3) / 4 * 4 + kChunk;
-    std::vector<PsRow> rows;
-    int slot[kKB];
+    const int workers = ps_workers(ntiles);
+    std::vector<int64_t> wpsw(workers, 0), wchunks(workers, 0);
+    ps_parallel_tiles(ntiles, workers, [&](int tb, int te, int wk) {
+        std::vector<PsRow> rows;
+        int slot[kKB];
+        for (int tile = tb; tile < te; ++tile)
+            for (int g = 0; g < ngroups; ++g) {
+                ps_classify(h, G, kKB, tile, g, rows, slot);
+                int64_t w = 0;
+                for (const PsRow& r : rows) w += ((int64_t)r.umax - r.umin + kTB + kChunk - 1) / kChunk * kChunk;
+                wpsw[wk] = std::max(wpsw[wk], w);
+                wchunks[wk] += w / kChunk;
+            }
+    });
     int64_t chunks = 0;
-    for (int tile = 0; tile < ntiles; ++tile)
-        for (int g = 0; g < ngroups; ++g) {
-            ps_classify(h, G, kKB, tile, g, rows, slot);
-            int64_t w = 0;
-            for (const PsRow& r : rows) w += ((int64_t)r.umax - r.umin + kTB + kChunk - 1) / kChunk * kChunk;
-            o.psw = std::max(o.psw, w);
-            chunks += w / kChunk;
-        }
+    for (int wk = 0; wk < workers; ++wk) {
+        o.psw = std::max(o.psw, wpsw[wk]);
+        chunks += wchunks[wk];
+    }
     o.desc_ints = (kDChunk + (G / 2) * (int)(o.psw / kChunk) + 3) / 4 * 4;
     o.smem = (size_t)kXStages * (G * o.xw + kChunk) * 4 + (size_t)2 * o.psw * 4 +
              (size_t)kXStages * o.desc_ints * 4 + (2 * kXStages + 4) * 8;
@@ -375,10 +383,14 @@ int build_ps_plan(dd_plan* p)
     }
     const int zero_pad = G * t->xw;                       // word offset of the stage's kChunk zero words
     bool bounds_ok = true;                                // every shared-memory offset written below is in range
+    const int workers = ps_workers(ntiles);
+    std::vector<char> wok(workers, 1);
+    ps_parallel_tiles(ntiles, workers, [&](int tb, int te, int wk) {
     std::vector<PsRow> rows;
     int slot[kKB];
     std::vector<int> rowbase;
-    for (int tile = 0; tile < ntiles; ++tile)
+    bool bounds_ok = true;
+    for (int tile = tb; tile < te; ++tile)
         for (int g = 0; g < ngroups; ++g) {
             ps_classify(h, G, kKB, tile, g, rows, slot);
             int32_t* ds = &desc[((size_t)tile * ngroups + g) * desc_ints];
@@ -420,6 +432,9 @@ int build_ps_plan(dd_plan* p)
                 bounds_ok = bounds_ok && ds[kDTrial + j] >= 0 && ds[kDTrial + j] + kTB <= t->psw;
             }
         }
+    wok[wk] = bounds_ok;
+    });
+    for (int wk = 0; wk < workers; ++wk) bounds_ok = bounds_ok && wok[wk];
     if (!bounds_ok) return DD_OK;                         // never expected; the plan stays unusable (generic kernel)
     cudaError_t e = cudaMalloc(&t->d_desc, desc.size() * sizeof(int32_t));
     if (e != cudaSuccess) {
@@ -452,17 +467,17 @@ void destroy_ps_plan(dd_plan* p)
 
 bool ps_plan_usable(const dd_plan* p) { return p->ps && p->ps->ok; }
 
+static bool ps_direct(const ExecArgs& a)
+{
+    return (((uintptr_t)a.X & 15) == 0) && (a.in_stride & 3) == 0 && (a.nbeams == 1 || (a.in_beam_stride & 3) == 0);
+}
+
 bool ps_args_ok(const dd_plan* p, const ExecArgs& a)
 {
     if (!ps_plan_usable(p)) return false;
     if ((a.nsamp_out + kTB - 1) / kTB > 65535 || a.nbeams > 65535) return false;
-    if ((int64_t)a.nbeams * p->nchans > 65535) return false;          // grid.y of the re-pitch copy
+    if (!ps_direct(a) && (int64_t)a.nbeams * p->nchans > 65535) return false;   // grid.y of the re-pitch copy
     return true;
-}
-
-static bool ps_direct(const ExecArgs& a)
-{
-    return (((uintptr_t)a.X & 15) == 0) && (a.in_stride & 3) == 0 && (a.nbeams == 1 || (a.in_beam_stride & 3) == 0);
 }
 
 int ps_launches(const dd_plan* p, const ExecArgs& a) { return ps_direct(a) ? 1 : 2; }

@@ -3,6 +3,7 @@
 #pragma once
 
 #include <algorithm>
+#include <thread>
 #include <vector>
 
 #include "dd_internal.h"
@@ -47,6 +48,29 @@ inline void ps_classify(const HostTable& h, int G, int kb, int tile, int g, std:
         rows[r].umax = std::max(rows[r].umax, s[0]);
         slot[j] = r;
     }
+}
+
+// Runs fn(tile_begin, tile_end, worker) over [0, ntiles) on up to 16 host threads (the descriptor
+// passes are independent per trial tile; config 3 has 64 tiles x 512 groups x 64 trials).
+inline int ps_workers(int ntiles)
+{
+    const unsigned hw = std::thread::hardware_concurrency();
+    return std::max(1, std::min({ntiles, (int)(hw ? hw : 1), 16}));
+}
+template <typename F>
+inline void ps_parallel_tiles(int ntiles, int workers, F fn)
+{
+    if (workers <= 1) {
+        fn(0, ntiles, 0);
+        return;
+    }
+    std::vector<std::thread> th;
+    const int per = (ntiles + workers - 1) / workers;
+    for (int w = 0; w < workers; ++w) {
+        const int b = std::min(ntiles, w * per), e = std::min(ntiles, b + per);
+        th.emplace_back([=] { fn(b, e, w); });
+    }
+    for (auto& t : th) t.join();
 }
 
 }  // namespace dd

@@ -337,20 +337,28 @@ int build_psu8_plan(dd_plan* p)
     // the kTB / 2 words every trial reads, in whole warp steps
     // warp steps of a pattern row: step c writes even-u words [62 c, 62 c + 64) and odd-u words [62 c, 62 c + 62)
     auto row_steps = [](const PsRow& r) { return ((r.umax - r.umin) / 2 + kTB / 2 + kStepW - 1) / kStepW; };
-    std::vector<PsRow> rows;
-    int slot[kKB];
-    int64_t psw = 0, max_steps = 0;
-    for (int tile = 0; tile < ntiles; ++tile)
-        for (int g = 0; g < ngroups; ++g) {
-            ps_classify(h, kG, kKB, tile, g, rows, slot);
-            int64_t w = 0, n = 0;
-            for (const PsRow& r : rows) {
-                n += row_steps(r);
-                w += 2 * (kStepW * row_steps(r) + 2);
+    const int workers = ps_workers(ntiles);
+    std::vector<int64_t> wpsw(workers, 0), wsteps(workers, 0);
+    ps_parallel_tiles(ntiles, workers, [&](int tb, int te, int wk) {
+        std::vector<PsRow> rows;
+        int slot[kKB];
+        for (int tile = tb; tile < te; ++tile)
+            for (int g = 0; g < ngroups; ++g) {
+                ps_classify(h, kG, kKB, tile, g, rows, slot);
+                int64_t w = 0, n = 0;
+                for (const PsRow& r : rows) {
+                    n += row_steps(r);
+                    w += 2 * (kStepW * row_steps(r) + 2);
+                }
+                wpsw[wk] = std::max(wpsw[wk], w);
+                wsteps[wk] = std::max(wsteps[wk], n);
             }
-            psw = std::max(psw, w);
-            max_steps = std::max(max_steps, n);
-        }
+    });
+    int64_t psw = 0, max_steps = 0;
+    for (int wk = 0; wk < workers; ++wk) {
+        psw = std::max(psw, wpsw[wk]);
+        max_steps = std::max(max_steps, wsteps[wk]);
+    }
     const int desc_ints = kDChunk + kCE * (int)max_steps;
     const size_t smem = (size_t)kXStages * xstage + (size_t)2 * psw * 4 +
                         (size_t)kXStages * desc_ints * 4 + 2 * kXStages * 8;
@@ -376,8 +384,13 @@ int build_psu8_plan(dd_plan* p)
     }
     const int zero_pad = kG * 4 * t->xwb;                 // byte offset of the stage's zero words
     bool bounds_ok = true;                                // every shared-memory offset written below is in range
+    std::vector<char> wok(workers, 1);
+    ps_parallel_tiles(ntiles, workers, [&](int tb, int te, int wk) {
+    std::vector<PsRow> rows;
+    int slot[kKB];
     std::vector<int> rowbase;
-    for (int tile = 0; tile < ntiles; ++tile)
+    bool bounds_ok = true;
+    for (int tile = tb; tile < te; ++tile)
         for (int g = 0; g < ngroups; ++g) {
             ps_classify(h, kG, kKB, tile, g, rows, slot);
             int32_t* ds = &desc[((size_t)tile * ngroups + g) * desc_ints];
@@ -419,6 +432,9 @@ int build_psu8_plan(dd_plan* p)
                 bounds_ok = bounds_ok && o >= 0 && ds[kDTrial + j] + kTB / 2 <= t->psw;
             }
         }
+    wok[wk] = bounds_ok;
+    });
+    for (int wk = 0; wk < workers; ++wk) bounds_ok = bounds_ok && wok[wk];
     if (!bounds_ok) return DD_OK;                         // never expected; the plan stays unusable (other kernels)
     cudaError_t e = cudaMalloc(&t->d_desc, desc.size() * sizeof(int32_t));
     if (e != cudaSuccess) {
