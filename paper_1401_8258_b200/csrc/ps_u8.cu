@@ -282,30 +282,36 @@ dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
     consumer_barrier();
 
     // st: stage of group g; sn / phn: stage and phase parity of group g + 1
-    int st = 0, sn = 1 % kXStages, phn = kXStages == 1 ? 1 : 0, flush_in = kFlushGroups;
-    for (int g = 0; g < ng; ++g) {
-        if (g + 1 < ng) {
-            mbar_wait(&full[sn], phn);
-            pre(sn, (g + 1) & 1);
-        }
-        // Step 3: one word per trial, sample pair and group
-        const int4 tr = *reinterpret_cast<const int4*>(Ds + st * p.desc_ints + kDTrial + warp * kKW);
-        const int tro[kKW] = {tr.x, tr.y, tr.z, tr.w};
-        const uint32_t* ps = Ps + (g & 1) * p.psw + lane;
+    int st = 0, sn = 1 % kXStages, phn = kXStages == 1 ? 1 : 0;
+    // blocks of kFlushGroups groups, one flush after each (a single flush site keeps its tail-tile
+    // predicates out of the inner loop)
+#pragma unroll 1
+    for (int g0 = 0; g0 < ng; g0 += kFlushGroups) {
+        const int g1 = min(ng, g0 + kFlushGroups);
+#pragma unroll 1
+        for (int g = g0; g < g1; ++g) {
+            if (g + 1 < ng) {
+                mbar_wait(&full[sn], phn);
+                pre(sn, (g + 1) & 1);
+            }
+            // Step 3: one word per trial, sample pair and group
+            const int4 tr = *reinterpret_cast<const int4*>(Ds + st * p.desc_ints + kDTrial + warp * kKW);
+            const int tro[kKW] = {tr.x, tr.y, tr.z, tr.w};
+            const uint32_t* ps = Ps + (g & 1) * p.psw + lane;
 #pragma unroll
-        for (int j = 0; j < kKW; ++j) {
-            const uint32_t* r = ps + tro[j];
+            for (int j = 0; j < kKW; ++j) {
+                const uint32_t* r = ps + tro[j];
 #pragma unroll
-            for (int i = 0; i < kNK; ++i) acc[j][i] += r[32 * i];
+                for (int i = 0; i < kNK; ++i) acc[j][i] += r[32 * i];
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[st]);      // stage st (vectors and descriptor) may be refilled
+            consumer_barrier();                          // partial sums of g+1 complete, those of g consumed
+            st = sn;
+            if (++sn == kXStages) { sn = 0; phn ^= 1; }
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[st]);          // stage st (vectors and descriptor) may be refilled
-        consumer_barrier();                              // partial sums of g+1 complete, those of g consumed
-        st = sn;
-        if (++sn == kXStages) { sn = 0; phn ^= 1; }
-        if (--flush_in == 0 && g + 1 < ng) { flush(); flush_in = kFlushGroups; }
+        flush();
     }
-    flush();
 }
 
 }  // namespace
