@@ -1,6 +1,6 @@
 // Generic "channel vector" kernel: works for ANY plan (unsorted / non-uniform DM lists, large
 // per-trial shift steps, unaligned pointers and strides).  It is the correctness anchor and the
-// fallback for shapes the register-window kernel (window.cu) does not take.
+// fallback for plans the partial-sum kernels (ps_f32.cu, ps_u8.cu) and tma_u8.cu do not take.
 //
 // Structure (the thesis' Alg. 1, modernised): the grid maps onto the output
 // plane (DM, t); a block owns KB consecutive (sorted) trials x TB = 1024 output
