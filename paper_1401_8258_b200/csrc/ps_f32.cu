@@ -4,7 +4,7 @@
 // nchans operands.  How: a float32 word holds one sample, so the thesis' loop (Alg. 1,
 // one shared-memory read per add) is capped at 32 adds/clk/SM, a quarter of
 // the FP32 add rate.  Here the channels are taken in groups of G = 4 or 8 (chosen per plan by a
-// cost model; the text below writes G = 4).  Within a tile of kKB
+// cost model; the text below writes G = 4).  Within a tile of KB = 64 or 128
 // adjacent (sorted) trials the relative delays of a group,
 //     r_k(d) = s(d, c0+k) - s(d, c0),  k = 1..3,
 // take only a few distinct values ("patterns": 3-7 per tile on the BASELINE.json workloads,
@@ -15,14 +15,14 @@
 //   2. forms one row per pattern,  P[u] = ((x0[u] + x1[u+r1]) + x2[u+r2]) + x3[u+r3],  in shared
 //      memory (all warps, 64 consecutive u per warp step);
 //   3. adds, for every trial d and sample t of the tile, ONE word:  acc += P_{pattern(d)}[t + s(d,c0)].
-// Step 3 costs one shared-memory word per FOUR channel-adds; step 2 adds about (patterns / kKB)
+// Step 3 costs one shared-memory word per FOUR channel-adds; step 2 adds about (patterns / KB)
 // * 5/4 words per channel-add.  Descriptors (windows, patterns, per-trial row offsets) are built on
 // the host at plan time from the exact delay table; nothing is approximated, and the order of
 // the additions depends only on the plan (groups in ascending channel order, inside a group the
 // expression above), never on the tile, so batch / streaming / one-shot results are identical.
 //
-// Layout of a block: 16 warps; warp w owns trials w*kKW .. w*kKW+kKW-1 of the tile, lane l owns
-// the output samples t0 + l + 32 i, i < kNK (accumulators acc[kKW][kNK] in registers,
+// Layout of a block: 16 warps; warp w owns trials w*KW .. w*KW+KW-1 of the tile, lane l owns
+// the output samples t0 + l + 32 i, i < NK (accumulators acc[KW][NK] in registers, KW * NK = 64,
 // PAPER.md:958).  D is written once with 128-byte coalesced warp stores.
 #include <cuda_runtime.h>
 
@@ -37,6 +37,7 @@ struct dd_ps_plan {
     bool ok = false;
     int ntiles = 0, ngroups = 0;
     int G = 4;                     // channels per group
+    int kw = 4;                    // trials per warp (block = 16 kw trials x 32 * 64 / kw samples)
     int desc_ints = 0;             // ints per (tile, group) descriptor (multiple of 4)
     int xw = 0;                    // words per staged channel vector
     int psw = 0;                   // words of one partial-sum buffer
@@ -51,10 +52,10 @@ namespace {
 constexpr int kGMax = kPsGMax;            // channels per group: 4 or 8
 constexpr int kWarps = 16;
 constexpr int kThreads = 32 * kWarps;
-constexpr int kKW = 4;                    // trials per warp
-constexpr int kKB = kKW * kWarps;         // trials per block
-constexpr int kNK = 16;                   // output samples per lane
-constexpr int kTB = 32 * kNK;             // output samples per block
+// tile shapes: KW trials per warp x NK = 64 / KW samples per lane (64 accumulators per thread), i.e.
+// 64 trials x 512 samples or 128 trials x 256 samples per block; chosen per plan by the cost model
+constexpr int kAccPerLane = 64;
+constexpr int kKBMax = 8 * kWarps;
 constexpr int kXStages = 3;
 constexpr int kMaxSmem = 200 * 1024;
 
@@ -64,8 +65,8 @@ constexpr int kDNChunks = 0;              // kChunk-word steps of the partial-su
 constexpr int kDBytes = 1;                // bytes of this descriptor that are in use (multiple of 16)
 constexpr int kDBase = 4;                 // [8]  first staged word of channel k, relative to t0 (multiple of 4)
 constexpr int kDLen = 12;                 // [8]  words to stage (multiple of 4; 0 for a missing channel)
-constexpr int kDTrial = 20;               // [kKB] flat word offset of trial j's first operand in the partial sums
-constexpr int kDChunk = kDTrial + kKB;    // [nchunks][G] uint16 word offset, from the stage's first staged word, of
+constexpr int kDTrial = 20;               // [KB] flat word offset of trial j's first operand in the partial sums
+// kDTrial + KB:                             [nchunks][G] uint16 word offset, from the stage's first staged word, of
                                           //      the operand of lane 0 in channel k (zero pad if missing); 16-bit
                                           //      entries because a warp-uniform LDS.128 still costs four data cycles
 
@@ -122,10 +123,11 @@ struct PsParams {
     int64_t in_stride, in_beam_stride, out_stride, out_beam_stride;
 };
 
-template <int G>
+template <int G, int KW>
 __global__ void __launch_bounds__(kThreads + 32, 1)
 dd_ps_f32_kernel(const PsParams p)
 {
+    constexpr int NK = kAccPerLane / KW, KB = KW * kWarps, TB = 32 * NK, kDChunk = kDTrial + KB;
     extern __shared__ __align__(128) uint8_t smem_raw[];
     const int xstage = G * p.xw + kChunk;                                      // words; the last kChunk stay zero
     float* Xs = reinterpret_cast<float*>(smem_raw);                            // [kXStages][xstage]
@@ -138,7 +140,7 @@ dd_ps_f32_kernel(const PsParams p)
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int tile = blockIdx.x;                          // trial tiles fastest: neighbours share L2 lines
-    const int64_t t0 = (int64_t)blockIdx.y * kTB;
+    const int64_t t0 = (int64_t)blockIdx.y * TB;
     const int beam = blockIdx.z;
     const int ng = p.ngroups;
 
@@ -229,11 +231,11 @@ dd_ps_f32_kernel(const PsParams p)
         }
     };
 
-    float acc[kKW][kNK];
+    float acc[KW][NK];
 #pragma unroll
-    for (int j = 0; j < kKW; ++j)
+    for (int j = 0; j < KW; ++j)
 #pragma unroll
-        for (int i = 0; i < kNK; ++i) acc[j][i] = 0.0f;
+        for (int i = 0; i < NK; ++i) acc[j][i] = 0.0f;
 
     // Warps synchronise through split-phase barriers instead of a block barrier: ready[b] completes
     // when all 16 warps have written their part of partial-sum buffer b, freeb[b] when all have
@@ -254,15 +256,19 @@ dd_ps_f32_kernel(const PsParams p)
             if (lane == 0) mbar_arrive(&ready[b ^ 1]);
         }
         // Step 3: one word per trial, sample and group
-        const int4 tr = *reinterpret_cast<const int4*>(Ds + st * p.desc_ints + kDTrial + warp * kKW);
-        const int tro[kKW] = {tr.x, tr.y, tr.z, tr.w};
+        int tro[KW];
+#pragma unroll
+        for (int q = 0; q < KW / 4; ++q) {
+            const int4 tr = *reinterpret_cast<const int4*>(Ds + st * p.desc_ints + kDTrial + warp * KW + 4 * q);
+            tro[4 * q] = tr.x; tro[4 * q + 1] = tr.y; tro[4 * q + 2] = tr.z; tro[4 * q + 3] = tr.w;
+        }
         const float* ps = Ps + b * p.psw + lane;
         mbar_wait(&ready[b], (g >> 1) & 1);                                // step 2 of g is done everywhere
 #pragma unroll
-        for (int j = 0; j < kKW; ++j) {
+        for (int j = 0; j < KW; ++j) {
             const float* r = ps + tro[j];
 #pragma unroll
-            for (int i = 0; i < kNK; ++i) acc[j][i] += r[32 * i];
+            for (int i = 0; i < NK; ++i) acc[j][i] += r[32 * i];
         }
         __syncwarp();
         if (lane == 0) {
@@ -275,12 +281,12 @@ dd_ps_f32_kernel(const PsParams p)
 
     float* Db = p.D + (int64_t)beam * p.out_beam_stride;
 #pragma unroll
-    for (int j = 0; j < kKW; ++j) {
-        const int d = tile * kKB + warp * kKW + j;
+    for (int j = 0; j < KW; ++j) {
+        const int d = tile * KB + warp * KW + j;
         if (d < p.ndm) {
             float* drow = Db + (int64_t)__ldg(p.order + d) * p.out_stride + t0 + lane;
 #pragma unroll
-            for (int i = 0; i < kNK; ++i)
+            for (int i = 0; i < NK; ++i)
                 if (t0 + lane + 32 * i < p.nsamp) drow[32 * i] = acc[j][i];
         }
     }
@@ -303,13 +309,21 @@ dd_repitch_f32(const float* __restrict__ X, float* __restrict__ W, int nchans, i
 
 namespace {
 
+typedef void (*PsKernel)(const PsParams);
+PsKernel ps_kernel_for(int G, int kw)
+{
+    if (kw == 8) return G == 8 ? dd_ps_f32_kernel<8, 8> : dd_ps_f32_kernel<4, 8>;
+    return G == 8 ? dd_ps_f32_kernel<8, 4> : dd_ps_f32_kernel<4, 4>;
+}
+
 struct PsShape { bool fits = false; int64_t psw = 0, xw = 0; int desc_ints = 0; size_t smem = 0; double cost = 0; };
 
 // Shared-memory need and modelled shared-memory wavefronts per output tile for group size G:
-// step 3 costs kKB * kNK per group, step 2 (2 G + 2 + G / 2) per kChunk words of pattern rows.
-PsShape shape_for(const HostTable& h, int G)
+// step 3 costs KB * NK per group, step 2 (2 G + 2 + G / 2) per kChunk words of pattern rows.
+PsShape shape_for(const HostTable& h, int G, int kw)
 {
     PsShape o;
+    const int kKB = kw * kWarps, kNK = kAccPerLane / kw, kTB = 32 * kNK, kDChunk = kDTrial + kKB;
     const int ntiles = (h.ndm + kKB - 1) / kKB, ngroups = (h.nchans + G - 1) / G;
     const int64_t spread = max_tile_spread(h, kKB);
     o.xw = (kTB + spread + 3 + 3) / 4 * 4 + kChunk;
@@ -317,7 +331,7 @@ PsShape shape_for(const HostTable& h, int G)
     std::vector<int64_t> wpsw(workers, 0), wchunks(workers, 0);
     ps_parallel_tiles(ntiles, workers, [&](int tb, int te, int wk) {
         std::vector<PsRow> rows;
-        int slot[kKB];
+        int slot[kKBMax];
         for (int tile = tb; tile < te; ++tile)
             for (int g = 0; g < ngroups; ++g) {
                 ps_classify(h, G, kKB, tile, g, rows, slot);
@@ -349,17 +363,22 @@ int build_ps_plan(dd_plan* p)
     const HostTable& h = p->host;
     const int nch = p->nchans, ndm = p->ndm;
     // group size: the cheaper of 8 and 4 by the wavefront model, among those that fit
-    int G = 0;
+    int G = 0, kw = 0;
     PsShape sh;
-    for (int cand : {8, 4}) {
-        if (cand == 8 && nch < 16) continue;
-        PsShape c = shape_for(h, cand);
-        if (c.fits && (G == 0 || c.cost < sh.cost)) {
-            G = cand;
-            sh = c;
+    for (int ckw : {4, 8})
+        for (int cand : {8, 4}) {
+            if (cand == 8 && nch < 16) continue;
+            if (ckw == 8 && ndm <= 64) continue;              // a 128-trial tile would be half empty
+            PsShape c = shape_for(h, cand, ckw);
+            if (c.fits && (G == 0 || c.cost < sh.cost)) {
+                G = cand;
+                kw = ckw;
+                sh = c;
+            }
         }
-    }
     if (G == 0) return DD_OK;        // per-trial delay steps too large / too many patterns: generic kernel
+    const int kKB = kw * kWarps, kNK = kAccPerLane / kw, kTB = 32 * kNK, kDChunk = kDTrial + kKB;
+    (void)kNK;
     const int ntiles = (ndm + kKB - 1) / kKB, ngroups = (nch + G - 1) / G;
     const int desc_ints = sh.desc_ints;
 
@@ -367,6 +386,7 @@ int build_ps_plan(dd_plan* p)
     if (!t) return fail(DD_ERR_NOMEM, "ps plan allocation failed");
     p->ps = t;
     t->G = G;
+    t->kw = kw;
     t->ntiles = ntiles;
     t->ngroups = ngroups;
     t->desc_ints = desc_ints;
@@ -387,7 +407,7 @@ int build_ps_plan(dd_plan* p)
     std::vector<char> wok(workers, 1);
     ps_parallel_tiles(ntiles, workers, [&](int tb, int te, int wk) {
     std::vector<PsRow> rows;
-    int slot[kKB];
+    int slot[kKBMax];
     std::vector<int> rowbase;
     bool bounds_ok = true;
     for (int tile = tb; tile < te; ++tile)
@@ -447,8 +467,7 @@ int build_ps_plan(dd_plan* p)
         destroy_ps_plan(p);
         return fail(DD_ERR_CUDA, std::string("ps descriptor upload: ") + cudaGetErrorString(e));
     }
-    e = G == 8 ? cudaFuncSetAttribute(dd_ps_f32_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->smem)
-               : cudaFuncSetAttribute(dd_ps_f32_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->smem);
+    e = cudaFuncSetAttribute(ps_kernel_for(G, kw), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->smem);
     if (e != cudaSuccess) {
         cudaGetLastError();
         return DD_OK;                                     // stays unusable; generic kernel serves
@@ -475,6 +494,7 @@ static bool ps_direct(const ExecArgs& a)
 bool ps_args_ok(const dd_plan* p, const ExecArgs& a)
 {
     if (!ps_plan_usable(p)) return false;
+    const int kTB = 32 * kAccPerLane / p->ps->kw;
     if ((a.nsamp_out + kTB - 1) / kTB > 65535 || a.nbeams > 65535) return false;
     if (!ps_direct(a) && (int64_t)a.nbeams * p->nchans > 65535) return false;   // grid.y of the re-pitch copy
     return true;
@@ -517,9 +537,9 @@ int launch_ps(const dd_plan* p, const ExecArgs& a)
     q.nsamp = a.nsamp_out;
     q.out_stride = a.out_stride;
     q.out_beam_stride = a.out_beam_stride;
+    const int kTB = 32 * kAccPerLane / t->kw;
     dim3 grid((unsigned)t->ntiles, (unsigned)((a.nsamp_out + kTB - 1) / kTB), (unsigned)a.nbeams);
-    if (t->G == 8) dd_ps_f32_kernel<8><<<grid, kThreads + 32, t->smem, st>>>(q);
-    else dd_ps_f32_kernel<4><<<grid, kThreads + 32, t->smem, st>>>(q);
+    ps_kernel_for(t->G, t->kw)<<<grid, kThreads + 32, t->smem, st>>>(q);
     cudaError_t e = cudaGetLastError();
     if (W) cudaFreeAsync(W, st);
     if (e != cudaSuccess) return fail(DD_ERR_CUDA, std::string("ps f32 launch: ") + cudaGetErrorString(e));
