@@ -1,7 +1,7 @@
 // uint8 -> int32 kernel with shared partial sums (SURVEY.md §8 rows a2-a6 for the uint8 path).
 //
 // Same idea as ps_f32.cu, same result as eq 2.1, exact integer arithmetic:
-// channels are taken in groups of G = 4; within a tile of kKB adjacent (sorted) trials the relative
+// channels are taken in groups of G = 4; within a tile of KB = 128 (or 64) adjacent (sorted) trials the relative
 // delays r_k(d) = s(d,c0+k) - s(d,c0) take a handful of distinct values ("patterns"), so a block
 //   1. has the channel vectors of the group in shared memory (eq 2.14): for every
 //      channel the 16-byte aligned window of each of the four byte-shifted copies W_r[i] = X[i+r]
@@ -21,7 +21,7 @@
 // read-modify-write that stays in L2 (plain store the first time).
 //
 // Layout of a block: 16 consumer warps + 1 producer warp; consumer warp w owns trials
-// w*kKW .. w*kKW+kKW-1, lane l owns output samples t0 + 2 (l + 32 i) + {0,1}, i < kNK.
+// w*KW .. w*KW+KW-1, lane l owns output samples t0 + 2 (l + 32 i) + {0,1}, i < NK = 64 / KW.
 #include <cuda.h>
 #include <cuda_runtime.h>
 
@@ -39,6 +39,7 @@ struct dd_psu8_plan {
     int xwb = 0;                   // bytes staged per row (one byte-shifted copy of one channel; multiple of 16)
     int xstage = 0;                // bytes of one stage: 16 rows, 256 zero bytes, over-read slack
     int psw = 0;                   // words of one partial-sum buffer
+    int kw = 8;                    // trials per warp (block = 16 kw trials x 64 * 64 / kw samples)
     size_t smem = 0;
     int32_t* d_desc = nullptr;     // device [ntiles][ngroups][desc_ints]
 };
@@ -50,10 +51,10 @@ namespace {
 constexpr int kG = 4;                     // channels per group
 constexpr int kWarps = 16;
 constexpr int kThreads = 32 * kWarps;
-constexpr int kKW = 4;                    // trials per warp
-constexpr int kKB = kKW * kWarps;         // trials per block
-constexpr int kNK = 16;                   // output sample PAIRS per lane
-constexpr int kTB = 2 * 32 * kNK;         // output samples per block
+// tile shapes: KW trials per warp x NK = 64 / KW sample PAIRS per lane (64 packed accumulators per
+// thread): 128 trials x 512 samples per block, or 64 x 1024 for plans of at most 64 trials
+constexpr int kAccPerLane = 64;
+constexpr int kKBMax = 8 * kWarps;
 constexpr int kXStages = 3;
 constexpr int kMaxSmem = 200 * 1024;
 constexpr int kFlushGroups = 64;          // 64 groups * 4 channels * 255 = 65280 < 65536
@@ -65,8 +66,8 @@ constexpr int kCE = 8;                    // ints per step entry of the descript
 constexpr int kDNChunks = 0;
 constexpr int kDBytes = 1;                // bytes of this descriptor that are in use (multiple of 16)
 constexpr int kDBase = 4;                 // first staged sample of the group's rows, relative to t0 (multiple of 16)
-constexpr int kDTrial = 12;               // [kKB] word offset of trial j's first operand in the partial sums
-constexpr int kDChunk = kDTrial + kKB;    // [nchunks][kCE]: [0..3] byte offset, from the stage's first byte, of the
+constexpr int kDTrial = 12;               // [KB] word offset of trial j's first operand in the partial sums
+// kDTrial + KB:                             [nchunks][kCE]: [0..3] byte offset, from the stage's first byte, of the
                                           //      aligned word lane 0 reads in channel k (zero pad if missing);
                                           //      [4], [5] first even-u / odd-u word the step writes (even numbers)
 
@@ -134,9 +135,11 @@ struct PsU8Params {
     int64_t nsamp, out_stride, out_beam_stride;
 };
 
+template <int KW>
 __global__ void __launch_bounds__(kThreads + 32, 1)
 dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
 {
+    constexpr int NK = kAccPerLane / KW, KB = KW * kWarps, TB = 2 * 32 * NK, kDChunk = kDTrial + KB;
     extern __shared__ __align__(128) uint8_t smem_raw[];
     const int xstage = p.xstage;                                               // bytes: 16 rows of xwb, 256 zero bytes, slack
     uint8_t* Xs = smem_raw;                                                    // [kXStages][xstage]
@@ -148,7 +151,7 @@ dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t xs0 = smem_u32(Xs);
     const int tile = blockIdx.x;                          // trial tiles fastest: neighbours share L2 lines
-    const int64_t t0 = (int64_t)blockIdx.y * kTB;
+    const int64_t t0 = (int64_t)blockIdx.y * TB;
     const int beam = blockIdx.z;
     const int ng = p.ngroups;
 
@@ -231,22 +234,22 @@ dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
         if (c < nchunks) pre_store(ps, ct[2 * c + 1], pre_load(xa, ct[2 * c]));
     };
 
-    uint32_t acc[kKW][kNK];
+    uint32_t acc[KW][NK];
 #pragma unroll
-    for (int j = 0; j < kKW; ++j)
+    for (int j = 0; j < KW; ++j)
 #pragma unroll
-        for (int i = 0; i < kNK; ++i) acc[j][i] = 0u;
+        for (int i = 0; i < NK; ++i) acc[j][i] = 0u;
 
     int32_t* Db = p.D + (int64_t)beam * p.out_beam_stride;
     int nflush = 0;
     // lanes 2m, 2m+1 exchange halves so that every lane writes four consecutive samples
     auto flush = [&]() {
 #pragma unroll
-        for (int j = 0; j < kKW; ++j) {
-            const int d = tile * kKB + warp * kKW + j;
+        for (int j = 0; j < KW; ++j) {
+            const int d = tile * KB + warp * KW + j;
             int32_t* drow = Db + (int64_t)(d < p.ndm ? __ldg(p.order + d) : 0) * p.out_stride;
 #pragma unroll
-            for (int i = 0; i < kNK; i += 2) {
+            for (int i = 0; i < NK; i += 2) {
                 // this lane holds samples 2l+64i+{0,1} (acc[j][i]) and 2l+64(i+1)+{0,1} (acc[j][i+1]);
                 // even lanes take both pairs of block i, odd lanes both pairs of block i+1
                 const uint32_t mine = (lane & 1) ? acc[j][i + 1] : acc[j][i];
@@ -295,14 +298,18 @@ dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
                 pre(sn, (g + 1) & 1);
             }
             // Step 3: one word per trial, sample pair and group
-            const int4 tr = *reinterpret_cast<const int4*>(Ds + st * p.desc_ints + kDTrial + warp * kKW);
-            const int tro[kKW] = {tr.x, tr.y, tr.z, tr.w};
+            int tro[KW];
+#pragma unroll
+            for (int q = 0; q < KW / 4; ++q) {
+                const int4 tr = *reinterpret_cast<const int4*>(Ds + st * p.desc_ints + kDTrial + warp * KW + 4 * q);
+                tro[4 * q] = tr.x; tro[4 * q + 1] = tr.y; tro[4 * q + 2] = tr.z; tro[4 * q + 3] = tr.w;
+            }
             const uint32_t* ps = Ps + (g & 1) * p.psw + lane;
 #pragma unroll
-            for (int j = 0; j < kKW; ++j) {
+            for (int j = 0; j < KW; ++j) {
                 const uint32_t* r = ps + tro[j];
 #pragma unroll
-                for (int i = 0; i < kNK; ++i) acc[j][i] += r[32 * i];
+                for (int i = 0; i < NK; ++i) acc[j][i] += r[32 * i];
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[st]);      // stage st (vectors and descriptor) may be refilled
@@ -316,10 +323,13 @@ dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
 
 }  // namespace
 
-int build_psu8_plan(dd_plan* p)
+typedef void (*PsU8Kernel)(const PsU8Params, const CUtensorMap);
+static PsU8Kernel psu8_kernel_for(int kw) { return kw == 8 ? dd_ps_u8_kernel<8> : dd_ps_u8_kernel<4>; }
+
+// Descriptors for tiles of 16 kw trials; leaves p->psu8 null or not ok when the shape does not fit.
+static int try_build_psu8(dd_plan* p, int kw)
 {
-    p->psu8 = nullptr;
-    if (p->ndm == 0 || p->dtype != DD_U8) return DD_OK;
+    const int kKB = kw * kWarps, kNK = kAccPerLane / kw, kTB = 2 * 32 * kNK, kDChunk = kDTrial + kKB;
     const HostTable& h = p->host;
     const int nch = p->nchans, ndm = p->ndm;
     const int ntiles = (ndm + kKB - 1) / kKB, ngroups = (nch + kG - 1) / kG;
@@ -342,12 +352,12 @@ int build_psu8_plan(dd_plan* p)
     // words of one parity copy of a pattern row: the largest offset of a trial in it, halved, plus
     // the kTB / 2 words every trial reads, in whole warp steps
     // warp steps of a pattern row: step c writes even-u words [62 c, 62 c + 64) and odd-u words [62 c, 62 c + 62)
-    auto row_steps = [](const PsRow& r) { return ((r.umax - r.umin) / 2 + kTB / 2 + kStepW - 1) / kStepW; };
+    auto row_steps = [kTB](const PsRow& r) { return ((r.umax - r.umin) / 2 + kTB / 2 + kStepW - 1) / kStepW; };
     const int workers = ps_workers(ntiles);
     std::vector<int64_t> wpsw(workers, 0), wsteps(workers, 0);
     ps_parallel_tiles(ntiles, workers, [&](int tb, int te, int wk) {
         std::vector<PsRow> rows;
-        int slot[kKB];
+        int slot[kKBMax];
         for (int tile = tb; tile < te; ++tile)
             for (int g = 0; g < ngroups; ++g) {
                 ps_classify(h, kG, kKB, tile, g, rows, slot);
@@ -373,6 +383,7 @@ int build_psu8_plan(dd_plan* p)
     dd_psu8_plan* t = new (std::nothrow) dd_psu8_plan;
     if (!t) return fail(DD_ERR_NOMEM, "ps u8 plan allocation failed");
     p->psu8 = t;
+    t->kw = kw;
     t->ntiles = ntiles;
     t->ngroups = ngroups;
     t->desc_ints = desc_ints;
@@ -393,7 +404,7 @@ int build_psu8_plan(dd_plan* p)
     std::vector<char> wok(workers, 1);
     ps_parallel_tiles(ntiles, workers, [&](int tb, int te, int wk) {
     std::vector<PsRow> rows;
-    int slot[kKB];
+    int slot[kKBMax];
     std::vector<int> rowbase;
     bool bounds_ok = true;
     for (int tile = tb; tile < te; ++tile)
@@ -453,12 +464,28 @@ int build_psu8_plan(dd_plan* p)
         destroy_psu8_plan(p);
         return fail(DD_ERR_CUDA, std::string("ps u8 descriptor upload: ") + cudaGetErrorString(e));
     }
-    e = cudaFuncSetAttribute(dd_ps_u8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->smem);
+    e = cudaFuncSetAttribute(psu8_kernel_for(kw), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->smem);
     if (e != cudaSuccess) {
         cudaGetLastError();
         return DD_OK;                                     // stays unusable; the other kernels serve
     }
     t->ok = true;
+    return DD_OK;
+}
+
+int build_psu8_plan(dd_plan* p)
+{
+    p->psu8 = nullptr;
+    if (p->ndm == 0 || p->dtype != DD_U8) return DD_OK;
+    // 128-trial tiles share the pattern rows between more trials (config 2: 4.82 vs 5.01 ms); plans of
+    // at most 64 trials, or whose rows do not fit then, take 64-trial tiles
+    for (int kw : {8, 4}) {
+        if (kw == 8 && p->ndm <= 64) continue;
+        int rc = try_build_psu8(p, kw);
+        if (rc != DD_OK) return rc;
+        if (psu8_plan_usable(p)) break;
+        destroy_psu8_plan(p);
+    }
     return DD_OK;
 }
 
@@ -475,6 +502,7 @@ bool psu8_plan_usable(const dd_plan* p) { return p->psu8 && p->psu8->ok; }
 bool psu8_args_ok(const dd_plan* p, const ExecArgs& a)
 {
     if (!psu8_plan_usable(p)) return false;
+    const int kTB = 2 * 32 * kAccPerLane / p->psu8->kw;
     if ((a.nsamp_out + kTB - 1) / kTB > 65535 || a.nbeams > 65535) return false;
     if ((int64_t)a.nbeams * p->nchans > 65535) return false;          // grid.y of the front end
     if ((a.nsamp_out + p->host.maxshift + 4096) / 8 >= ((int64_t)1 << 31)) return false;   // tensor coordinates
@@ -538,8 +566,9 @@ int launch_psu8(const dd_plan* p, const ExecArgs& a)
     q.out_stride = a.out_stride;
     q.out_beam_stride = a.out_beam_stride;
     q.vec_ok = !(((uintptr_t)a.D & 15) || (a.out_stride & 3) || (a.nbeams > 1 && (a.out_beam_stride & 3)));
+    const int kTB = 2 * 32 * kAccPerLane / t->kw;
     dim3 grid((unsigned)t->ntiles, (unsigned)((a.nsamp_out + kTB - 1) / kTB), (unsigned)a.nbeams);
-    dd_ps_u8_kernel<<<grid, kThreads + 32, t->smem, st>>>(q, tmap);
+    psu8_kernel_for(t->kw)<<<grid, kThreads + 32, t->smem, st>>>(q, tmap);
     cudaError_t e = cudaGetLastError();
     cudaFreeAsync(W, st);
     if (e != cudaSuccess) return fail(DD_ERR_CUDA, std::string("ps u8 launch: ") + cudaGetErrorString(e));
