@@ -5,6 +5,7 @@
 
 #include <algorithm>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "dd_internal.h"
@@ -58,8 +59,10 @@ static size_t elem_size(int dtype) { return dtype == DD_F32 ? 4 : 1; }
 int workspace_alloc(void** out, size_t bytes, void* stream)
 {
     static cudaMemPool_t pools[64] = {};
+    static std::mutex pools_mutex;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
+    std::lock_guard<std::mutex> lock(pools_mutex);
     if (e == cudaSuccess && dev >= 0 && dev < 64 && !pools[dev]) {
         cudaMemPoolProps props = {};
         props.allocType = cudaMemAllocationTypePinned;
