@@ -79,6 +79,13 @@ int64_t dd_max_shift(int nchans, double fch1, double foff, double tsamp,
 int dd_shift_table(int nchans, double fch1, double foff, double tsamp,
                    const double* dm_list, int ndm, int32_t* host_out);
 
+/* Delay-pattern statistics behind the partial-sum kernels, host only, no GPU needed:
+ * over all tiles of `tile_trials` consecutive sorted trials and all groups of `group` adjacent channels
+ * (1 <= group <= 8), the number of distinct vectors (s(d,c0+k) - s(d,c0))_{k<group} among a tile's
+ * trials.  Writes the mean to *mean_out and the maximum to *max_out (HOST pointers). */
+int dd_pattern_stats(int nchans, double fch1, double foff, double tsamp, const double* dm_list, int ndm,
+                     int group, int tile_trials, double* mean_out, int* max_out);
+
 /* ---- one-shot calls (north_star signature): X, D are DEVICE pointers ---------------------
  * X: [nchans][nsamp + maxshift] contiguous; D: [ndm][nsamp] contiguous, rows in dm_list order.
  * Builds a plan, runs it on the legacy default stream, synchronises, destroys the plan. */

@@ -29,6 +29,8 @@ SIGNATURES = {
     "dd_version": (C.c_char_p, []),
     "dd_max_shift": (_i64, [C.c_int, C.c_double, C.c_double, C.c_double, _dp, C.c_int]),
     "dd_shift_table": (C.c_int, [C.c_int, C.c_double, C.c_double, C.c_double, _dp, C.c_int, _vp]),
+    "dd_pattern_stats": (C.c_int, [C.c_int, C.c_double, C.c_double, C.c_double, _dp, C.c_int, C.c_int, C.c_int,
+                                   C.POINTER(C.c_double), C.POINTER(C.c_int)]),
     "dd_dedisperse_f32": (C.c_int, [_vp, C.c_int, _i64, C.c_double, C.c_double, C.c_double, _dp, C.c_int, _vp]),
     "dd_dedisperse_u8_i32": (C.c_int, [_vp, C.c_int, _i64, C.c_double, C.c_double, C.c_double, _dp, C.c_int, _vp]),
     "dd_dedisperse_f32_host": (C.c_int, [_vp, C.c_int, _i64, C.c_double, C.c_double, C.c_double, _dp, C.c_int, _vp]),
@@ -132,6 +134,14 @@ def dd_shift_table(nchans, fch1, foff, tsamp, dm_list) -> np.ndarray:
     out = np.empty((n, nchans), dtype=np.int32)
     _check(lib().dd_shift_table(nchans, fch1, foff, tsamp, p, n, out.ctypes.data), "dd_shift_table")
     return out
+
+
+def dd_pattern_stats(nchans, fch1, foff, tsamp, dm_list, group, tile_trials):
+    a, p, n = _dms(dm_list)
+    mean, mx = C.c_double(0.0), C.c_int(0)
+    _check(lib().dd_pattern_stats(nchans, fch1, foff, tsamp, p, n, group, tile_trials, C.byref(mean), C.byref(mx)),
+           "dd_pattern_stats")
+    return float(mean.value), int(mx.value)
 
 
 def dd_dedisperse_f32(X, nchans, nsamp, fch1, foff, tsamp, dm_list, D) -> None:

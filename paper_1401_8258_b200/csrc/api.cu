@@ -9,6 +9,7 @@
 #include <new>
 
 #include "dd_internal.h"
+#include "ps_host.h"
 
 namespace dd {
 
@@ -145,6 +146,32 @@ int dd_shift_table(int nchans, double fch1, double foff, double tsamp, const dou
     for (int r = 0; r < ndm; ++r)
         std::memcpy(host_out + (size_t)t.order[r] * nchans, &t.shift[(size_t)r * nchans],
                     (size_t)nchans * sizeof(int32_t));
+    return DD_OK;
+}
+
+int dd_pattern_stats(int nchans, double fch1, double foff, double tsamp, const double* dm_list, int ndm,
+                     int group, int tile_trials, double* mean_out, int* max_out)
+{
+    if (!mean_out || !max_out) return fail(DD_ERR_BAD_ARG, "null output");
+    if (group < 1 || group > kPsGMax) return fail(DD_ERR_BAD_ARG, "group must be 1..8");
+    if (tile_trials < 1 || tile_trials > 4096) return fail(DD_ERR_BAD_ARG, "tile_trials must be 1..4096");
+    HostTable t;
+    int rc = build_host_table(nchans, fch1, foff, tsamp, dm_list, ndm, &t);
+    if (rc != DD_OK) return rc;
+    *mean_out = 0.0;
+    *max_out = 0;
+    if (ndm == 0) return DD_OK;
+    const int ntiles = (ndm + tile_trials - 1) / tile_trials, ngroups = (nchans + group - 1) / group;
+    std::vector<PsRow> rows;
+    std::vector<int> slot(tile_trials);
+    double sum = 0.0;
+    for (int tile = 0; tile < ntiles; ++tile)
+        for (int g = 0; g < ngroups; ++g) {
+            ps_classify(t, group, tile_trials, tile, g, rows, slot.data());
+            sum += (double)rows.size();
+            *max_out = std::max(*max_out, (int)rows.size());
+        }
+    *mean_out = sum / ((double)ntiles * ngroups);
     return DD_OK;
 }
 
