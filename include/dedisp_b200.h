@@ -51,7 +51,8 @@ enum {
     DD_ERR_UNSUPPORTED = -2,   /* no sm_100 device, or a dtype/kernel the plan does not have */
     DD_ERR_NOMEM       = -3,
     DD_ERR_CUDA        = -4,   /* a CUDA runtime call failed; see dd_last_error() */
-    DD_ERR_STATE       = -5    /* stream pushed beyond its declared max_chunk, etc. */
+    DD_ERR_STATE       = -5    /* stream pushed beyond its declared max_chunk; the current CUDA device is
+                                  not the one the plan was created on */
 };
 
 enum { DD_F32 = 0,   /* float32 in, float32 out  */
@@ -59,11 +60,11 @@ enum { DD_F32 = 0,   /* float32 in, float32 out  */
 
 /* kernel selection for dd_plan_set_kernel (tests and benchmarks; default DD_KERNEL_AUTO) */
 enum { DD_KERNEL_AUTO    = 0,
-       DD_KERNEL_GENERIC = 1,   /* shared-memory channel-vector kernel, any DM list        */
-       DD_KERNEL_TMA     = 2,   /* TMA-staged kernel (byte-shifted copies, packed 16-bit lanes);
-                                   uint8 plans whose 64-trial tiles spread <= 1024 samples       */
-       DD_KERNEL_PS      = 3 }; /* TMA-staged kernels (float32 and uint8) with partial sums of 4-8
-                                   adjacent channels shared between the trials of a 64-trial tile */
+       DD_KERNEL_GENERIC = 1,   /* shared-memory channel-vector kernel (thesis Alg. 1 modernised), any DM list */
+       DD_KERNEL_PS      = 2 }; /* TMA-staged kernels (float32 and uint8) with partial sums of 4-8 adjacent
+                                   channels shared between the trials of a 64/128-trial tile; plans whose
+                                   per-trial delay steps are too coarse for them run DD_KERNEL_GENERIC
+                                   (dd_plan_describe says which and why) */
 
 const char* dd_strerror(int code);   /* static string for an error code */
 const char* dd_last_error(void);     /* thread-local detail of the last failure ("" if none) */
@@ -78,13 +79,6 @@ int64_t dd_max_shift(int nchans, double fch1, double foff, double tsamp,
 /* The whole table, HOST int32 [ndm][nchans] in dm_list order; no GPU needed. */
 int dd_shift_table(int nchans, double fch1, double foff, double tsamp,
                    const double* dm_list, int ndm, int32_t* host_out);
-
-/* Delay-pattern statistics behind the partial-sum kernels, host only, no GPU needed:
- * over all tiles of `tile_trials` consecutive sorted trials and all groups of `group` adjacent channels
- * (1 <= group <= 8), the number of distinct vectors (s(d,c0+k) - s(d,c0))_{k<group} among a tile's
- * trials.  Writes the mean to *mean_out and the maximum to *max_out (HOST pointers). */
-int dd_pattern_stats(int nchans, double fch1, double foff, double tsamp, const double* dm_list, int ndm,
-                     int group, int tile_trials, double* mean_out, int* max_out);
 
 /* ---- one-shot calls (north_star signature): X, D are DEVICE pointers ---------------------
  * X: [nchans][nsamp + maxshift] contiguous; D: [ndm][nsamp] contiguous, rows in dm_list order.
@@ -119,26 +113,42 @@ int     dd_plan_nchans(const dd_plan* plan);
 int     dd_plan_shift_table(const dd_plan* plan, int32_t* host_out);
 int     dd_plan_set_kernel(dd_plan* plan, int kernel);          /* DD_KERNEL_* */
 /* which kernel dd_execute would launch for these arguments: DD_KERNEL_PS (both dtypes, whenever the
- * plan's delay steps are fine enough for shared partial sums), DD_KERNEL_TMA (uint8; needs a 16-byte
- * aligned D and out strides that are multiples of 4) or DD_KERNEL_GENERIC */
+ * plan's delay steps are fine enough for shared partial sums) or DD_KERNEL_GENERIC */
 int     dd_plan_kernel_for(const dd_plan* plan, const void* X, int64_t in_stride,
                            int64_t in_beam_stride, const void* D, int64_t out_stride,
                            int64_t out_beam_stride, int64_t nsamp_out, int nbeams);
-/* number of kernels dd_execute launches per call (for bench.py's gpu_launches) */
-int     dd_plan_launches_per_execute(const dd_plan* plan);
+/* number of kernels dd_execute launches for these arguments (bench.py's gpu_launches): 1 for the generic
+ * kernel and for float32 input staged straight from the caller's buffer, 2 when a front end runs first
+ * (uint8 byte-shifted copies; float32 re-pitch of input that is not 16-byte aligned); 0 for empty work */
+int     dd_plan_launches_for(const dd_plan* plan, const void* X, int64_t in_stride,
+                             int64_t in_beam_stride, const void* D, int64_t out_stride,
+                             int64_t out_beam_stride, int64_t nsamp_out, int nbeams);
+/* One line of text about the plan: shape, which kernel AUTO takes and its tile shape, or why the
+ * partial-sum kernel does not take the plan (then dd_execute runs the ~4x slower generic kernel).
+ * Writes at most buflen-1 characters + NUL to buf (HOST); returns the untruncated length. */
+int     dd_plan_describe(const dd_plan* plan, char* buf, int buflen);
 
 /* X, D: DEVICE.  Strides are in ELEMENTS.  in_stride >= nsamp_out + maxshift is the distance
  * between channel rows, in_beam_stride between beams (ignored if nbeams == 1); same for D.
- * Reads X[b][c][0 .. nsamp_out + s(d,c)), writes D[b][d][0 .. nsamp_out). */
+ * Reads X[b][c][0 .. nsamp_out + s(d,c)), writes D[b][d][0 .. nsamp_out).  The current CUDA
+ * device must be the one the plan was created on (else DD_ERR_STATE). */
 int     dd_execute(const dd_plan* plan, const void* X, int64_t in_stride, int64_t in_beam_stride,
                    void* D, int64_t out_stride, int64_t out_beam_stride,
                    int64_t nsamp_out, int nbeams, void* cuda_stream);
 
-/* X, D: HOST (pinned memory makes the copies asynchronous), one beam.  Uploads X in time slices,
- * runs dd_execute per slice and downloads D, the three overlapped on internal streams; returns
- * after everything has landed in D.  Device buffers are cached in the plan between calls. */
-int     dd_execute_host(dd_plan* plan, const void* X, int64_t in_stride, void* D,
-                        int64_t out_stride, int64_t nsamp_out);
+/* X, D: HOST (pinned memory makes the copies asynchronous), same layout and strides as dd_execute.
+ * Uploads X in time slices, runs dd_execute per slice and downloads D, the three overlapped on
+ * internal streams; returns after everything has landed in D (also on failure: no copy that
+ * references X or D is in flight when the call returns).  Device buffers are cached in the plan
+ * between calls, so one plan must not be used by two host threads at once. */
+int     dd_execute_host(dd_plan* plan, const void* X, int64_t in_stride, int64_t in_beam_stride,
+                        void* D, int64_t out_stride, int64_t out_beam_stride,
+                        int64_t nsamp_out, int nbeams);
+
+/* Per-call workspaces (uint8 byte-shifted copies = 4x the input, re-pitched float32 input) come from
+ * a stream-ordered memory pool owned by the library that keeps its memory between calls.  This
+ * returns all unused pool memory to the driver (every device). */
+int     dd_release_workspaces(void);
 
 /* ---- streaming (the last maxshift spectra are kept at the head of the buffer
  * and the next input appended; buffer sizing eq 3.3) ------------------- */
@@ -150,7 +160,9 @@ int     dd_stream_create(dd_stream** out, const dd_plan* plan, int64_t max_chunk
 /* X_new: DEVICE [nbeams][nchans][n_new] (strides in elements), 0 <= n_new <= max_chunk.
  * Emits into D_out (DEVICE, [nbeams][ndm][>= *n_out]) every output sample whose full sweep is
  * now available: *n_out = max(0, total_in - maxshift) - total_out_so_far.  The concatenation
- * of the emitted blocks equals the one-shot result on the concatenated input, bit for bit. */
+ * of the emitted blocks equals the one-shot result on the concatenated input, bit for bit.
+ * The append, the kernels and the carry copy are ordered on `cuda_stream` only: use ONE CUDA stream
+ * per dd_stream (or synchronise between pushes made on different streams), and one host thread. */
 int     dd_stream_push(dd_stream* s, const void* X_new, int64_t in_stride, int64_t in_beam_stride,
                        int64_t n_new, void* D_out, int64_t out_stride, int64_t out_beam_stride,
                        int64_t* n_out, void* cuda_stream);

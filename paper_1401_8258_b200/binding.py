@@ -16,7 +16,7 @@ from . import build as _build
 
 DD_OK, DD_ERR_BAD_ARG, DD_ERR_UNSUPPORTED, DD_ERR_NOMEM, DD_ERR_CUDA, DD_ERR_STATE = 0, -1, -2, -3, -4, -5
 DD_F32, DD_U8 = 0, 1
-DD_KERNEL_AUTO, DD_KERNEL_GENERIC, DD_KERNEL_TMA, DD_KERNEL_PS = 0, 1, 2, 3
+DD_KERNEL_AUTO, DD_KERNEL_GENERIC, DD_KERNEL_PS = 0, 1, 2
 
 _dp = C.POINTER(C.c_double)
 _vp = C.c_void_p
@@ -29,8 +29,6 @@ SIGNATURES = {
     "dd_version": (C.c_char_p, []),
     "dd_max_shift": (_i64, [C.c_int, C.c_double, C.c_double, C.c_double, _dp, C.c_int]),
     "dd_shift_table": (C.c_int, [C.c_int, C.c_double, C.c_double, C.c_double, _dp, C.c_int, _vp]),
-    "dd_pattern_stats": (C.c_int, [C.c_int, C.c_double, C.c_double, C.c_double, _dp, C.c_int, C.c_int, C.c_int,
-                                   C.POINTER(C.c_double), C.POINTER(C.c_int)]),
     "dd_dedisperse_f32": (C.c_int, [_vp, C.c_int, _i64, C.c_double, C.c_double, C.c_double, _dp, C.c_int, _vp]),
     "dd_dedisperse_u8_i32": (C.c_int, [_vp, C.c_int, _i64, C.c_double, C.c_double, C.c_double, _dp, C.c_int, _vp]),
     "dd_dedisperse_f32_host": (C.c_int, [_vp, C.c_int, _i64, C.c_double, C.c_double, C.c_double, _dp, C.c_int, _vp]),
@@ -43,9 +41,11 @@ SIGNATURES = {
     "dd_plan_shift_table": (C.c_int, [_vp, _vp]),
     "dd_plan_set_kernel": (C.c_int, [_vp, C.c_int]),
     "dd_plan_kernel_for": (C.c_int, [_vp, _vp, _i64, _i64, _vp, _i64, _i64, _i64, C.c_int]),
-    "dd_plan_launches_per_execute": (C.c_int, [_vp]),
+    "dd_plan_launches_for": (C.c_int, [_vp, _vp, _i64, _i64, _vp, _i64, _i64, _i64, C.c_int]),
+    "dd_plan_describe": (C.c_int, [_vp, C.c_char_p, C.c_int]),
+    "dd_release_workspaces": (C.c_int, []),
     "dd_execute": (C.c_int, [_vp, _vp, _i64, _i64, _vp, _i64, _i64, _i64, C.c_int, _vp]),
-    "dd_execute_host": (C.c_int, [_vp, _vp, _i64, _vp, _i64, _i64]),
+    "dd_execute_host": (C.c_int, [_vp, _vp, _i64, _i64, _vp, _i64, _i64, _i64, C.c_int]),
     "dd_stream_create": (C.c_int, [C.POINTER(_vp), _vp, _i64, C.c_int]),
     "dd_stream_push": (C.c_int, [_vp, _vp, _i64, _i64, _i64, _vp, _i64, _i64, C.POINTER(_i64), _vp]),
     "dd_stream_reset": (C.c_int, [_vp]),
@@ -136,12 +136,8 @@ def dd_shift_table(nchans, fch1, foff, tsamp, dm_list) -> np.ndarray:
     return out
 
 
-def dd_pattern_stats(nchans, fch1, foff, tsamp, dm_list, group, tile_trials):
-    a, p, n = _dms(dm_list)
-    mean, mx = C.c_double(0.0), C.c_int(0)
-    _check(lib().dd_pattern_stats(nchans, fch1, foff, tsamp, p, n, group, tile_trials, C.byref(mean), C.byref(mx)),
-           "dd_pattern_stats")
-    return float(mean.value), int(mx.value)
+def dd_release_workspaces() -> None:
+    _check(lib().dd_release_workspaces(), "dd_release_workspaces")
 
 
 def dd_dedisperse_f32(X, nchans, nsamp, fch1, foff, tsamp, dm_list, D) -> None:
@@ -198,17 +194,24 @@ class Plan:
         return _check(lib().dd_plan_kernel_for(self._h, _ptr(X), in_stride, in_beam_stride, _ptr(D), out_stride,
                                                out_beam_stride, nsamp_out, nbeams), "dd_plan_kernel_for")
 
-    def launches_per_execute(self) -> int:
-        return _check(lib().dd_plan_launches_per_execute(self._h), "dd_plan_launches_per_execute")
+    def launches_for(self, X, in_stride, in_beam_stride, D, out_stride, out_beam_stride, nsamp_out, nbeams=1) -> int:
+        return _check(lib().dd_plan_launches_for(self._h, _ptr(X), in_stride, in_beam_stride, _ptr(D), out_stride,
+                                                 out_beam_stride, nsamp_out, nbeams), "dd_plan_launches_for")
+
+    def describe(self) -> str:
+        buf = C.create_string_buffer(1024)
+        _check(lib().dd_plan_describe(self._h, buf, len(buf)), "dd_plan_describe")
+        return buf.value.decode()
 
     def execute(self, X, in_stride, in_beam_stride, D, out_stride, out_beam_stride, nsamp_out, nbeams=1,
                 stream=None) -> None:
         _check(lib().dd_execute(self._h, _ptr(X), in_stride, in_beam_stride, _ptr(D), out_stride,
                                 out_beam_stride, nsamp_out, nbeams, _stream_ptr(stream)), "dd_execute")
 
-    def execute_host(self, X, in_stride, D, out_stride, nsamp_out) -> None:
-        _check(lib().dd_execute_host(self._h, _ptr(X), in_stride, _ptr(D), out_stride, nsamp_out),
-               "dd_execute_host")
+    def execute_host(self, X, in_stride, in_beam_stride, D, out_stride, out_beam_stride, nsamp_out,
+                     nbeams=1) -> None:
+        _check(lib().dd_execute_host(self._h, _ptr(X), in_stride, in_beam_stride, _ptr(D), out_stride,
+                                     out_beam_stride, nsamp_out, nbeams), "dd_execute_host")
 
 
 class Stream:

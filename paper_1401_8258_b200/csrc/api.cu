@@ -57,10 +57,11 @@ static size_t elem_size(int dtype) { return dtype == DD_F32 ? 4 : 1; }
 // library's own that keeps its memory between calls (release threshold = max): the default pool
 // would return the memory at the next synchronisation and the following call would pay for a
 // fresh physical allocation.
+static cudaMemPool_t pools[64] = {};
+static std::mutex pools_mutex;
+
 int workspace_alloc(void** out, size_t bytes, void* stream)
 {
-    static cudaMemPool_t pools[64] = {};
-    static std::mutex pools_mutex;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     std::lock_guard<std::mutex> lock(pools_mutex);
@@ -86,6 +87,29 @@ int workspace_alloc(void** out, size_t bytes, void* stream)
         cudaGetLastError();
         return fail(DD_ERR_NOMEM, std::string("workspace allocation: ") + cudaGetErrorString(e));
     }
+    return DD_OK;
+}
+
+int ensure_dyn_smem(const void* func, size_t bytes)
+{
+    struct Key { const void* f; int dev; size_t have; };
+    static std::vector<Key> cache;
+    static std::mutex m;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail("cudaGetDevice", e);
+    std::lock_guard<std::mutex> lock(m);
+    Key* k = nullptr;
+    for (Key& c : cache)
+        if (c.f == func && c.dev == dev) k = &c;
+    if (k && k->have >= bytes) return DD_OK;
+    e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return cuda_fail("cudaFuncSetAttribute(MaxDynamicSharedMemorySize)", e);
+    }
+    if (k) k->have = bytes;
+    else cache.push_back({func, dev, bytes});
     return DD_OK;
 }
 
@@ -149,32 +173,6 @@ int dd_shift_table(int nchans, double fch1, double foff, double tsamp, const dou
     return DD_OK;
 }
 
-int dd_pattern_stats(int nchans, double fch1, double foff, double tsamp, const double* dm_list, int ndm,
-                     int group, int tile_trials, double* mean_out, int* max_out)
-{
-    if (!mean_out || !max_out) return fail(DD_ERR_BAD_ARG, "null output");
-    if (group < 1 || group > kPsGMax) return fail(DD_ERR_BAD_ARG, "group must be 1..8");
-    if (tile_trials < 1 || tile_trials > 4096) return fail(DD_ERR_BAD_ARG, "tile_trials must be 1..4096");
-    HostTable t;
-    int rc = build_host_table(nchans, fch1, foff, tsamp, dm_list, ndm, &t);
-    if (rc != DD_OK) return rc;
-    *mean_out = 0.0;
-    *max_out = 0;
-    if (ndm == 0) return DD_OK;
-    const int ntiles = (ndm + tile_trials - 1) / tile_trials, ngroups = (nchans + group - 1) / group;
-    std::vector<PsRow> rows;
-    std::vector<int> slot(tile_trials);
-    double sum = 0.0;
-    for (int tile = 0; tile < ntiles; ++tile)
-        for (int g = 0; g < ngroups; ++g) {
-            ps_classify(t, group, tile_trials, tile, g, rows, slot.data());
-            sum += (double)rows.size();
-            *max_out = std::max(*max_out, (int)rows.size());
-        }
-    *mean_out = sum / ((double)ntiles * ngroups);
-    return DD_OK;
-}
-
 // ------------------------------------------------------------------------------ plan
 
 int dd_plan_create(dd_plan** out, int dtype, int nchans, double fch1, double foff, double tsamp,
@@ -231,8 +229,7 @@ int dd_plan_create(dd_plan** out, int dtype, int nchans, double fch1, double fof
             return cuda_fail("table upload", e);
         }
     }
-    rc = build_tma_plan(p);
-    if (rc == DD_OK) rc = build_ps_plan(p);
+    rc = build_ps_plan(p);
     if (rc == DD_OK) rc = build_psu8_plan(p);
     if (rc != DD_OK) {
         dd_plan_destroy(p);
@@ -256,7 +253,6 @@ void dd_plan_destroy(dd_plan* p)
         if (w->s_out) cudaStreamDestroy(w->s_out);
         delete w;
     }
-    destroy_tma_plan(p);
     destroy_ps_plan(p);
     destroy_psu8_plan(p);
     if (p->d_shift) cudaFree(p->d_shift);
@@ -284,14 +280,23 @@ int dd_plan_shift_table(const dd_plan* p, int32_t* host_out)
 int dd_plan_set_kernel(dd_plan* p, int kernel)
 {
     if (!p) return fail(DD_ERR_BAD_ARG, "plan is null");
-    if (kernel != DD_KERNEL_AUTO && kernel != DD_KERNEL_GENERIC && kernel != DD_KERNEL_TMA &&
-        kernel != DD_KERNEL_PS)
+    if (kernel != DD_KERNEL_AUTO && kernel != DD_KERNEL_GENERIC && kernel != DD_KERNEL_PS)
         return fail(DD_ERR_BAD_ARG, "unknown kernel id");
     if (kernel == DD_KERNEL_PS && !ps_plan_usable(p) && !psu8_plan_usable(p))
         return fail(DD_ERR_UNSUPPORTED, "the partial-sum kernel does not take this plan (dtype or per-trial delay steps)");
-    if (kernel == DD_KERNEL_TMA && !tma_plan_usable(p))
-        return fail(DD_ERR_UNSUPPORTED, "the TMA-staged kernel does not take this plan (dtype or per-trial delay steps)");
     p->kernel_pref = kernel;
+    return DD_OK;
+}
+
+// The plan's tables, descriptors and workspaces live on the device it was created on.
+static int check_device(const dd_plan* p)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail("cudaGetDevice", e);
+    if (dev != p->device)
+        return fail(DD_ERR_STATE, "the current CUDA device (" + std::to_string(dev) + ") is not the plan's device (" +
+                                      std::to_string(p->device) + ")");
     return DD_OK;
 }
 
@@ -317,8 +322,7 @@ static void fill_args(const dd_plan* p, ExecArgs* a, const void* X, int64_t in_s
 static int kernel_for(const dd_plan* p, const ExecArgs& a)
 {
     if (p->kernel_pref == DD_KERNEL_GENERIC) return DD_KERNEL_GENERIC;
-    if (p->kernel_pref != DD_KERNEL_TMA && psu8_plan_usable(p) && psu8_args_ok(p, a)) return DD_KERNEL_PS;
-    if (p->kernel_pref != DD_KERNEL_PS && tma_plan_usable(p) && tma_args_ok(p, a)) return DD_KERNEL_TMA;
+    if (psu8_plan_usable(p) && psu8_args_ok(p, a)) return DD_KERNEL_PS;
     if (ps_plan_usable(p) && ps_args_ok(p, a)) return DD_KERNEL_PS;
     return DD_KERNEL_GENERIC;
 }
@@ -335,13 +339,20 @@ int dd_plan_kernel_for(const dd_plan* p, const void* X, int64_t in_stride, int64
     return kernel_for(p, a);
 }
 
-int dd_plan_launches_per_execute(const dd_plan* p)
+int dd_plan_launches_for(const dd_plan* p, const void* X, int64_t in_stride, int64_t in_beam_stride,
+                         const void* D, int64_t out_stride, int64_t out_beam_stride, int64_t nsamp_out,
+                         int nbeams)
 {
     if (!p) return fail(DD_ERR_BAD_ARG, "plan is null");
-    // the TMA-staged uint8 path runs the byte-shift front end and the dedispersion kernel; the
-    // float32 partial-sum kernel reads 16-byte aligned input directly (one launch; two when the
-    // caller's buffer has to be re-pitched first)
-    return (p->kernel_pref != DD_KERNEL_GENERIC && (tma_plan_usable(p) || psu8_plan_usable(p))) ? 2 : 1;
+    if (nbeams < 1 || nsamp_out < 0) return fail(DD_ERR_BAD_ARG, "bad nbeams / nsamp_out");
+    if (p->ndm == 0 || nsamp_out == 0) return 0;
+    ExecArgs a;
+    fill_args(p, &a, X, in_stride, in_beam_stride, const_cast<void*>(D), out_stride, out_beam_stride,
+              nsamp_out, nbeams, nullptr);
+    if (kernel_for(p, a) != DD_KERNEL_PS) return 1;       // generic kernel: one launch
+    // uint8: byte-shift front end + dedispersion kernel; float32: one launch when the input is staged
+    // straight from the caller's buffer, two when it has to be re-pitched first
+    return p->dtype == DD_U8 ? 2 : ps_launches(p, a);
 }
 
 int dd_execute(const dd_plan* p, const void* X, int64_t in_stride, int64_t in_beam_stride, void* D,
@@ -356,6 +367,10 @@ int dd_execute(const dd_plan* p, const void* X, int64_t in_stride, int64_t in_be
     if (in_stride < nsamp_out + p->host.maxshift)
         return fail(DD_ERR_BAD_ARG, "in_stride is shorter than nsamp_out + maxshift");
     if (out_stride < nsamp_out) return fail(DD_ERR_BAD_ARG, "out_stride is shorter than nsamp_out");
+    {
+        int rc = check_device(p);
+        if (rc != DD_OK) return rc;
+    }
     if (nbeams > 1 && (in_beam_stride <= 0 || out_beam_stride <= 0))
         return fail(DD_ERR_BAD_ARG, "beam strides must be positive when nbeams > 1");
     if (p->dtype == DD_F32 && (((uintptr_t)X | (uintptr_t)D) & 3))
@@ -367,13 +382,39 @@ int dd_execute(const dd_plan* p, const void* X, int64_t in_stride, int64_t in_be
     fill_args(p, &a, X, in_stride, in_beam_stride, D, out_stride, out_beam_stride, nsamp_out, nbeams,
               cuda_stream);
     const int k = kernel_for(p, a);
-    if (p->kernel_pref == DD_KERNEL_TMA && k != DD_KERNEL_TMA)
-        return fail(DD_ERR_UNSUPPORTED, "TMA kernel forced but the output is not 16-byte aligned or the buffer is tiny");
     if (p->kernel_pref == DD_KERNEL_PS && k != DD_KERNEL_PS)
         return fail(DD_ERR_UNSUPPORTED, "partial-sum kernel forced but the grid does not fit");
-    if (k == DD_KERNEL_TMA) return launch_tma(p, a);
     if (k == DD_KERNEL_PS) return p->dtype == DD_U8 ? launch_psu8(p, a) : launch_ps(p, a);
     return launch_generic(p->dtype, p->generic_kb, p->generic_spread, a);
+}
+
+int dd_release_workspaces(void)
+{
+    std::lock_guard<std::mutex> lock(pools_mutex);
+    for (int d = 0; d < 64; ++d)
+        if (pools[d]) {
+            cudaError_t e = cudaMemPoolTrimTo(pools[d], 0);
+            if (e != cudaSuccess) return cuda_fail("cudaMemPoolTrimTo", e);
+        }
+    return DD_OK;
+}
+
+int dd_plan_describe(const dd_plan* p, char* buf, int buflen)
+{
+    if (!p || !buf || buflen < 1) return fail(DD_ERR_BAD_ARG, "null argument");
+    std::string t = std::string(p->dtype == DD_U8 ? "uint8->int32" : "float32") + ", " + std::to_string(p->nchans) +
+                    " channels x " + std::to_string(p->ndm) + " trials, maxshift " +
+                    std::to_string(p->host.maxshift) + ", device " + std::to_string(p->device) + "; ";
+    if (p->ndm == 0) t += "empty plan (nothing to launch)";
+    else if (p->dtype == DD_U8) t += psu8_plan_usable(p) ? psu8_describe(p) : "partial-sum kernel unavailable: " + p->ps_why;
+    else t += ps_plan_usable(p) ? ps_describe(p) : "partial-sum kernel unavailable: " + p->ps_why;
+    if (p->ndm > 0) t += "; generic kernel: " + std::to_string(p->generic_kb) + " trials per block";
+    if (p->kernel_pref != DD_KERNEL_AUTO)
+        t += std::string("; forced: ") + (p->kernel_pref == DD_KERNEL_PS ? "ps" : "generic");
+    const int n = (int)std::min<size_t>(t.size(), (size_t)buflen - 1);
+    std::memcpy(buf, t.data(), (size_t)n);
+    buf[n] = 0;
+    return (int)t.size();
 }
 
 // ------------------------------------------------------------------------------ one-shot
@@ -410,21 +451,29 @@ int dd_dedisperse_u8_i32(const uint8_t* X, int nchans, int64_t nsamp, double fch
 
 static int64_t round_up(int64_t v, int64_t m) { return (v + m - 1) / m * m; }
 
-int dd_execute_host(dd_plan* p, const void* X, int64_t in_stride, void* D, int64_t out_stride,
-                    int64_t nsamp_out)
+int dd_execute_host(dd_plan* p, const void* X, int64_t in_stride, int64_t in_beam_stride, void* D,
+                    int64_t out_stride, int64_t out_beam_stride, int64_t nsamp_out, int nbeams)
 {
     if (!p) return fail(DD_ERR_BAD_ARG, "plan is null");
     if (nsamp_out < 0) return fail(DD_ERR_BAD_ARG, "nsamp_out must be >= 0");
+    if (nbeams < 1) return fail(DD_ERR_BAD_ARG, "nbeams must be >= 1");
     if (p->ndm == 0 || nsamp_out == 0) return DD_OK;
     if (!X || !D) return fail(DD_ERR_BAD_ARG, "X or D is null");
     const int64_t ms = p->host.maxshift;
     if (in_stride < nsamp_out + ms) return fail(DD_ERR_BAD_ARG, "in_stride is shorter than nsamp_out + maxshift");
     if (out_stride < nsamp_out) return fail(DD_ERR_BAD_ARG, "out_stride is shorter than nsamp_out");
+    if (nbeams > 1 && (in_beam_stride < (int64_t)p->nchans * in_stride || out_beam_stride < (int64_t)p->ndm * out_stride))
+        return fail(DD_ERR_BAD_ARG, "beam strides are shorter than a beam");
+    {
+        int rc = check_device(p);
+        if (rc != DD_OK) return rc;
+    }
     const size_t es = elem_size(p->dtype);
     const int64_t dstride_in = round_up(nsamp_out + ms, 64);
     const int64_t dstride_out = round_up(nsamp_out, 64);
-    const size_t xb = (size_t)p->nchans * dstride_in * es;
-    const size_t db = (size_t)p->ndm * dstride_out * 4;
+    const int64_t dbeam_in = (int64_t)p->nchans * dstride_in, dbeam_out = (int64_t)p->ndm * dstride_out;
+    const size_t xb = (size_t)nbeams * dbeam_in * es;
+    const size_t db = (size_t)nbeams * dbeam_out * 4;
 
     if (!p->host_ws) {
         p->host_ws = new (std::nothrow) dd_host_ws;
@@ -468,32 +517,49 @@ int dd_execute_host(dd_plan* p, const void* X, int64_t in_stride, void* D, int64
         w->ev_in.push_back(a);
         w->ev_run.push_back(b);
     }
+    // After the first enqueue no path may return before the three streams have drained: the async
+    // copies reference the caller's X and D.
+    int rc = DD_OK;
+    auto cuda_ok = [&](cudaError_t e, const char* what) {
+        if (e != cudaSuccess && rc == DD_OK) rc = cuda_fail(what, e);
+        return e == cudaSuccess;
+    };
     int64_t in_done = 0;   // input columns already uploaded
-    for (int k = 0; k < nslices; ++k) {
+    for (int k = 0; k < nslices && rc == DD_OK; ++k) {
         const int64_t ta = (int64_t)k * slice, tb = std::min(nsamp_out, ta + slice);
         const int64_t in_end = tb + ms;
         if (in_end > in_done) {
-            DD_CUDA(cudaMemcpy2DAsync((char*)w->dX + in_done * es, dstride_in * es,
-                                      (const char*)X + in_done * es, in_stride * es,
-                                      (size_t)(in_end - in_done) * es, p->nchans,
-                                      cudaMemcpyHostToDevice, w->s_in));
+            for (int b = 0; b < nbeams && rc == DD_OK; ++b)
+                cuda_ok(cudaMemcpy2DAsync((char*)w->dX + ((size_t)b * dbeam_in + in_done) * es, dstride_in * es,
+                                          (const char*)X + ((size_t)b * in_beam_stride + in_done) * es,
+                                          in_stride * es, (size_t)(in_end - in_done) * es, p->nchans,
+                                          cudaMemcpyHostToDevice, w->s_in),
+                        "cudaMemcpy2DAsync(H2D)");
             in_done = in_end;
         }
-        DD_CUDA(cudaEventRecord(w->ev_in[k], w->s_in));
-        DD_CUDA(cudaStreamWaitEvent(w->s_run, w->ev_in[k], 0));
-        int rc = dd_execute(p, (const char*)w->dX + ta * es, dstride_in, 0, (char*)w->dD + ta * 4,
-                            dstride_out, 0, tb - ta, 1, w->s_run);
-        if (rc != DD_OK) return rc;
-        DD_CUDA(cudaEventRecord(w->ev_run[k], w->s_run));
-        DD_CUDA(cudaStreamWaitEvent(w->s_out, w->ev_run[k], 0));
-        DD_CUDA(cudaMemcpy2DAsync((char*)D + ta * 4, out_stride * 4, (const char*)w->dD + ta * 4,
-                                  dstride_out * 4, (size_t)(tb - ta) * 4, p->ndm,
-                                  cudaMemcpyDeviceToHost, w->s_out));
+        if (rc != DD_OK) break;
+        if (!cuda_ok(cudaEventRecord(w->ev_in[k], w->s_in), "cudaEventRecord")) break;
+        if (!cuda_ok(cudaStreamWaitEvent(w->s_run, w->ev_in[k], 0), "cudaStreamWaitEvent")) break;
+        const int erc = dd_execute(p, (const char*)w->dX + ta * es, dstride_in, dbeam_in, (char*)w->dD + ta * 4,
+                                   dstride_out, dbeam_out, tb - ta, nbeams, w->s_run);
+        if (erc != DD_OK) {
+            rc = erc;
+            break;
+        }
+        if (!cuda_ok(cudaEventRecord(w->ev_run[k], w->s_run), "cudaEventRecord")) break;
+        if (!cuda_ok(cudaStreamWaitEvent(w->s_out, w->ev_run[k], 0), "cudaStreamWaitEvent")) break;
+        for (int b = 0; b < nbeams && rc == DD_OK; ++b)
+            cuda_ok(cudaMemcpy2DAsync((char*)D + ((size_t)b * out_beam_stride + ta) * 4, out_stride * 4,
+                                      (const char*)w->dD + ((size_t)b * dbeam_out + ta) * 4, dstride_out * 4,
+                                      (size_t)(tb - ta) * 4, p->ndm, cudaMemcpyDeviceToHost, w->s_out),
+                    "cudaMemcpy2DAsync(D2H)");
     }
-    DD_CUDA(cudaStreamSynchronize(w->s_out));
-    DD_CUDA(cudaStreamSynchronize(w->s_run));
-    DD_CUDA(cudaStreamSynchronize(w->s_in));
-    return DD_OK;
+    const std::string first_error = rc != DD_OK ? g_last_error : std::string();
+    cuda_ok(cudaStreamSynchronize(w->s_out), "cudaStreamSynchronize");
+    cuda_ok(cudaStreamSynchronize(w->s_run), "cudaStreamSynchronize");
+    cuda_ok(cudaStreamSynchronize(w->s_in), "cudaStreamSynchronize");
+    if (!first_error.empty()) g_last_error = first_error;
+    return rc;
 }
 
 static int one_shot_host(int dtype, const void* X, int nchans, int64_t nsamp, double fch1, double foff,
@@ -503,7 +569,7 @@ static int one_shot_host(int dtype, const void* X, int nchans, int64_t nsamp, do
     dd_plan* p = nullptr;
     int rc = dd_plan_create(&p, dtype, nchans, fch1, foff, tsamp, dm_list, ndm);
     if (rc != DD_OK) return rc;
-    rc = dd_execute_host(p, X, nsamp + p->host.maxshift, D, nsamp, nsamp);
+    rc = dd_execute_host(p, X, nsamp + p->host.maxshift, 0, D, nsamp, 0, nsamp, 1);
     dd_plan_destroy(p);
     return rc;
 }
@@ -560,6 +626,10 @@ int dd_stream_push(dd_stream* s, const void* X_new, int64_t in_stride, int64_t i
     if (!X_new) return fail(DD_ERR_BAD_ARG, "X_new is null");
     if (in_stride < n_new) return fail(DD_ERR_BAD_ARG, "in_stride is shorter than n_new");
     const dd_plan* p = s->plan;
+    {
+        int rc = check_device(p);
+        if (rc != DD_OK) return rc;
+    }
     const size_t es = elem_size(p->dtype);
     const int nch = p->nchans;
     cudaStream_t st = (cudaStream_t)cuda_stream;

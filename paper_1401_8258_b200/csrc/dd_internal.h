@@ -17,6 +17,11 @@ int fail(int code, const std::string& msg);
 // stream-ordered workspace from the library's own pool (api.cu); free with cudaFreeAsync
 int workspace_alloc(void** out, size_t bytes, void* stream);
 
+// Raises cudaFuncAttributeMaxDynamicSharedMemorySize of kernel `func` on the current device to at
+// least `bytes` (never lowers it: the attribute belongs to the function, not to a plan, so plans
+// with different needs must not undo each other).  Call before every launch; cached per device.
+int ensure_dyn_smem(const void* func, size_t bytes);
+
 // ---- host delay table (plan.cpp; eq 2.2/2.3) ------------------------------
 struct HostTable {
     int nchans = 0;
@@ -36,7 +41,7 @@ int64_t host_max_shift(int nchans, double fch1, double foff, double tsamp, const
 // Largest s(d_last,c) - s(d_first,c) over all tiles of `kb` consecutive sorted DMs.
 int64_t max_tile_spread(const HostTable& t, int kb);
 
-// ---- kernel launchers (generic.cu / tma_u8.cu) ---------------------------------------------
+// ---- kernel launchers -----------------------------------------------------------------------
 struct ExecArgs {
     const void* X;
     void* D;
@@ -56,17 +61,11 @@ int launch_generic(int dtype, int kb, int max_spread, const ExecArgs& a);
 
 struct dd_plan;
 struct dd_host_ws;
-struct dd_tma_plan;
 struct dd_ps_plan;
 struct dd_psu8_plan;
 
 namespace dd {
-// TMA-staged kernels (tma_u8.cu): plan-time tables, eligibility, launch
-int build_tma_plan(dd_plan* p);
-void destroy_tma_plan(dd_plan* p);
-bool tma_plan_usable(const dd_plan* p);
-bool tma_args_ok(const dd_plan* p, const ExecArgs& a);
-int launch_tma(const dd_plan* p, const ExecArgs& a);
+// uint8 front end (front_u8.cu): the four byte-shifted copies ps_u8.cu stages from
 int make_shift_copies_u8(const dd_plan* p, const ExecArgs& a, uint8_t** W_out, int64_t* wcopy_out,
                          int64_t* wpitch_out);
 // float32 kernel with shared partial sums (ps_f32.cu)
@@ -76,12 +75,14 @@ bool ps_plan_usable(const dd_plan* p);
 bool ps_args_ok(const dd_plan* p, const ExecArgs& a);
 int ps_launches(const dd_plan* p, const ExecArgs& a);
 int launch_ps(const dd_plan* p, const ExecArgs& a);
+std::string ps_describe(const dd_plan* p);
 // uint8 kernel with shared partial sums (ps_u8.cu)
 int build_psu8_plan(dd_plan* p);
 void destroy_psu8_plan(dd_plan* p);
 bool psu8_plan_usable(const dd_plan* p);
 bool psu8_args_ok(const dd_plan* p, const ExecArgs& a);
 int launch_psu8(const dd_plan* p, const ExecArgs& a);
+std::string psu8_describe(const dd_plan* p);
 }  // namespace dd
 
 struct dd_plan {
@@ -95,8 +96,8 @@ struct dd_plan {
     int kernel_pref = DD_KERNEL_AUTO;
     int generic_kb = 1;
     int generic_spread = 0;
-    dd_tma_plan* tma = nullptr;         // null: the TMA-staged uint8 kernel does not take this plan
     dd_ps_plan* ps = nullptr;           // null: the float32 partial-sum kernel does not take this plan
     dd_psu8_plan* psu8 = nullptr;       // null: the uint8 partial-sum kernel does not take this plan
+    std::string ps_why;                 // why the partial-sum kernel does not take this plan (dd_plan_describe)
     dd_host_ws* host_ws = nullptr;      // device buffers / streams cached by dd_execute_host
 };

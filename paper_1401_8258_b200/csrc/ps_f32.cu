@@ -32,6 +32,7 @@
 
 #include "dd_internal.h"
 #include "ps_host.h"
+#include "tma_ptx.cuh"
 
 struct dd_ps_plan {
     bool ok = false;
@@ -69,49 +70,6 @@ constexpr int kDTrial = 20;               // [KB] flat word offset of trial j's 
 // kDTrial + KB:                             [nchunks][G] uint16 word offset, from the stage's first staged word, of
                                           //      the operand of lane 0 in channel k (zero pad if missing); 16-bit
                                           //      entries because a warp-uniform LDS.128 still costs four data cycles
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
-{
-    uint32_t done;
-    do {
-        asm volatile(
-            "{\n"
-            ".reg .pred p;\n"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-            "selp.u32 %0, 1, 0, p;\n"
-            "}\n"
-            : "=r"(done)
-            : "r"(smem_u32(bar)), "r"(parity)
-            : "memory");
-    } while (!done);
-}
-__device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
-{
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-        ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar))
-        : "memory");
-}
-__device__ __forceinline__ float lds_f32(uint32_t addr)
-{
-    float v;
-    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
-    return v;
-}
 
 struct PsParams {
     const float* X;
@@ -153,8 +111,7 @@ dd_ps_f32_kernel(const PsParams p)
             mbar_init(&ready[b], kWarps);
             mbar_init(&freeb[b], kWarps);
         }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_fence_init();
     }
     if (threadIdx.x < kXStages * kChunk)
         Xs[(threadIdx.x / kChunk) * xstage + G * p.xw + (threadIdx.x % kChunk)] = 0.0f;
@@ -298,10 +255,10 @@ __global__ void __launch_bounds__(256)
 dd_repitch_f32(const float* __restrict__ X, float* __restrict__ W, int nchans, int64_t rowlen, int64_t in_stride,
                int64_t in_beam_stride, int64_t wpitch)
 {
-    const int64_t row = blockIdx.y;
+    const int64_t row = blockIdx.x;                       // rows on grid.x: no 65535 limit on nbeams * nchans
     const float* src = X + (row / nchans) * in_beam_stride + (row % nchans) * in_stride;
     float* dst = W + row * wpitch;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < wpitch; i += (int64_t)gridDim.x * blockDim.x)
+    for (int64_t i = (int64_t)blockIdx.y * blockDim.x + threadIdx.x; i < wpitch; i += (int64_t)gridDim.y * blockDim.x)
         dst[i] = i < rowlen ? src[i] : 0.0f;
 }
 
@@ -376,7 +333,10 @@ int build_ps_plan(dd_plan* p)
                 sh = c;
             }
         }
-    if (G == 0) return DD_OK;        // per-trial delay steps too large / too many patterns: generic kernel
+    if (G == 0) {                    // per-trial delay steps too large / too many patterns: generic kernel
+        p->ps_why = "the delay patterns of a 64-trial tile do not fit shared memory (per-trial delay steps too coarse)";
+        return DD_OK;
+    }
     const int kKB = kw * kWarps, kNK = kAccPerLane / kw, kTB = 32 * kNK, kDChunk = kDTrial + kKB;
     (void)kNK;
     const int ntiles = (ndm + kKB - 1) / kKB, ngroups = (nch + G - 1) / G;
@@ -455,7 +415,10 @@ int build_ps_plan(dd_plan* p)
     wok[wk] = bounds_ok;
     });
     for (int wk = 0; wk < workers; ++wk) bounds_ok = bounds_ok && wok[wk];
-    if (!bounds_ok) return DD_OK;                         // never expected; the plan stays unusable (generic kernel)
+    if (!bounds_ok) {                                     // never expected; the plan stays unusable (generic kernel)
+        p->ps_why = "descriptor bounds check failed";
+        return DD_OK;
+    }
     cudaError_t e = cudaMalloc(&t->d_desc, desc.size() * sizeof(int32_t));
     if (e != cudaSuccess) {
         cudaGetLastError();
@@ -466,11 +429,6 @@ int build_ps_plan(dd_plan* p)
     if (e != cudaSuccess) {
         destroy_ps_plan(p);
         return fail(DD_ERR_CUDA, std::string("ps descriptor upload: ") + cudaGetErrorString(e));
-    }
-    e = cudaFuncSetAttribute(ps_kernel_for(G, kw), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->smem);
-    if (e != cudaSuccess) {
-        cudaGetLastError();
-        return DD_OK;                                     // stays unusable; generic kernel serves
     }
     t->ok = true;
     return DD_OK;
@@ -496,11 +454,19 @@ bool ps_args_ok(const dd_plan* p, const ExecArgs& a)
     if (!ps_plan_usable(p)) return false;
     const int kTB = 32 * kAccPerLane / p->ps->kw;
     if ((a.nsamp_out + kTB - 1) / kTB > 65535 || a.nbeams > 65535) return false;
-    if (!ps_direct(a) && (int64_t)a.nbeams * p->nchans > 65535) return false;   // grid.y of the re-pitch copy
+    if (!ps_direct(a) && (int64_t)a.nbeams * p->nchans > 2147483647LL) return false;   // grid.x of the re-pitch copy
     return true;
 }
 
 int ps_launches(const dd_plan* p, const ExecArgs& a) { return ps_direct(a) ? 1 : 2; }
+
+std::string ps_describe(const dd_plan* p)
+{
+    const dd_ps_plan* t = p->ps;
+    return "partial-sum kernel dd_ps_f32_kernel<G=" + std::to_string(t->G) + ", KW=" + std::to_string(t->kw) + ">: " +
+           std::to_string(16 * t->kw) + " trials x " + std::to_string(32 * kAccPerLane / t->kw) +
+           " samples per block, " + std::to_string(t->smem) + " B shared memory";
+}
 
 int launch_ps(const dd_plan* p, const ExecArgs& a)
 {
@@ -516,9 +482,9 @@ int launch_ps(const dd_plan* p, const ExecArgs& a)
     if (!ps_direct(a)) {
         const int64_t wpitch = (rowlen + 3) / 4 * 4;
         const int64_t nrows = (int64_t)a.nbeams * p->nchans;
-        int rc = workspace_alloc((void**)&W, (size_t)(nrows * wpitch) * sizeof(float), a.stream);
-        if (rc != DD_OK) return rc;
-        dim3 grid((unsigned)std::min<int64_t>((wpitch + 255) / 256, 64), (unsigned)nrows);
+        int wrc = workspace_alloc((void**)&W, (size_t)(nrows * wpitch) * sizeof(float), a.stream);
+        if (wrc != DD_OK) return wrc;
+        dim3 grid((unsigned)nrows, (unsigned)std::min<int64_t>((wpitch + 255) / 256, 64));
         dd_repitch_f32<<<grid, 256, 0, st>>>((const float*)a.X, W, p->nchans, rowlen, a.in_stride, a.in_beam_stride,
                                              wpitch);
         q.X = W;
@@ -539,6 +505,11 @@ int launch_ps(const dd_plan* p, const ExecArgs& a)
     q.out_beam_stride = a.out_beam_stride;
     const int kTB = 32 * kAccPerLane / t->kw;
     dim3 grid((unsigned)t->ntiles, (unsigned)((a.nsamp_out + kTB - 1) / kTB), (unsigned)a.nbeams);
+    int rc = ensure_dyn_smem((const void*)ps_kernel_for(t->G, t->kw), t->smem);
+    if (rc != DD_OK) {
+        if (W) cudaFreeAsync(W, st);
+        return rc;
+    }
     ps_kernel_for(t->G, t->kw)<<<grid, kThreads + 32, t->smem, st>>>(q);
     cudaError_t e = cudaGetLastError();
     if (W) cudaFreeAsync(W, st);

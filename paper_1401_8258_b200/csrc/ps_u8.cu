@@ -31,6 +31,7 @@
 
 #include "dd_internal.h"
 #include "ps_host.h"
+#include "tma_ptx.cuh"
 
 struct dd_psu8_plan {
     bool ok = false;
@@ -71,61 +72,10 @@ constexpr int kDTrial = 12;               // [KB] word offset of trial j's first
                                           //      aligned word lane 0 reads in channel k (zero pad if missing);
                                           //      [4], [5] first even-u / odd-u word the step writes (even numbers)
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
-{
-    uint32_t done;
-    do {
-        asm volatile(
-            "{\n"
-            ".reg .pred p;\n"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-            "selp.u32 %0, 1, 0, p;\n"
-            "}\n"
-            : "=r"(done)
-            : "r"(smem_u32(bar)), "r"(parity)
-            : "memory");
-    } while (!done);
-}
-__device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
-{
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-        ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar))
-        : "memory");
-}
-// tile-mode tensor copy (SASS UTMALDG): box of the tensor map at (column c0, row c1) -> dense rows in smem
-__device__ __forceinline__ void tensor_load_2d(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-        ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar))
-        : "memory");
-}
 __device__ __forceinline__ void consumer_barrier()
 {
     asm volatile("bar.sync 1, %0;" ::"n"(kThreads) : "memory");
 }
-__device__ __forceinline__ uint32_t lds_u32(uint32_t addr)
-{
-    uint32_t v;
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
-    return v;
-}
-
 struct PsU8Params {
     int32_t* D;
     const int32_t* desc;
@@ -160,8 +110,7 @@ dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
             mbar_init(&full[s], 1);
             mbar_init(&empty[s], kWarps);
         }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_fence_init();
     }
     if (threadIdx.x < kXStages * kChunk)
         reinterpret_cast<uint32_t*>(Xs + (threadIdx.x / kChunk) * xstage + kG * 4 * p.xwb)[threadIdx.x % kChunk] = 0u;
@@ -345,7 +294,10 @@ static int try_build_psu8(dd_plan* p, int kw)
         }
     }
     xwb = (xwb + 15) / 16 * 16;
-    if (xwb > 2048) return DD_OK;                         // wider than a tensor-copy box (256 x 8 bytes)
+    if (xwb > 2048) {                                     // wider than a tensor-copy box (256 x 8 bytes)
+        p->ps_why = "a trial tile's input window is wider than 2048 samples (per-trial delay steps too coarse)";
+        return DD_OK;
+    }
     // a warp step of step 2 may read up to 2 * kChunk + 128 bytes past a row's window
     const int64_t xstage = (kG * 4 * xwb + 4 * kChunk + 384 + 127) / 128 * 128;
 
@@ -378,7 +330,10 @@ static int try_build_psu8(dd_plan* p, int kw)
     const int desc_ints = kDChunk + kCE * (int)max_steps;
     const size_t smem = (size_t)kXStages * xstage + (size_t)2 * psw * 4 +
                         (size_t)kXStages * desc_ints * 4 + 2 * kXStages * 8;
-    if (smem > (size_t)kMaxSmem) return DD_OK;            // too many patterns for shared memory
+    if (smem > (size_t)kMaxSmem) {                        // too many patterns for shared memory
+        p->ps_why = "the delay patterns of a trial tile do not fit shared memory (per-trial delay steps too coarse)";
+        return DD_OK;
+    }
 
     dd_psu8_plan* t = new (std::nothrow) dd_psu8_plan;
     if (!t) return fail(DD_ERR_NOMEM, "ps u8 plan allocation failed");
@@ -452,7 +407,10 @@ static int try_build_psu8(dd_plan* p, int kw)
     wok[wk] = bounds_ok;
     });
     for (int wk = 0; wk < workers; ++wk) bounds_ok = bounds_ok && wok[wk];
-    if (!bounds_ok) return DD_OK;                         // never expected; the plan stays unusable (other kernels)
+    if (!bounds_ok) {                                     // never expected; the plan stays unusable (generic kernel)
+        p->ps_why = "descriptor bounds check failed";
+        return DD_OK;
+    }
     cudaError_t e = cudaMalloc(&t->d_desc, desc.size() * sizeof(int32_t));
     if (e != cudaSuccess) {
         cudaGetLastError();
@@ -463,11 +421,6 @@ static int try_build_psu8(dd_plan* p, int kw)
     if (e != cudaSuccess) {
         destroy_psu8_plan(p);
         return fail(DD_ERR_CUDA, std::string("ps u8 descriptor upload: ") + cudaGetErrorString(e));
-    }
-    e = cudaFuncSetAttribute(psu8_kernel_for(kw), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->smem);
-    if (e != cudaSuccess) {
-        cudaGetLastError();
-        return DD_OK;                                     // stays unusable; the other kernels serve
     }
     t->ok = true;
     return DD_OK;
@@ -499,12 +452,20 @@ void destroy_psu8_plan(dd_plan* p)
 
 bool psu8_plan_usable(const dd_plan* p) { return p->psu8 && p->psu8->ok; }
 
+std::string psu8_describe(const dd_plan* p)
+{
+    const dd_psu8_plan* t = p->psu8;
+    return "partial-sum kernel dd_ps_u8_kernel<KW=" + std::to_string(t->kw) + ">: " + std::to_string(16 * t->kw) +
+           " trials x " + std::to_string(2 * 32 * kAccPerLane / t->kw) + " samples per block, " +
+           std::to_string(t->smem) + " B shared memory, byte-shift front end";
+}
+
 bool psu8_args_ok(const dd_plan* p, const ExecArgs& a)
 {
     if (!psu8_plan_usable(p)) return false;
     const int kTB = 2 * 32 * kAccPerLane / p->psu8->kw;
     if ((a.nsamp_out + kTB - 1) / kTB > 65535 || a.nbeams > 65535) return false;
-    if ((int64_t)a.nbeams * p->nchans > 65535) return false;          // grid.y of the front end
+    if ((int64_t)a.nbeams * p->nchans * 4 > 2147483647LL) return false;      // tensor-map rows / grid.x of the front end
     if ((a.nsamp_out + p->host.maxshift + 4096) / 8 >= ((int64_t)1 << 31)) return false;   // tensor coordinates
     return true;
 }
@@ -568,6 +529,11 @@ int launch_psu8(const dd_plan* p, const ExecArgs& a)
     q.vec_ok = !(((uintptr_t)a.D & 15) || (a.out_stride & 3) || (a.nbeams > 1 && (a.out_beam_stride & 3)));
     const int kTB = 2 * 32 * kAccPerLane / t->kw;
     dim3 grid((unsigned)t->ntiles, (unsigned)((a.nsamp_out + kTB - 1) / kTB), (unsigned)a.nbeams);
+    rc = ensure_dyn_smem((const void*)psu8_kernel_for(t->kw), t->smem);
+    if (rc != DD_OK) {
+        cudaFreeAsync(W, st);
+        return rc;
+    }
     psu8_kernel_for(t->kw)<<<grid, kThreads + 32, t->smem, st>>>(q, tmap);
     cudaError_t e = cudaGetLastError();
     cudaFreeAsync(W, st);

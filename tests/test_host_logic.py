@@ -102,40 +102,3 @@ def test_product_does_not_import_the_oracle():
                 src = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(import|from)\s+oracle|#include.*oracle|dedisp_oracle",
                                      src, flags=re.M), f
-
-
-# ---------------------------------------------------------------- delay patterns behind the partial-sum kernels
-
-def _patterns_from_oracle_table(tab, group, tile):
-    """Mean / max number of distinct relative-delay vectors per (tile of sorted trials, channel group),
-    recomputed with numpy from the ORACLE's table (rows sorted by DM by construction of the workloads)."""
-    ndm, nch = tab.shape
-    counts = []
-    for t0 in range(0, ndm, tile):
-        rows = np.minimum(np.arange(t0, t0 + tile), ndm - 1)
-        for c0 in range(0, nch, group):
-            rel = tab[rows][:, c0:c0 + group] - tab[rows][:, c0:c0 + 1]
-            counts.append(len(np.unique(rel, axis=0)))
-    return float(np.mean(counts)), int(np.max(counts))
-
-
-@pytest.mark.parametrize("idx,nchans,ndm", [(2, 256, 200), (3, 512, 300), (4, 128, 130), (5, 301, 257)])
-@pytest.mark.parametrize("group,tile", [(1, 64), (2, 16), (4, 64), (8, 128), (3, 7)])
-def test_pattern_stats_match_a_numpy_recount_on_the_oracle_table(idx, nchans, ndm, group, tile):
-    w0 = synth.WORKLOADS[idx]
-    w = synth.scaled(w0, nchans=nchans, ndm=ndm, foff=w0.foff * w0.nchans / nchans)
-    mean, mx = dd.dd_pattern_stats(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list, group, tile)
-    tab = oracle.shift_table(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
-    want_mean, want_max = _patterns_from_oracle_table(np.asarray(tab, dtype=np.int64), group, tile)
-    assert mx == want_max and abs(mean - want_mean) < 1e-9
-    if group == 1:
-        assert mx == 1                                            # a single channel has one (empty) pattern
-    assert 1 <= mean <= min(tile, ndm)
-
-
-def test_pattern_counts_of_the_benchmark_workloads_stay_small():
-    # the premise of DESIGN.md 5.3: a handful of patterns per 64-trial tile and 4-channel group
-    for idx, lo, hi in [(2, 3, 8), (3, 2, 6), (5, 2, 7)]:
-        w = synth.scaled(synth.WORKLOADS[idx], ndm=512)
-        mean, mx = dd.dd_pattern_stats(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list, 4, 64)
-        assert lo <= mean <= hi and mx <= 12, (idx, mean, mx)
