@@ -1,20 +1,26 @@
 #!/usr/bin/env python
 """Benchmark of the direct-dedispersion hot path on B200 (contract: see DESIGN.md "Measurement").
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
 
-A step = one pass of the whole hot path (delay table already in the plan; staging, unpack,
-accumulation, store — one dd_execute) over one synthetic filterbank of BASELINE.json's
-configs[1] (uint8, 1024 channels x 1024 DM trials x 2^17 samples) resident in HBM.  Prints ONE
-JSON line.  `--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same
-workload instead.  Under torchrun every rank dedisperses its own beam (independent seeds, no
-data-path collective): weak scaling.
+A step = one pass of the whole hot path (delay table already in the plan; front end, staging,
+unpack, accumulation, store -- one dd_execute, or the four dd_stream_push calls of config 5) over
+one synthetic filterbank resident in HBM.  The headline workload is the largest single-GPU
+configuration of BASELINE.json: configs[2] (float32, 4096 channels x 4096 DM trials x 2^18
+samples, 4.4e12 adds).  The other four configs are timed in the same process and reported under
+`per_config`.  Prints ONE JSON line.  `--impl reference` times the CPU oracle (oracle/) on a
+bounded sample of the same workload instead.
+
+Multi-GPU: the path shards by beam with no exchange step.  Under torchrun (RANK / WORLD_SIZE in
+the environment) every rank dedisperses its own beam; `python bench.py --gpus N` without torchrun
+spawns the N ranks itself.  Weak scaling; the only collective is the max-reduction of the timings.
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import socket
 import sys
 import threading
 import time
@@ -29,6 +35,10 @@ from paper_1401_8258_b200 import sharding, synth  # noqa: E402
 METRIC = "dedispersed DM·channel·samples/s"
 UNIT = "G/s"
 SM_COUNT, LANES_PER_SM = 148, 128          # FP32/INT32 add lanes per SM
+# measured add lanes per clock per SM of the instruction each path accumulates with (dependent-chain
+# microbenchmark, profiles/r1_pipe_rates.txt: FADD 3.868 and IADD3 3.852 warp-instructions/clk/SM)
+MEASURED_LANES = {"f32": 123.8, "u8": 123.2}
+HEADLINE = 3
 
 
 def _env_int(name, default):
@@ -98,23 +108,29 @@ def visible_gpu_index(local_rank):
 
 # ----------------------------------------------------------------------------- CPU oracle legs
 
-def oracle_sample(w, seconds_target=12.0):
+def _oracle_fn(w):
+    import oracle
+    return oracle.dedisperse_f32 if w.dtype == "f32" else oracle.dedisperse_u8
+
+
+def oracle_sample(w, seconds_target=10.0):
     """Times oracle/ (as it stands) on a bounded sample of workload w: a subset of DM rows over a
-    shortened time range of the same filterbank.  Returns (G/s, cores, description)."""
+    shortened time range of the same filterbank.  Returns a dict with the all-core literal-nest rate
+    (the cpu_baseline value), the single-core rate and the interchanged-nest rate."""
     import oracle
     cores = oracle.num_threads()
     ms = oracle.max_shift(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
     nsamp = min(w.nsamp, 1 << 15)
     X = synth.make_input(w, nsamp + ms)
+    f = _oracle_fn(w)
     nrows = max(cores, 8)
     rows = np.unique(np.linspace(0, w.ndm - 1, nrows).astype(np.int32))
-    f = oracle.dedisperse_f32 if w.dtype == "f32" else oracle.dedisperse_u8
     f(X, 256, w.fch1, w.foff, w.tsamp, w.dm_list, rows=rows[:cores])           # warm caches / threads
     t0 = time.perf_counter()
     f(X, nsamp, w.fch1, w.foff, w.tsamp, w.dm_list, rows=rows)
     dt = time.perf_counter() - t0
     # grow the sample towards the time target (once), keeping the run bounded
-    grow = int(min(8, seconds_target / max(dt, 1e-3)))
+    grow = int(min(16, seconds_target / max(dt, 1e-3)))
     if grow >= 2:
         rows = np.unique(np.linspace(0, w.ndm - 1, nrows * grow).astype(np.int32))
         t0 = time.perf_counter()
@@ -123,16 +139,30 @@ def oracle_sample(w, seconds_target=12.0):
     adds = len(rows) * w.nchans * nsamp
     desc = "%d of %d DM rows x %d of %d samples x %d channels, literal (d,t,c) nest" % (
         len(rows), w.ndm, nsamp, w.nsamp, w.nchans)
-    return adds / dt / 1e9, cores, desc, dt, (X, nsamp, rows)
+    out = {"value": adds / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+           "seconds": dt, "_replay": (X, nsamp, rows)}
+    # the same rows through the interchanged (d,c,t) nest (bit-identical results, vectorisable inner loop)
+    t0 = time.perf_counter()
+    f(X, nsamp, w.fch1, w.foff, w.tsamp, w.dm_list, rows=rows, interchanged=True)
+    out["interchanged_nest"] = {"value": adds / (time.perf_counter() - t0) / 1e9, "unit": UNIT, "cores": cores}
+    # one core: a single row (the OpenMP loop runs over rows, so one row = one thread)
+    one = rows[len(rows) // 2: len(rows) // 2 + 1]
+    t0 = time.perf_counter()
+    f(X, nsamp, w.fch1, w.foff, w.tsamp, w.dm_list, rows=one)
+    out["single_core"] = {"value": w.nchans * nsamp / (time.perf_counter() - t0) / 1e9, "unit": UNIT, "cores": 1,
+                          "sample": "one DM row x %d samples x %d channels, literal nest" % (nsamp, w.nchans)}
+    full = w.adds / (out["value"] * 1e9)
+    out["extrapolated_full_workload_s"] = full
+    return out
 
 
 def run_reference(args, w):
     rank = _env_int("RANK", 0)
     if rank != 0:
         return
-    import oracle
-    gps, cores, desc, dt, (X, nsamp, rows) = oracle_sample(w, seconds_target=6.0)
-    f = oracle.dedisperse_f32 if w.dtype == "f32" else oracle.dedisperse_u8
+    smp = oracle_sample(w, seconds_target=6.0)
+    X, nsamp, rows = smp.pop("_replay")
+    f = _oracle_fn(w)
     steps = max(1, min(args.steps, 5))
     for _ in range(min(args.warmup, 1)):
         f(X, nsamp, w.fch1, w.foff, w.tsamp, w.dm_list, rows=rows)
@@ -141,12 +171,13 @@ def run_reference(args, w):
         f(X, nsamp, w.fch1, w.foff, w.tsamp, w.dm_list, rows=rows)
     dt = (time.perf_counter() - t0) / steps
     val = len(rows) * w.nchans * nsamp / dt / 1e9
+    smp["value"] = val
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": steps, "warmup": min(args.warmup, 1), "ms_per_step": dt * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "sample": desc},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "config": {"workload": w.name, "sample": smp["sample"]},
+        "cpu_baseline": smp,
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -154,6 +185,148 @@ def run_reference(args, w):
 
 
 # ----------------------------------------------------------------------------- GPU leg
+
+class Case:
+    """One workload resident on the device: plan, X, D and the step function bench.py times."""
+
+    def __init__(self, dd, torch, w, rank=0, world=1, kernel=None, host_input=False):
+        self.dd, self.torch, self.w = dd, torch, w
+        dtype = dd.DD_F32 if w.dtype == "f32" else dd.DD_U8
+        self.tdt = torch.float32 if w.dtype == "f32" else torch.uint8
+        self.odt = torch.float32 if w.dtype == "f32" else torch.int32
+        self.es = 4 if w.dtype == "f32" else 1
+        self.plan = dd.Plan(dtype, w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+        if kernel:
+            self.plan.set_kernel({"generic": dd.DD_KERNEL_GENERIC, "ps": dd.DD_KERNEL_PS}[kernel])
+        self.ms = ms = self.plan.max_shift()
+        nb = self.nb = w.nbeams
+        self.in_stride = (w.nsamp + ms + 63) // 64 * 64
+        self.out_stride = w.nsamp
+        self.Xh = None
+        if host_input:
+            # pinned host input, one beam per rank-beam (rank r uses beam seeds r*nb .. r*nb+nb-1), generated
+            # by synth (numpy Philox) exactly as the parity tests generate it
+            self.Xh = torch.empty((nb, w.nchans, self.in_stride), dtype=self.tdt).pin_memory()
+            self.Xh.zero_()
+            wb = synth.scaled(w, nbeams=max(2, nb * world))           # per-beam seeds
+            for b, beam in enumerate(sharding.beams_of_rank(rank, world, nb)):
+                synth.make_input(wb, w.nsamp + ms, beam=beam, out=self.Xh[b, :, :w.nsamp + ms].numpy())
+            self.Xd = self.Xh.cuda()
+        else:
+            # same distributions drawn on the device (seeded); control flow is data-independent
+            g = torch.Generator(device="cuda").manual_seed(w.seed + 7919 * rank)
+            if w.dtype == "f32":
+                self.Xd = torch.randn((nb, w.nchans, self.in_stride), dtype=torch.float32, device="cuda", generator=g)
+            else:
+                z = torch.randn((nb, w.nchans, self.in_stride), dtype=torch.float32, device="cuda", generator=g)
+                self.Xd = z.mul_(16.0).add_(128.0).round_().clamp_(0, 255).to(torch.uint8)
+                del z
+        self.Dd = torch.empty((nb, w.ndm, self.out_stride), dtype=self.odt, device="cuda")
+        self.stream = torch.cuda.Stream()
+        a = (self.Xd, self.in_stride, w.nchans * self.in_stride, self.Dd, self.out_stride, w.ndm * self.out_stride)
+        self.kern = self.plan.kernel_for(*a, w.nsamp, nb)
+        self.streamer = None
+        if w.nchunks > 1:
+            # config 5: fed through the streaming API: first push nsamp/nchunks + maxshift, then equal chunks
+            self.chunk = w.nsamp // w.nchunks
+            self.streamer = dd.Stream(self.plan, self.chunk + ms, nb)
+            # per push: the append and carry copies (2 strided device copies) + the kernels of one dd_execute
+            per_push = 2 + self.plan.launches_for(self.Xd, self.ms + self.chunk + 64, 0, self.Dd, self.out_stride,
+                                                  w.ndm * self.out_stride, self.chunk, nb)
+            self.launches = w.nchunks * per_push
+        else:
+            self.launches = self.plan.launches_for(*a, w.nsamp, nb)
+        self.hbm_bytes = nb * (w.nchans * (w.nsamp + ms) * self.es + w.ndm * w.nsamp * 4)
+
+    def step(self):
+        w, nb = self.w, self.nb
+        if self.streamer is None:
+            self.plan.execute(self.Xd, self.in_stride, w.nchans * self.in_stride, self.Dd, self.out_stride,
+                              w.ndm * self.out_stride, w.nsamp, nb, self.stream)
+            return
+        self.streamer.reset()
+        pos = emitted = 0
+        for k in range(w.nchunks):
+            n_new = self.chunk + (self.ms if k == 0 else 0)
+            n = self.streamer.push(self.Xd[:, :, pos:], self.in_stride, w.nchans * self.in_stride, n_new,
+                                   self.Dd[:, :, emitted:], self.out_stride, w.ndm * self.out_stride, self.stream)
+            pos += n_new
+            emitted += n
+        assert emitted == w.nsamp
+
+    def timed(self, steps, warmup, barrier, gpu_index):
+        """W warm-up steps, then K steps between CUDA events on the launching stream; returns
+        (per-step ms list, total ms, clocks)."""
+        torch = self.torch
+        with torch.cuda.stream(self.stream):
+            for _ in range(warmup):
+                self.step()
+        barrier()
+        sampler = ClockSampler(gpu_index)
+        sampler.start()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+        with torch.cuda.stream(self.stream):
+            ev[0].record(self.stream)
+            for i in range(steps):
+                self.step()
+                ev[i + 1].record(self.stream)
+        barrier()
+        clocks = sampler.result()
+        per_step = [ev[i].elapsed_time(ev[i + 1]) for i in range(steps)]
+        return per_step, ev[0].elapsed_time(ev[-1]), clocks
+
+    def close(self):
+        if self.streamer is not None:
+            self.streamer.destroy()
+        self.plan.destroy()
+        self.Xd = self.Dd = self.Xh = None
+        self.torch.cuda.empty_cache()
+
+
+def counters_for(workload, kern):
+    """Counters of the dominant kernel from the tracked ncu summaries (profiles/kernel_counters.txt): DRAM
+    traffic per launch, issue-slot and LSU utilisation, issued add instructions / algorithmic adds, each
+    with the commit of the capture so that staleness is visible."""
+    out = None
+    try:
+        for ln in open(os.path.join(ROOT, "profiles", "kernel_counters.txt")):
+            f = ln.split()
+            if len(f) >= 8 and not ln.startswith("#") and f[0] == workload and f[1] == str(kern):
+                num = lambda v: None if v == "na" else float(v)
+                out = {"traffic": num(f[2]), "issue_active": num(f[3]), "lsu_wavefront_frac": num(f[4]),
+                       "issued_add_frac": num(f[5]), "captured_at_commit": f[6], "source": "profiles/" + f[7]}
+    except OSError:
+        pass
+    return out
+
+
+def kernel_name(kern):
+    return {1: "generic", 2: "ps"}.get(kern, str(kern))
+
+
+def roofline_of(w, case, kernel_ms, clocks):
+    peak_max = SM_COUNT * LANES_PER_SM * (clocks["sm_max_mhz"] or 1965) * 1e6 / 1e12
+    achieved = w.adds / (kernel_ms * 1e-3) / 1e12
+    clk = clocks["sm_mhz"] or clocks["sm_max_mhz"] or 1965
+    peak_meas = SM_COUNT * MEASURED_LANES[w.dtype] * clk * 1e6 / 1e12
+    r = {"bound": "alu", "achieved": achieved, "peak": peak_max, "unit": "Tadd/s", "frac": achieved / peak_max,
+         "traffic": None,
+         "peak_note": "148 SM x 128 add lanes x sm_max_mhz (nominal; DESIGN.md 5)",
+         "kernel_ms": kernel_ms,
+         "frac_at_sampled_clock": achieved / (SM_COUNT * LANES_PER_SM * clk * 1e6 / 1e12),
+         "peak_measured": peak_meas, "frac_measured": achieved / peak_meas,
+         "peak_measured_note": "148 SM x %.1f lanes/clk/SM (%s dependent-chain microbenchmark, "
+                               "profiles/r1_pipe_rates.txt) x sampled SM clock" % (
+                                   MEASURED_LANES[w.dtype], "FADD" if w.dtype == "f32" else "IADD3"),
+         "algorithmic_adds_per_launch": w.adds,
+         "hbm_algorithmic_bytes": case.hbm_bytes,
+         "hbm_achieved_gbs": case.hbm_bytes / (kernel_ms * 1e-3) / 1e9}
+    c = counters_for(w.name, case.kern)
+    if c:
+        r["traffic"] = c.pop("traffic")
+        r["ncu"] = c
+    return r
+
 
 def run_ours(args, w):
     import torch
@@ -165,169 +338,166 @@ def run_ours(args, w):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-
-    dtype = dd.DD_F32 if w.dtype == "f32" else dd.DD_U8
-    tdt = torch.float32 if w.dtype == "f32" else torch.uint8
-    odt = torch.float32 if w.dtype == "f32" else torch.int32
-    plan = dd.Plan(dtype, w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
-    if args.kernel:
-        plan.set_kernel({"generic": dd.DD_KERNEL_GENERIC, "tma": dd.DD_KERNEL_TMA, "ps": dd.DD_KERNEL_PS}[args.kernel])
-    ms = plan.max_shift()
-    nb = w.nbeams
-    in_stride = (w.nsamp + ms + 63) // 64 * 64
-    out_stride = w.nsamp
-
-    # host input: pinned, one beam per rank-beam (rank r uses beam seeds r*nb .. r*nb+nb-1)
-    Xh = torch.empty((nb, w.nchans, in_stride), dtype=tdt).pin_memory()
-    Xh.zero_()
-    wb = synth.scaled(w, nbeams=max(2, nb * world))           # per-beam seeds
-    for b, beam in enumerate(sharding.beams_of_rank(rank, world, nb)):
-        Xh[b, :, :w.nsamp + ms] = torch.from_numpy(synth.make_input(wb, w.nsamp + ms, beam=beam))
-    Xd = Xh.cuda()
-    Dd = torch.empty((nb, w.ndm, out_stride), dtype=odt, device="cuda")
-    stream = torch.cuda.Stream()
-    kern = plan.kernel_for(Xd, in_stride, w.nchans * in_stride, Dd, out_stride, w.ndm * out_stride, w.nsamp, nb)
-
-    lpe = plan.launches_per_execute()          # kernels per dd_execute (front end + main kernel)
-    streamer = None
-    if w.nchunks > 1:
-        # config 5: fed through the streaming API: first push nsamp/nchunks + maxshift, then equal chunks
-        chunk = w.nsamp // w.nchunks
-        streamer = dd.Stream(plan, chunk + ms, nb)
-
-    def step():
-        if streamer is None:
-            plan.execute(Xd, in_stride, w.nchans * in_stride, Dd, out_stride, w.ndm * out_stride,
-                         w.nsamp, nb, stream)
-            return lpe
-        streamer.reset()
-        pos = emitted = 0
-        chunk = w.nsamp // w.nchunks
-        for k in range(w.nchunks):
-            n_new = chunk + (ms if k == 0 else 0)
-            n = streamer.push(Xd[:, :, pos:], in_stride, w.nchans * in_stride, n_new,
-                              Dd[:, :, emitted:], out_stride, w.ndm * out_stride, stream)
-            pos += n_new
-            emitted += n
-        assert emitted == w.nsamp
-        return w.nchunks * lpe
+    gpu_index = visible_gpu_index(local)
 
     def barrier():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    launches = 0
-    with torch.cuda.stream(stream):
-        for _ in range(args.warmup):
-            step()
-    barrier()
-    sampler = ClockSampler(visible_gpu_index(local))
-    sampler.start()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    with torch.cuda.stream(stream):
-        ev[0].record(stream)
-        for i in range(args.steps):
-            launches += step()
-            ev[i + 1].record(stream)
-    barrier()
-    clocks = sampler.result()
-    total_ms = ev[0].elapsed_time(ev[-1])
-    per_step = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
-    total_ms = sharding.max_over_ranks(total_ms, dist, "cuda")
-    ms_per_step = total_ms / args.steps
-    adds_rank = w.adds
-    value = sharding.whole_job_rate(adds_rank, world, ms_per_step * 1e-3) / 1e9
+    case = Case(dd, torch, w, rank, world, args.kernel, host_input=True)
+    per_step, total_ms, clocks = case.timed(args.steps, args.warmup, barrier, gpu_index)
+    ms_per_step, value = finish_timing(total_ms, args.steps, w.adds, world, dist, "cuda")
 
     # ---- end to end through the host-buffer C-ABI call (pinned host X and D; copies inside)
     e2e = None
-    if nb == 1 and streamer is None:
-        Dh = torch.empty((w.ndm, out_stride), dtype=odt).pin_memory()
-        plan.execute_host(Xh[0], in_stride, Dh, out_stride, w.nsamp)          # warm-up (allocates workspace)
-        plan.execute_host(Xh[0], in_stride, Dh, out_stride, w.nsamp)
-        n_e2e = max(3, min(args.steps, 10))
+    if case.streamer is None:
+        nb = w.nbeams
+        Dh = torch.empty((nb, w.ndm, case.out_stride), dtype=case.odt).pin_memory()
+        a = (case.Xh, case.in_stride, w.nchans * case.in_stride, Dh, case.out_stride, w.ndm * case.out_stride,
+             w.nsamp, nb)
+        case.plan.execute_host(*a)                                   # warm-up (allocates the cached device buffers)
+        n_e2e = max(3, min(args.steps, 5))
         barrier()
         t0 = time.perf_counter()
         for _ in range(n_e2e):
-            plan.execute_host(Xh[0], in_stride, Dh, out_stride, w.nsamp)
+            case.plan.execute_host(*a)
         torch.cuda.synchronize()
         dt = (time.perf_counter() - t0) / n_e2e
         dt = sharding.max_over_ranks(dt, dist, "cuda")
-        es = 4 if w.dtype == "f32" else 1
-        e2e = {"value": sharding.whole_job_rate(adds_rank, world, dt) / 1e9, "unit": UNIT,
-               "h2d_bytes_per_step": int(w.nchans * (w.nsamp + ms) * es),
-               "d2h_bytes_per_step": int(w.ndm * w.nsamp * 4), "ms_per_step": dt * 1e3,
+        e2e = {"value": sharding.whole_job_rate(w.adds, world, dt) / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": int(nb * w.nchans * (w.nsamp + case.ms) * case.es),
+               "d2h_bytes_per_step": int(nb * w.ndm * w.nsamp * 4), "ms_per_step": dt * 1e3,
                "timer": "host wall clock around the synchronous dd_execute_host call, pinned buffers"}
-        # the host path must give the same bits as the resident path
-        same = bool(torch.equal(Dh[:, :w.nsamp].cuda(), Dd[0][:, :w.nsamp]))
+        # the host path must give the same bits as the resident path (compared slice by slice on the device)
+        same = True
+        for b in range(nb):
+            for r0 in range(0, w.ndm, 512):
+                same = same and bool(torch.equal(Dh[b, r0:r0 + 512].cuda(), case.Dd[b, r0:r0 + 512]))
         e2e["matches_resident_result"] = same
+        del Dh
 
+    line = None
     if rank == 0:
-        peak_max = SM_COUNT * LANES_PER_SM * (clocks["sm_max_mhz"] or 1965) * 1e6 / 1e12
         kernel_ms = float(np.mean(per_step))
-        achieved = adds_rank / (kernel_ms * 1e-3) / 1e12
-        hbm_bytes = nb * (w.nchans * (w.nsamp + ms) * (4 if w.dtype == "f32" else 1) + w.ndm * w.nsamp * 4)
-        hbm_peak = None
-        try:
-            hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs")
-        except (OSError, ValueError):
-            pass
-        traffic = None
-        try:
-            for ln in open(os.path.join(ROOT, "profiles", "dram_traffic.txt")):
-                f = ln.split()
-                if len(f) >= 3 and not ln.startswith("#") and f[0] == w.name and f[1] == str(kern):
-                    traffic = float(f[2])
-        except OSError:
-            pass
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "int32" if w.dtype == "u8" else "f32",
             "data": "synthetic",
-            "config": {"workload": w.name, "nbeams": nb, "nchans": w.nchans, "ndm": w.ndm,
-                       "nsamp": w.nsamp, "maxshift": ms, "tsamp": w.tsamp, "fch1": w.fch1, "foff": w.foff,
-                       "kernel": {1: "generic", 2: "tma", 3: "ps"}.get(kern, str(kern)),
+            "config": {"workload": w.name, "nbeams": w.nbeams, "nchans": w.nchans, "ndm": w.ndm,
+                       "nsamp": w.nsamp, "maxshift": case.ms, "tsamp": w.tsamp, "fch1": w.fch1, "foff": w.foff,
+                       "kernel": kernel_name(case.kern), "plan": case.plan.describe(),
                        "parallelism": "beam-per-rank" if world > 1 else "single",
-                       "l2": "X+D per step = %.0f MB > 126 MB L2 (no flush needed)" % (hbm_bytes / 1e6)},
+                       "l2": "X+D per step = %.0f MB > 126 MB L2 (no flush needed)" % (case.hbm_bytes / 1e6)
+                             if case.hbm_bytes > 200e6 else "L2 flushed between steps: no (working set fits L2; "
+                             "the step is launch-bound)"},
             "real_time_factor": w.nsamp * w.tsamp / (ms_per_step * 1e-3),
-            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_max, "unit": "Tadd/s",
-                         "frac": achieved / peak_max, "traffic": traffic,
-                         "peak_note": "148 SM x 128 add lanes x sm_max_mhz (nominal; DESIGN.md)",
-                         "kernel_ms": kernel_ms,
-                         "frac_at_sampled_clock": (achieved / (SM_COUNT * LANES_PER_SM * clocks["sm_mhz"] * 1e6 / 1e12)
-                                                   if clocks["sm_mhz"] else None),
-                         "algorithmic_adds_per_launch": adds_rank,
-                         "work_note": ("achieved = nbeams*nchans*ndm*nsamp adds (one per DM-channel-sample, SURVEY "
-                                       "8(d)) / CUDA-event time of the step; the ps kernels form each output from the "
-                                       "same operands but share partial sums of 4-8 channels between trials "
-                                       "(DESIGN.md 5.3), so fewer add instructions are issued"),
-                         "hbm_algorithmic_bytes": hbm_bytes,
-                         "hbm_achieved_gbs": hbm_bytes / (kernel_ms * 1e-3) / 1e9,
-                         "hbm_peak_gbs_measured": hbm_peak},
-            "clocks": clocks, "gpu_launches": launches,
+            "roofline": roofline_of(w, case, kernel_ms, clocks),
+            "clocks": clocks, "gpu_launches": case.launches * args.steps,
         }
+        line["roofline"]["work_note"] = (
+            "achieved = nbeams*nchans*ndm*nsamp adds (one per DM-channel-sample, SURVEY 8(d)) / CUDA-event time of "
+            "the step; an EFFECTIVE rate: the ps kernels form each output from the same operands but share partial "
+            "sums of 4-8 channels between trials (DESIGN.md 5.3), so fewer add instructions are issued "
+            "(ncu.issued_add_frac) and the binding unit is shared-memory bandwidth (ncu.lsu_wavefront_frac)")
         if e2e is not None:
             line["e2e"] = e2e
-        if not args.no_cpu and world >= 1:
-            gps, cores, desc, dt, _ = oracle_sample(w)
-            line["cpu_baseline"] = {"value": gps, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                    "sample": desc, "seconds": dt}
+    case.close()
+
+    # ---- the other BASELINE.json configs, same process (single GPU only)
+    if rank == 0 and world == 1 and not args.no_per_config and not args.nsamp:
+        per = {}
+        for idx in sorted(synth.WORKLOADS):
+            if idx == w.index:
+                continue
+            wi = synth.WORKLOADS[idx]
+            c = Case(dd, torch, wi, 0, 1, args.kernel, host_input=False)
+            # tiny steps need more repetitions for a stable mean
+            k = args.steps if wi.adds > 1e10 else max(args.steps, 200)
+            ps, tot, clk = c.timed(min(k, max(3, int(3000 / max(1.0, wi.adds / 25e9)))), 3, barrier, gpu_index)
+            ms_i = tot / len(ps)
+            rf = roofline_of(wi, c, ms_i, clk)
+            per["cfg%d" % idx] = {
+                "workload": wi.name, "ms_per_step": ms_i, "steps": len(ps), "value": wi.adds / (ms_i * 1e-3) / 1e9,
+                "frac": rf["frac"], "frac_measured": rf["frac_measured"], "kernel": kernel_name(c.kern),
+                "plan": c.plan.describe(), "real_time_factor": wi.nsamp * wi.tsamp / (ms_i * 1e-3),
+                "gpu_launches_per_step": c.launches, "clocks": clk, "traffic": rf["traffic"],
+                "data": "synthetic, drawn on the device (seeded)"}
+            if wi.adds < 1e9:
+                per["cfg%d" % idx]["note"] = ("launch-bound: %.2f us of adds at the roofline; empty-kernel launch "
+                                              "measured beside it" % (wi.adds / 37.2e12 * 1e6))
+                per["cfg%d" % idx]["empty_launch_us"] = empty_launch_us(torch)
+            c.close()
+        line["per_config"] = per
+
+    if rank == 0:
+        if not args.no_cpu:
+            smp = oracle_sample(w)
+            smp.pop("_replay")
+            line["cpu_baseline"] = smp
         print(json.dumps(line))
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
 
 
+def finish_timing(total_ms, steps, units_per_rank, world, dist, device):
+    """Max over ranks of the device-timed region -> (ms per step, whole-job G units/s): every rank processed
+    units_per_rank per step (weak scaling, no data-path collective)."""
+    total_ms = sharding.max_over_ranks(total_ms, dist, device)
+    ms_per_step = total_ms / steps
+    return ms_per_step, sharding.whole_job_rate(units_per_rank, world, ms_per_step * 1e-3) / 1e9
+
+
+def empty_launch_us(torch, n=200):
+    """Back-to-back launches of a trivial torch kernel on one stream (device time per launch): the floor
+    under any single-kernel step."""
+    x = torch.zeros(32, device="cuda")
+    for _ in range(20):
+        x.add_(1.0)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(n):
+        x.add_(1.0)
+    b.record()
+    torch.cuda.synchronize()
+    return a.elapsed_time(b) / n * 1e3
+
+
+def _rank_entry(local_rank, world, port, target, extra):
+    os.environ.update({"RANK": str(local_rank), "LOCAL_RANK": str(local_rank), "WORLD_SIZE": str(world),
+                       "MASTER_ADDR": "127.0.0.1", "MASTER_PORT": str(port)})
+    target(*extra)
+
+
+def launch_ranks(world, target, extra=()):
+    """`python bench.py --gpus N` without torchrun: one process per GPU on this node, rendezvous on
+    127.0.0.1 (the same environment torchrun would set)."""
+    import torch.multiprocessing as mp
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    mp.spawn(_rank_entry, args=(world, port, target, tuple(extra)), nprocs=world, join=True)
+
+
+def _main_with_argv(argv):
+    sys.argv = list(argv)
+    main()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=30)
-    ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); default 2 = configs[1]")
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=HEADLINE,
+                    help="BASELINE.json config number (1-5); default 3 = configs[2], the largest single-GPU shape")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--kernel", default=None, choices=["generic", "tma", "ps"])
+    ap.add_argument("--kernel", default=None, choices=["generic", "ps"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config legs (profiling aid)")
     ap.add_argument("--nsamp", type=int, default=0,
                     help="profiling aid: cut the workload to this many output samples (the line then names it)")
     args = ap.parse_args()
@@ -337,8 +507,17 @@ def main():
         w = synth.scaled(w, nsamp=args.nsamp, name="%s_cut_to_%d_samples" % (w.name, args.nsamp))
     if args.impl == "reference":
         run_reference(args, w)
-    else:
-        run_ours(args, w)
+        return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # the contract command without torchrun: start the N ranks here, one device each
+        import torch
+        have = torch.cuda.device_count()
+        if have < args.gpus:
+            print(json.dumps({"error": "--gpus %d but only %d CUDA devices are visible" % (args.gpus, have)}))
+            sys.exit(1)
+        launch_ranks(args.gpus, _main_with_argv, (list(sys.argv),))
+        return
+    run_ours(args, w)
 
 
 if __name__ == "__main__":

@@ -58,6 +58,10 @@ def _load():
     lib.oracle_dedisperse_u8.restype = None
     lib.oracle_dedisperse_u8.argtypes = [C.c_void_p, C.c_int, C.c_int64, C.c_int64, C.c_double,
                                          C.c_double, C.c_double, dp, C.c_int, ip, C.c_int, lp]
+    lib.oracle_dedisperse_f32_dct.restype = None
+    lib.oracle_dedisperse_f32_dct.argtypes = lib.oracle_dedisperse_f32.argtypes
+    lib.oracle_dedisperse_u8_dct.restype = None
+    lib.oracle_dedisperse_u8_dct.argtypes = lib.oracle_dedisperse_u8.argtypes
     lib.oracle_elements_f32.restype = None
     lib.oracle_elements_f32.argtypes = [C.c_void_p, C.c_int, C.c_int64, C.c_double, C.c_double,
                                         C.c_double, dp, ip, lp, C.c_int64, dp, dp]
@@ -109,10 +113,11 @@ def _check_X(X, dtype, nsamp, maxshift):
     return X
 
 
-def dedisperse_f32(X, nsamp, fch1, foff, tsamp, dm_list, rows=None):
+def dedisperse_f32(X, nsamp, fch1, foff, tsamp, dm_list, rows=None, interchanged=False):
     """X float32 [nchans][>= nsamp+maxshift] -> (D, A) float64 [nrows][nsamp].
 
     D = eq 2.1 sums in double; A = sum_c |X| (scale of the float tolerance).
+    interchanged=True runs the (d, c, t) nest (bit-identical results, see dedisp_oracle.cpp).
     """
     dms = _dms(dm_list)
     nchans = X.shape[0]
@@ -121,13 +126,13 @@ def dedisperse_f32(X, nsamp, fch1, foff, tsamp, dm_list, rows=None):
     nr = len(dms) if rws is None else len(rws)
     D = np.empty((nr, nsamp), dtype=np.float64)
     A = np.empty((nr, nsamp), dtype=np.float64)
-    _load().oracle_dedisperse_f32(X.ctypes.data, nchans, nsamp, X.shape[1], fch1, foff, tsamp,
-                                  _dp(dms), len(dms), None if rws is None else _ip(rws), nr,
-                                  _dp(D), _dp(A))
+    f = _load().oracle_dedisperse_f32_dct if interchanged else _load().oracle_dedisperse_f32
+    f(X.ctypes.data, nchans, nsamp, X.shape[1], fch1, foff, tsamp,
+      _dp(dms), len(dms), None if rws is None else _ip(rws), nr, _dp(D), _dp(A))
     return D, A
 
 
-def dedisperse_u8(X, nsamp, fch1, foff, tsamp, dm_list, rows=None):
+def dedisperse_u8(X, nsamp, fch1, foff, tsamp, dm_list, rows=None, interchanged=False):
     """X uint8 [nchans][>= nsamp+maxshift] -> D int64 [nrows][nsamp] (exact)."""
     dms = _dms(dm_list)
     nchans = X.shape[0]
@@ -135,8 +140,9 @@ def dedisperse_u8(X, nsamp, fch1, foff, tsamp, dm_list, rows=None):
     rws = None if rows is None else np.ascontiguousarray(np.asarray(rows, dtype=np.int32))
     nr = len(dms) if rws is None else len(rws)
     D = np.empty((nr, nsamp), dtype=np.int64)
-    _load().oracle_dedisperse_u8(X.ctypes.data, nchans, nsamp, X.shape[1], fch1, foff, tsamp,
-                                 _dp(dms), len(dms), None if rws is None else _ip(rws), nr, _lp(D))
+    f = _load().oracle_dedisperse_u8_dct if interchanged else _load().oracle_dedisperse_u8
+    f(X.ctypes.data, nchans, nsamp, X.shape[1], fch1, foff, tsamp,
+      _dp(dms), len(dms), None if rws is None else _ip(rws), nr, _lp(D))
     return D
 
 

@@ -83,26 +83,67 @@ def assert_sampled_parity(w, X, D_gpu, n=200000, seed=0):
         assert np.all(err <= F32_RTOL * A), (err / (F32_RTOL * A)).max()
 
 
-def assert_row_checksums(w, X, D_gpu, table):
-    """P7: sum_t D[d][t] = sum_c (P_c[nsamp + s(d,c)] - P_c[s(d,c)]) for EVERY trial d, with
-    P_c the prefix sum of channel row c.  `table` is the ORACLE's delay table."""
-    nch = w.nchans
+def row_checksums(w, X, table):
+    """P7 (SURVEY 8(c)): sum_t D[d][t] = sum_c (P_c[nsamp + s(d,c)] - P_c[s(d,c)]) for EVERY trial d, with
+    P_c the prefix sum of channel row c -- O(nchans * (ndm + nsamp)), one channel in memory at a time.
+    `table` is the ORACLE's delay table.  Returns (want, scale): exact int64 sums for uint8; for float32
+    double sums and sum_t of the per-element tolerance scale sum_c |X|."""
+    table = np.asarray(table)
+    n = w.nsamp
     if w.dtype == "u8":
-        P = np.zeros((nch, X.shape[1] + 1), dtype=np.int64)
-        np.cumsum(X, axis=1, dtype=np.int64, out=P[:, 1:])
         want = np.zeros(len(table), dtype=np.int64)
-        for c in range(nch):
-            want += P[c, w.nsamp + table[:, c]] - P[c, table[:, c]]
-        got = D_gpu.sum(axis=1, dtype=np.int64)
-        assert np.array_equal(got, want)
+        p = np.zeros(X.shape[1] + 1, dtype=np.int64)
+        for c in range(w.nchans):
+            np.cumsum(X[c], dtype=np.int64, out=p[1:])
+            want += p[n + table[:, c]] - p[table[:, c]]
+        return want, None
+    want = np.zeros(len(table))
+    scale = np.zeros(len(table))
+    p = np.zeros(X.shape[1] + 1, dtype=np.float64)
+    for c in range(w.nchans):
+        np.cumsum(X[c], dtype=np.float64, out=p[1:])
+        want += p[n + table[:, c]] - p[table[:, c]]
+        np.cumsum(np.abs(X[c]), dtype=np.float64, out=p[1:])
+        scale += p[n + table[:, c]] - p[table[:, c]]
+    return want, scale
+
+
+def assert_row_checksums(w, X, D_gpu, table):
+    """P7 on a result held as numpy ([ndm][nsamp]) or as a torch tensor on the device (the row sums are
+    then formed there in int64 / float64 -- a reduction by the checker, not by the product)."""
+    want, scale = row_checksums(w, X, table)
+    if isinstance(D_gpu, np.ndarray):
+        got = D_gpu.sum(axis=1, dtype=np.int64 if w.dtype == "u8" else np.float64)
     else:
-        P = np.zeros((nch, X.shape[1] + 1), dtype=np.float64)
-        np.cumsum(X, axis=1, dtype=np.float64, out=P[:, 1:])
-        PA = np.zeros((nch, X.shape[1] + 1), dtype=np.float64)
-        np.cumsum(np.abs(X), axis=1, dtype=np.float64, out=PA[:, 1:])
-        want = np.zeros(len(table)); scale = np.zeros(len(table))
-        for c in range(nch):
-            want += P[c, w.nsamp + table[:, c]] - P[c, table[:, c]]
-            scale += PA[c, w.nsamp + table[:, c]] - PA[c, table[:, c]]
-        got = D_gpu.sum(axis=1, dtype=np.float64)
-        assert np.all(np.abs(got - want) <= F32_RTOL * scale + 1e-6 * np.abs(want))
+        import torch
+        got = D_gpu.sum(dim=1, dtype=torch.int64 if w.dtype == "u8" else torch.float64).cpu().numpy()
+    if w.dtype == "u8":
+        assert np.array_equal(got, want), np.argwhere(got != want)[:5].tolist()
+    else:
+        # sum of the per-element tolerances, plus the rounding of the prefix-sum differences themselves
+        tol = F32_RTOL * scale + 1e-9 * scale
+        bad = np.abs(got - want) > tol
+        assert not bad.any(), (np.argwhere(bad)[:5].tolist(), (np.abs(got - want) / tol).max())
+
+
+def assert_whole_rows(w, X, D_rows_gpu, rows, dms=None):
+    """P8: whole oracle rows (all nsamp samples) for the trials in `rows`; D_rows_gpu[i] is the product's
+    row for trial rows[i] (numpy).  The oracle runs its interchanged nest (pinned bit-identical to the
+    literal one in tests/test_oracle_pins.py)."""
+    dms = w.dm_list if dms is None else dms
+    rows = np.asarray(rows, dtype=np.int32)
+    if w.dtype == "u8":
+        want = oracle.dedisperse_u8(X, w.nsamp, w.fch1, w.foff, w.tsamp, dms, rows=rows, interchanged=True)
+        assert np.array_equal(D_rows_gpu.astype(np.int64), want), np.argwhere(D_rows_gpu != want)[:5].tolist()
+        return 0.0
+    want, A = oracle.dedisperse_f32(X, w.nsamp, w.fch1, w.foff, w.tsamp, dms, rows=rows, interchanged=True)
+    err = np.abs(D_rows_gpu.astype(np.float64) - want)
+    worst = float((err / (F32_RTOL * A + 1e-300)).max())
+    assert worst <= 1.0, "f32 mismatch: worst err/(1e-5*A) = %g at %s" % (worst, np.argwhere(err > F32_RTOL * A)[:5].tolist())
+    return worst
+
+
+def p8_rows(w, pulses=()):
+    """first, last, every 64th trial, the tile seams around 63/64 and 127/128, and each injected-pulse DM"""
+    r = set(range(0, w.ndm, 64)) | {w.ndm - 1, 63, 127, 128} | {d for d, _, _ in pulses}
+    return np.array(sorted(x for x in r if 0 <= x < w.ndm), dtype=np.int32)

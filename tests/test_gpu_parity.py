@@ -1,6 +1,8 @@
 """GPU parity tests proper: the CUDA path (through the C ABI) against the oracle, element by
 element, on the same seeded inputs.  Bit-exact for uint8->int32; |D_gpu - D_oracle| <=
 1e-5 * sum_c|X| per element for float32 (north_star)."""
+import os
+
 import numpy as np
 import pytest
 
@@ -8,8 +10,8 @@ import oracle
 import paper_1401_8258_b200 as dd
 from paper_1401_8258_b200 import synth
 
-from _util import (assert_parity, assert_row_checksums, assert_sampled_parity, dd_dtype,
-                   gpu_dedisperse, make_case, small)
+from _util import (assert_parity, assert_row_checksums, assert_sampled_parity, assert_whole_rows, dd_dtype,
+                   gpu_dedisperse, make_case, p8_rows, small)
 
 pytestmark = pytest.mark.gpu
 
@@ -384,15 +386,33 @@ def _sample_points(w, n, seed):
     return di, ti
 
 
-def test_config3_full_size_sampled():
+FULL_PARITY = bool(int(os.environ.get("DD_FULL_PARITY", "0")))   # every-element passes of configs 3-5 (minutes of CPU)
+
+
+def _every_element(w, X, Dd, label, block=64):
+    """All ndm x nsamp outputs of one beam against the oracle's interchanged nest (pinned bit-identical to
+    the literal nest), 64 trials at a time; returns the worst err / (1e-5 * A) (0 for uint8)."""
+    worst = 0.0
+    for r0 in range(0, w.ndm, block):
+        rows = np.arange(r0, min(w.ndm, r0 + block), dtype=np.int32)
+        worst = max(worst, assert_whole_rows(w, X, Dd[r0:r0 + len(rows)].cpu().numpy(), rows))
+    print("FULL_PARITY %s: %d x %d = %d elements, worst err/(1e-5*A) = %.4f" % (
+        label, w.ndm, w.nsamp, w.ndm * w.nsamp, worst))
+    return worst
+
+
+def test_config3_full_size_checksums_rows_and_samples():
     # BASELINE.json configs[2] exactly as bench.py times it: 4096 ch x 4096 DMs x 2^18 samples, float32,
-    # one dd_execute on 16-byte aligned input (partial-sum kernel, G = 8)
+    # one dd_execute on 16-byte aligned input (partial-sum kernel).  P7: prefix-sum checksum of EVERY trial
+    # row; P8: whole rows for the first / last / every 64th trial, the tile seams and the pulse DMs;
+    # P9: sampled elements; with DD_FULL_PARITY=1 every element.
     import torch
     w = synth.WORKLOADS[3]
     tab = oracle.shift_table(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
     ms = int(tab.max())
     X = synth.make_input(w, w.nsamp + ms)
-    for d, t0, width in synth.pulse_plan(w, 5):
+    pulses = synth.pulse_plan(w, 5)
+    for d, t0, width in pulses:
         synth.inject_pulse(X, t0, width, 0.25, tab[d])
     stride = (w.nsamp + ms + 63) // 64 * 64
     plan = dd.Plan(dd.DD_F32, w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
@@ -402,48 +422,67 @@ def test_config3_full_size_sampled():
     assert plan.kernel_for(Xd, stride, 0, Dd, w.nsamp, 0, w.nsamp, 1) == dd.DD_KERNEL_PS
     plan.execute(Xd, stride, 0, Dd, w.nsamp, 0, w.nsamp, 1)
     torch.cuda.synchronize()
+    del Xd
+    assert_row_checksums(w, X, Dd, tab)
+    rows = p8_rows(w, pulses)
+    assert_whole_rows(w, X, Dd[torch.from_numpy(rows).long().cuda()].cpu().numpy(), rows)
     di, ti = _sample_points(w, 40000, 33)
     got = Dd[torch.from_numpy(di).cuda(), torch.from_numpy(ti).cuda()].cpu().numpy()
     _sampled(w, X, di, ti, got)
     # the injected pulses peak at their trial and start sample (S/N ~ A sqrt(nchans) = 16 per sample)
-    for d, t0, width in synth.pulse_plan(w, 5):
+    for d, t0, width in pulses:
         row = Dd[d].cpu().numpy()
         assert abs(int(np.argmax(np.convolve(row, np.ones(width), "valid"))) - t0) <= 1
+    if FULL_PARITY:
+        _every_element(w, X, Dd, w.name)
     plan.destroy()
 
 
-def test_config4_full_size_sampled_batch():
+def test_config4_full_size_batch_checksums_rows_and_samples():
     # BASELINE.json configs[3] as bench.py times it: 32 beams x 512 ch x 2048 DMs x 2^16 samples in ONE
-    # dd_execute (grid.z = beam); sampled elements of three beams against the oracle
+    # dd_execute (grid.z = beam).  P7 on every trial row of ALL 32 beams, P8 whole rows and sampled
+    # elements on three beams; with DD_FULL_PARITY=1 every element of those three beams.
     import torch
     w = synth.WORKLOADS[4]
     plan = dd.Plan(dd.DD_F32, w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    tab = oracle.shift_table(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
     ms = plan.max_shift()
+    assert ms == int(tab.max()) == 9760
     stride = (w.nsamp + ms + 63) // 64 * 64
     Xd = torch.zeros((w.nbeams, w.nchans, stride), dtype=torch.float32, device="cuda")
-    keep = {}
+    xs = []
     for b in range(w.nbeams):
         X = synth.make_input(w, w.nsamp + ms, beam=b)
         Xd[b, :, :w.nsamp + ms] = torch.from_numpy(X).cuda()
-        if b in (0, 13, 31):
-            keep[b] = X
+        xs.append(X)
     Dd = torch.empty((w.nbeams, w.ndm, w.nsamp), dtype=torch.float32, device="cuda")
     assert plan.kernel_for(Xd, stride, w.nchans * stride, Dd, w.nsamp, w.ndm * w.nsamp, w.nsamp, w.nbeams) == dd.DD_KERNEL_PS
     plan.execute(Xd, stride, w.nchans * stride, Dd, w.nsamp, w.ndm * w.nsamp, w.nsamp, w.nbeams)
     torch.cuda.synchronize()
-    for b, X in keep.items():
+    del Xd
+    ws = synth.scaled(w, nbeams=1)
+    for b in range(w.nbeams):
+        assert_row_checksums(ws, xs[b], Dd[b], tab)
+    rows = p8_rows(w)
+    for b in (0, 13, 31):
+        assert_whole_rows(ws, xs[b], Dd[b][torch.from_numpy(rows).long().cuda()].cpu().numpy(), rows)
         di, ti = _sample_points(w, 30000, 40 + b)
         got = Dd[b][torch.from_numpy(di).cuda(), torch.from_numpy(ti).cuda()].cpu().numpy()
-        _sampled(w, X, di, ti, got)
+        _sampled(w, xs[b], di, ti, got)
+        if FULL_PARITY:
+            _every_element(ws, xs[b], Dd[b], "%s beam %d" % (w.name, b))
     plan.destroy()
 
 
-def test_config5_full_size_streamed_in_four_pushes():
+def test_config5_full_size_streamed_checksums_rows_and_samples():
     # BASELINE.json configs[4] as bench.py times it: 2048 ch uint8, 10000 DMs, 2^18 samples fed through
-    # dd_stream_push in 4 chunks (the first carries maxshift extra samples); bit-exact sampled elements
+    # dd_stream_push in 4 chunks (the first carries maxshift extra samples).  Bit-exact: P7 on every trial
+    # row of the concatenated output, P8 whole rows, sampled elements around the chunk seams; with
+    # DD_FULL_PARITY=1 every element.
     import torch
     w = synth.WORKLOADS[5]
     plan = dd.Plan(dd.DD_U8, w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    tab = oracle.shift_table(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
     ms = plan.max_shift()
     assert ms == 37599                                               # golden maxshift of config 5
     X = synth.make_input(w, w.nsamp + ms)
@@ -460,12 +499,106 @@ def test_config5_full_size_streamed_in_four_pushes():
         emitted += n
     torch.cuda.synchronize()
     assert emitted == w.nsamp
+    del Xd
+    assert_row_checksums(w, X, Dd, tab)
+    rows = p8_rows(w)
+    assert_whole_rows(w, X, Dd[torch.from_numpy(rows).long().cuda()].cpu().numpy(), rows)
     di, ti = _sample_points(w, 40000, 55)
     ti[8:16] = [chunk - 1, chunk, 2 * chunk - 1, 2 * chunk, 3 * chunk - 1, 3 * chunk, chunk + 1, 3 * chunk + 1]
     got = Dd[torch.from_numpy(di).cuda(), torch.from_numpy(ti).cuda()].cpu().numpy()
     _sampled(w, X, di, ti, got)
     assert np.array_equal(Dd[0].cpu().numpy().astype(np.int64), X[:, :w.nsamp].sum(axis=0, dtype=np.int64))   # DM = 0 row
+    if FULL_PARITY:
+        _every_element(w, X, Dd, w.name)
     st.destroy(); plan.destroy()
+
+
+# ------------------------------------------------------------------ plan-level hazards
+
+def test_two_live_plans_do_not_undo_each_others_kernel_attributes():
+    # a plan with a large shared-memory need, then a small plan and a one-shot call on the same kernel
+    # instantiations, then the large plan again (the dynamic shared-memory attribute belongs to the
+    # kernel function, not to a plan)
+    import torch
+    for dtype in ("f32", "u8"):
+        big = small(3 if dtype == "f32" else 5, 512, 300, 3000, dtype=dtype)
+        # same channel width and trial grid, fewer channels: a plan the same partial-sum kernels take with a
+        # much smaller shared-memory need
+        tiny = synth.scaled(big, nchans=32, ndm=130, nsamp=700)
+        Xb, _ = make_case(big)
+        Xt, _ = make_case(tiny)
+        pb = dd.Plan(dd_dtype(big), big.nchans, big.fch1, big.foff, big.tsamp, big.dm_list)
+        odt = torch.float32 if dtype == "f32" else torch.int32
+        Xbd = torch.from_numpy(Xb).cuda()
+        Db = torch.empty((big.ndm, big.nsamp), dtype=odt, device="cuda")
+        pb.execute(Xbd, Xb.shape[1], 0, Db, big.nsamp, 0, big.nsamp, 1)
+        torch.cuda.synchronize()
+        first = Db.clone()
+        pt = dd.Plan(dd_dtype(tiny), tiny.nchans, tiny.fch1, tiny.foff, tiny.tsamp, tiny.dm_list)
+        Dt = gpu_dedisperse(tiny, Xt, dd.DD_KERNEL_AUTO)
+        assert_parity(tiny, Xt, Dt)
+        f = dd.dd_dedisperse_f32 if dtype == "f32" else dd.dd_dedisperse_u8_i32
+        Dt2 = torch.empty((tiny.ndm, tiny.nsamp), dtype=odt, device="cuda")
+        f(torch.from_numpy(Xt).cuda(), tiny.nchans, tiny.nsamp, tiny.fch1, tiny.foff, tiny.tsamp, tiny.dm_list, Dt2)
+        assert np.array_equal(Dt2.cpu().numpy(), Dt)
+        Db.fill_(-7)
+        pb.execute(Xbd, Xb.shape[1], 0, Db, big.nsamp, 0, big.nsamp, 1)      # the older, larger plan still launches
+        torch.cuda.synchronize()
+        assert torch.equal(Db, first)
+        assert_parity(big, Xb, Db.cpu().numpy())
+        pt.destroy(); pb.destroy()
+
+
+def test_many_beams_times_channels_stay_on_the_partial_sum_kernel():
+    # 64 beams x 1024 channels = 65536 rows: more than a grid.y of the front end could hold (the rows are on
+    # grid.x); AUTO must not drop to the generic kernel, and the result must stay exact
+    import torch
+    nb = 64
+    w = synth.scaled(synth.WORKLOADS[2], ndm=64, nsamp=600, nbeams=nb)
+    plan = dd.Plan(dd.DD_U8, w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    ms = plan.max_shift()
+    total = w.nsamp + ms
+    g = torch.Generator(device="cuda").manual_seed(5)
+    Xd = torch.randint(0, 256, (nb, w.nchans, total), dtype=torch.uint8, device="cuda", generator=g)
+    Dd = torch.empty((nb, w.ndm, w.nsamp), dtype=torch.int32, device="cuda")
+    assert plan.kernel_for(Xd, total, w.nchans * total, Dd, w.nsamp, w.ndm * w.nsamp, w.nsamp, nb) == dd.DD_KERNEL_PS
+    assert plan.launches_for(Xd, total, w.nchans * total, Dd, w.nsamp, w.ndm * w.nsamp, w.nsamp, nb) == 2
+    plan.execute(Xd, total, w.nchans * total, Dd, w.nsamp, w.ndm * w.nsamp, w.nsamp, nb)
+    torch.cuda.synchronize()
+    ws = synth.scaled(w, nbeams=1)
+    for b in (0, 31, 63):
+        assert_parity(ws, Xd[b].cpu().numpy(), Dd[b].cpu().numpy())
+    assert "dd_ps_u8_kernel" in plan.describe()
+    plan.destroy()
+    # a plan the partial-sum kernel cannot take says so
+    coarse = small(1, 64, 9, 2500, dm_step=40.0)
+    pc = dd.Plan(dd.DD_F32, coarse.nchans, coarse.fch1, coarse.foff, coarse.tsamp, coarse.dm_list)
+    assert pc.kernel_for(0x1000, 1 << 20, 0, 0x2000, 2500, 0, 2500, 1) == dd.DD_KERNEL_GENERIC
+    assert "unavailable" in pc.describe() and pc.launches_for(0x1000, 1 << 20, 0, 0x2000, 2500, 0, 2500, 1) == 1
+    pc.destroy()
+
+
+def test_execute_host_with_beams():
+    import torch
+    nb = 3
+    for dtype in ("f32", "u8"):
+        w = small(4, 128, 70, 9000 + 5, dtype=dtype, nbeams=nb)
+        plan = dd.Plan(dd_dtype(w), w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+        ms = plan.max_shift()
+        total = w.nsamp + ms
+        xs = np.stack([synth.make_input(w, total, beam=b) for b in range(nb)])
+        Xp = torch.from_numpy(xs).pin_memory()
+        Dp = torch.full((nb, w.ndm, w.nsamp), -7, dtype=torch.float32 if dtype == "f32" else torch.int32).pin_memory()
+        plan.execute_host(Xp, total, w.nchans * total, Dp, w.nsamp, w.ndm * w.nsamp, w.nsamp, nb)
+        ws = synth.scaled(w, nbeams=1)
+        for b in range(nb):
+            assert_parity(ws, xs[b], Dp[b].numpy())
+        Dd = torch.empty((nb, w.ndm, w.nsamp), dtype=Dp.dtype, device="cuda")
+        plan.execute(torch.from_numpy(xs).cuda(), total, w.nchans * total, Dd, w.nsamp, w.ndm * w.nsamp, w.nsamp, nb)
+        torch.cuda.synchronize()
+        assert torch.equal(Dd.cpu(), Dp)                                # host path == resident path, bit for bit
+        plan.destroy()
+    dd.dd_release_workspaces()
 
 
 def test_uint8_partial_sum_kernel_takes_unaligned_output():

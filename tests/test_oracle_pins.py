@@ -239,3 +239,42 @@ def test_generators_are_seeded_and_shaped():
     assert abs(f.mean()) < 0.05 and abs(f.std() - 1) < 0.05
     assert not np.array_equal(synth.noise_f32(3, 4, 100), synth.noise_f32(4, 4, 100))
     assert [synth.WORKLOADS[i].adds for i in (1, 2)] == [64 * 32 * 8192, 1024 * 1024 * (1 << 17)]
+
+
+# ---------------------------------------------------------------- the interchanged (d, c, t) nest
+
+def test_interchanged_nest_is_bit_identical_to_the_literal_nest():
+    """oracle_dedisperse_*_dct adds the channels of every element in the same order into a double
+    that starts at zero, so its output must equal the literal (d, t, c) nest BIT FOR BIT -- on
+    BASELINE.json config 1 in full, on config 2 (all channels and trials, time axis cut), on a
+    row subset, and on a float32 case whose sums are inexact in double only through the order."""
+    # config 1, full size, D and A
+    w = synth.WORKLOADS[1]
+    ms = oracle.max_shift(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    X = synth.make_input(w, w.nsamp + ms)
+    D1, A1 = oracle.dedisperse_f32(X, w.nsamp, w.fch1, w.foff, w.tsamp, w.dm_list)
+    D2, A2 = oracle.dedisperse_f32(X, w.nsamp, w.fch1, w.foff, w.tsamp, w.dm_list, interchanged=True)
+    assert np.array_equal(D1.view(np.int64), D2.view(np.int64))
+    assert np.array_equal(A1.view(np.int64), A2.view(np.int64))
+    # config 2: 1024 channels x 1024 trials, 3000 samples
+    w = synth.scaled(synth.WORKLOADS[2], nsamp=3000)
+    ms = oracle.max_shift(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    X = synth.make_input(w, w.nsamp + ms)
+    assert np.array_equal(oracle.dedisperse_u8(X, w.nsamp, w.fch1, w.foff, w.tsamp, w.dm_list),
+                          oracle.dedisperse_u8(X, w.nsamp, w.fch1, w.foff, w.tsamp, w.dm_list, interchanged=True))
+    # row subsets in arbitrary order, float32 data with a large dynamic range (order-sensitive sums)
+    g = np.random.default_rng(77)
+    w = synth.scaled(synth.WORKLOADS[3], nchans=300, foff=-300.0 / 300, ndm=90, nsamp=2001)
+    ms = oracle.max_shift(w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+    X = (g.standard_normal((w.nchans, w.nsamp + ms)) * 10.0 ** g.uniform(-6, 6, (w.nchans, 1))).astype(np.float32)
+    rows = np.array([89, 0, 17, 17, 44], dtype=np.int32)
+    D1, A1 = oracle.dedisperse_f32(X, w.nsamp, w.fch1, w.foff, w.tsamp, w.dm_list, rows=rows)
+    D2, A2 = oracle.dedisperse_f32(X, w.nsamp, w.fch1, w.foff, w.tsamp, w.dm_list, rows=rows, interchanged=True)
+    assert np.array_equal(D1.view(np.int64), D2.view(np.int64))
+    assert np.array_equal(A1.view(np.int64), A2.view(np.int64))
+    # and the interchanged nest against the separate pure-Python brute force on a tiny input
+    fch1, foff, tsamp, dms = 400.0, -3.0, 2e-4, np.linspace(0.0, 7.5, 6)
+    ms = oracle.max_shift(7, fch1, foff, tsamp, dms)
+    Xf = g.standard_normal((7, 40 + ms)).astype(np.float32)
+    D, _ = oracle.dedisperse_f32(Xf, 40, fch1, foff, tsamp, dms, interchanged=True)
+    assert np.allclose(D, brute(Xf, 40, fch1, foff, tsamp, dms), rtol=0, atol=1e-12)

@@ -45,6 +45,38 @@ def test_two_ranks_shard_beams_and_reduce_the_timing():
         assert rate == 10 * 2 / 2.0
 
 
+def _bench_rank(out):
+    # what bench.run_ours does around its timed region, with a stubbed step time: process group from the
+    # environment bench.launch_ranks set, max-over-ranks reduction, whole-job rate
+    import bench
+    rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+    assert os.environ["MASTER_ADDR"] == "127.0.0.1" and int(os.environ["LOCAL_RANK"]) == rank
+    dist.init_process_group("gloo")
+    try:
+        total_ms = 100.0 * (1 + rank)                                   # rank 1 took twice as long
+        out[rank] = bench.finish_timing(total_ms, 10, 1000, world, dist, None)
+    finally:
+        dist.destroy_process_group()
+
+
+def test_bench_launches_its_own_ranks_and_reduces_over_them():
+    # `python bench.py --gpus 2` without torchrun goes through bench.launch_ranks
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    if root not in sys.path:
+        sys.path.insert(0, root)
+    import bench
+    with mp.Manager() as m:
+        out = m.dict()
+        bench.launch_ranks(2, _bench_rank, (out,))
+        res = dict(out)
+    assert sorted(res) == [0, 1]
+    for rank in (0, 1):
+        ms_per_step, value = res[rank]
+        assert ms_per_step == 20.0                                          # slowest rank: 200 ms / 10 steps
+        assert value == 1000 * 2 / 0.020 / 1e9                              # both ranks' units over that time
+
+
 def test_single_process_is_the_identity():
     assert sharding.max_over_ranks(3.5) == 3.5
     assert sharding.beams_of_rank(0, 1, 4) == [0, 1, 2, 3]
