@@ -197,7 +197,7 @@ class Case:
         self.es = 4 if w.dtype == "f32" else 1
         self.plan = dd.Plan(dtype, w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
         if kernel:
-            self.plan.set_kernel({"generic": dd.DD_KERNEL_GENERIC, "ps": dd.DD_KERNEL_PS}[kernel])
+            self.plan.set_kernel({"generic": dd.DD_KERNEL_GENERIC, "ps": dd.DD_KERNEL_PS, "direct": dd.DD_KERNEL_DIRECT}[kernel])
         self.ms = ms = self.plan.max_shift()
         nb = self.nb = w.nbeams
         self.in_stride = (w.nsamp + ms + 63) // 64 * 64
@@ -301,7 +301,7 @@ def counters_for(workload, kern):
 
 
 def kernel_name(kern):
-    return {1: "generic", 2: "ps"}.get(kern, str(kern))
+    return {1: "generic", 2: "ps", 3: "direct"}.get(kern, str(kern))
 
 
 def roofline_of(w, case, kernel_ms, clocks):
@@ -495,7 +495,7 @@ def main():
     ap.add_argument("--config", type=int, default=HEADLINE,
                     help="BASELINE.json config number (1-5); default 3 = configs[2], the largest single-GPU shape")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--kernel", default=None, choices=["generic", "ps"])
+    ap.add_argument("--kernel", default=None, choices=["generic", "ps", "direct"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config legs (profiling aid)")
     ap.add_argument("--nsamp", type=int, default=0,

@@ -61,6 +61,10 @@ enum { DD_F32 = 0,   /* float32 in, float32 out  */
 /* kernel selection for dd_plan_set_kernel (tests and benchmarks; default DD_KERNEL_AUTO) */
 enum { DD_KERNEL_AUTO    = 0,
        DD_KERNEL_GENERIC = 1,   /* shared-memory channel-vector kernel (thesis Alg. 1 modernised), any DM list */
+       DD_KERNEL_DIRECT  = 3,   /* one thread per output sample, operands straight from global memory / L2;
+                                   AUTO takes it for tiny plans (nchans * ndm <= 4096), which are bound by
+                                   launch latency and grid size, not by any pipe (decided from the plan
+                                   alone, so all calls of a plan add in the same order) */
        DD_KERNEL_PS      = 2 }; /* TMA-staged kernels (float32 and uint8) with partial sums of 4-8 adjacent
                                    channels shared between the trials of a 64/128-trial tile; plans whose
                                    per-trial delay steps are too coarse for them run DD_KERNEL_GENERIC
@@ -112,8 +116,9 @@ int     dd_plan_nchans(const dd_plan* plan);
  * with the oracle's independently built table) */
 int     dd_plan_shift_table(const dd_plan* plan, int32_t* host_out);
 int     dd_plan_set_kernel(dd_plan* plan, int kernel);          /* DD_KERNEL_* */
-/* which kernel dd_execute would launch for these arguments: DD_KERNEL_PS (both dtypes, whenever the
- * plan's delay steps are fine enough for shared partial sums) or DD_KERNEL_GENERIC */
+/* which kernel dd_execute would launch for these arguments: DD_KERNEL_DIRECT (tiny plans), DD_KERNEL_PS
+ * (both dtypes, whenever the plan's delay steps are fine enough for shared partial sums) or
+ * DD_KERNEL_GENERIC */
 int     dd_plan_kernel_for(const dd_plan* plan, const void* X, int64_t in_stride,
                            int64_t in_beam_stride, const void* D, int64_t out_stride,
                            int64_t out_beam_stride, int64_t nsamp_out, int nbeams);

@@ -5,7 +5,7 @@ input generators and the BASELINE.json workload shapes (no arithmetic of the met
 """
 from .binding import (  # noqa: F401
     DD_OK, DD_ERR_BAD_ARG, DD_ERR_UNSUPPORTED, DD_ERR_NOMEM, DD_ERR_CUDA, DD_ERR_STATE,
-    DD_F32, DD_U8, DD_KERNEL_AUTO, DD_KERNEL_GENERIC, DD_KERNEL_PS,
+    DD_F32, DD_U8, DD_KERNEL_AUTO, DD_KERNEL_GENERIC, DD_KERNEL_PS, DD_KERNEL_DIRECT,
     DedispError, Plan, Stream, lib,
     dd_version, dd_max_shift, dd_shift_table, dd_release_workspaces,
     dd_dedisperse_f32, dd_dedisperse_u8_i32, dd_dedisperse_f32_host, dd_dedisperse_u8_i32_host,

@@ -16,7 +16,7 @@ from . import build as _build
 
 DD_OK, DD_ERR_BAD_ARG, DD_ERR_UNSUPPORTED, DD_ERR_NOMEM, DD_ERR_CUDA, DD_ERR_STATE = 0, -1, -2, -3, -4, -5
 DD_F32, DD_U8 = 0, 1
-DD_KERNEL_AUTO, DD_KERNEL_GENERIC, DD_KERNEL_PS = 0, 1, 2
+DD_KERNEL_AUTO, DD_KERNEL_GENERIC, DD_KERNEL_PS, DD_KERNEL_DIRECT = 0, 1, 2, 3
 
 _dp = C.POINTER(C.c_double)
 _vp = C.c_void_p

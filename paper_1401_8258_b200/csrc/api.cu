@@ -199,6 +199,7 @@ int dd_plan_create(dd_plan** out, int dtype, int nchans, double fch1, double fof
         delete p;
         return rc;
     }
+    p->tiny = (int64_t)nchans * ndm <= kDirectMaxCells;
     // generic kernel tiling: the most trials per block whose channel vector still fits
     p->generic_kb = 1;
     p->generic_spread = 0;
@@ -280,7 +281,8 @@ int dd_plan_shift_table(const dd_plan* p, int32_t* host_out)
 int dd_plan_set_kernel(dd_plan* p, int kernel)
 {
     if (!p) return fail(DD_ERR_BAD_ARG, "plan is null");
-    if (kernel != DD_KERNEL_AUTO && kernel != DD_KERNEL_GENERIC && kernel != DD_KERNEL_PS)
+    if (kernel != DD_KERNEL_AUTO && kernel != DD_KERNEL_GENERIC && kernel != DD_KERNEL_PS &&
+        kernel != DD_KERNEL_DIRECT)
         return fail(DD_ERR_BAD_ARG, "unknown kernel id");
     if (kernel == DD_KERNEL_PS && !ps_plan_usable(p) && !psu8_plan_usable(p))
         return fail(DD_ERR_UNSUPPORTED, "the partial-sum kernel does not take this plan (dtype or per-trial delay steps)");
@@ -322,6 +324,9 @@ static void fill_args(const dd_plan* p, ExecArgs* a, const void* X, int64_t in_s
 static int kernel_for(const dd_plan* p, const ExecArgs& a)
 {
     if (p->kernel_pref == DD_KERNEL_GENERIC) return DD_KERNEL_GENERIC;
+    if (p->kernel_pref == DD_KERNEL_DIRECT) return direct_args_ok(a) ? DD_KERNEL_DIRECT : DD_KERNEL_GENERIC;
+    // tiny plans: decided from the plan alone, so every call of the plan adds in the same order
+    if (p->kernel_pref == DD_KERNEL_AUTO && p->tiny && direct_args_ok(a)) return DD_KERNEL_DIRECT;
     if (psu8_plan_usable(p) && psu8_args_ok(p, a)) return DD_KERNEL_PS;
     if (ps_plan_usable(p) && ps_args_ok(p, a)) return DD_KERNEL_PS;
     return DD_KERNEL_GENERIC;
@@ -384,6 +389,9 @@ int dd_execute(const dd_plan* p, const void* X, int64_t in_stride, int64_t in_be
     const int k = kernel_for(p, a);
     if (p->kernel_pref == DD_KERNEL_PS && k != DD_KERNEL_PS)
         return fail(DD_ERR_UNSUPPORTED, "partial-sum kernel forced but the grid does not fit");
+    if (p->kernel_pref == DD_KERNEL_DIRECT && k != DD_KERNEL_DIRECT)
+        return fail(DD_ERR_UNSUPPORTED, "direct kernel forced but the grid does not fit");
+    if (k == DD_KERNEL_DIRECT) return launch_direct(p->dtype, a);
     if (k == DD_KERNEL_PS) return p->dtype == DD_U8 ? launch_psu8(p, a) : launch_ps(p, a);
     return launch_generic(p->dtype, p->generic_kb, p->generic_spread, a);
 }
@@ -406,11 +414,14 @@ int dd_plan_describe(const dd_plan* p, char* buf, int buflen)
                     " channels x " + std::to_string(p->ndm) + " trials, maxshift " +
                     std::to_string(p->host.maxshift) + ", device " + std::to_string(p->device) + "; ";
     if (p->ndm == 0) t += "empty plan (nothing to launch)";
+    else if (p->tiny && p->kernel_pref == DD_KERNEL_AUTO)
+        t += "direct kernel dd_direct_kernel (tiny plan: nchans * ndm <= " + std::to_string(kDirectMaxCells) +
+             ", one thread per output sample)";
     else if (p->dtype == DD_U8) t += psu8_plan_usable(p) ? psu8_describe(p) : "partial-sum kernel unavailable: " + p->ps_why;
     else t += ps_plan_usable(p) ? ps_describe(p) : "partial-sum kernel unavailable: " + p->ps_why;
     if (p->ndm > 0) t += "; generic kernel: " + std::to_string(p->generic_kb) + " trials per block";
     if (p->kernel_pref != DD_KERNEL_AUTO)
-        t += std::string("; forced: ") + (p->kernel_pref == DD_KERNEL_PS ? "ps" : "generic");
+        t += std::string("; forced: ") + (p->kernel_pref == DD_KERNEL_PS ? "ps" : p->kernel_pref == DD_KERNEL_DIRECT ? "direct" : "generic");
     const int n = (int)std::min<size_t>(t.size(), (size_t)buflen - 1);
     std::memcpy(buf, t.data(), (size_t)n);
     buf[n] = 0;

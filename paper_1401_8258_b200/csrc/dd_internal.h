@@ -56,6 +56,10 @@ struct ExecArgs {
 
 // generic channel-vector kernel; kb in {16,8,4,2,1}; max_spread = largest tile spread (samples)
 int launch_generic(int dtype, int kb, int max_spread, const ExecArgs& a);
+// one thread per output element (direct.cu): tiny plans, nchans * ndm <= kDirectMaxCells
+constexpr int64_t kDirectMaxCells = 4096;
+bool direct_args_ok(const ExecArgs& a);
+int launch_direct(int dtype, const ExecArgs& a);
 
 }  // namespace dd
 
@@ -94,6 +98,7 @@ struct dd_plan {
     int32_t* d_shift = nullptr;
     int32_t* d_order = nullptr;
     int kernel_pref = DD_KERNEL_AUTO;
+    bool tiny = false;                  // nchans * ndm <= kDirectMaxCells: AUTO takes the direct kernel
     int generic_kb = 1;
     int generic_spread = 0;
     dd_ps_plan* ps = nullptr;           // null: the float32 partial-sum kernel does not take this plan

@@ -1,6 +1,6 @@
 // Generic "channel vector" kernel: works for ANY plan (unsorted / non-uniform DM lists, large
 // per-trial shift steps, unaligned pointers and strides).  It is the correctness anchor and the
-// fallback for plans the partial-sum kernels (ps_f32.cu, ps_u8.cu) and tma_u8.cu do not take.
+// fallback for plans the partial-sum kernels (ps_f32.cu, ps_u8.cu) do not take.
 //
 // Structure (the thesis' Alg. 1, modernised): the grid maps onto the output
 // plane (DM, t); a block owns KB consecutive (sorted) trials x TB = 1024 output
@@ -148,8 +148,9 @@ int launch_one(const ExecArgs& a, int max_spread)
     const int rowwords = (kTB + max_spread + EPW - 1) / EPW + (EPW > 1 ? 1 : 0);
     const size_t smem = (size_t)2 * kCH * rowwords * 4 + (size_t)2 * kCH * KB * 4;
     auto kern = dd_generic_kernel<TIn, KB>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return fail(DD_ERR_CUDA, std::string("generic smem attr: ") + cudaGetErrorString(e));
+    int rc = ensure_dyn_smem((const void*)kern, smem);
+    if (rc != DD_OK) return rc;
+    cudaError_t e;
     const int64_t ntile_t = (a.nsamp_out + kTB - 1) / kTB;
     if (ntile_t > 65535 || a.nbeams > 65535)
         return fail(DD_ERR_UNSUPPORTED, "nsamp_out / nbeams too large for one launch");

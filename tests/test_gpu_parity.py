@@ -15,7 +15,8 @@ from _util import (assert_parity, assert_row_checksums, assert_sampled_parity, a
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = [pytest.param(dd.DD_KERNEL_GENERIC, id="generic"), pytest.param(dd.DD_KERNEL_AUTO, id="auto")]
+KERNELS = [pytest.param(dd.DD_KERNEL_GENERIC, id="generic"), pytest.param(dd.DD_KERNEL_AUTO, id="auto"),
+           pytest.param(dd.DD_KERNEL_DIRECT, id="direct")]
 # AUTO takes the partial-sum kernels (uint8 and float32; float32 through a re-pitched copy when X is not
 # 16-byte aligned) whenever the plan's delay steps are fine enough, else the generic kernel
 
@@ -40,6 +41,11 @@ def test_config1_full(kernel):
     assert_parity(w, X, D)
     d, t = np.unravel_index(D.argmax(), D.shape)
     assert (d, t) == (10, 4000) and abs(D[10, 4000] / 8.0 - 24.0) < 4.0      # S/N ~ A*sqrt(nchans)
+    if kernel == dd.DD_KERNEL_AUTO:                                           # a tiny plan: the direct kernel
+        plan = dd.Plan(dd.DD_F32, w.nchans, w.fch1, w.foff, w.tsamp, w.dm_list)
+        assert plan.kernel_for(0x1000, 1 << 20, 0, 0x2000, w.nsamp, 0, w.nsamp, 1) == dd.DD_KERNEL_DIRECT
+        assert "dd_direct_kernel" in plan.describe()
+        plan.destroy()
 
 
 CASES = [
@@ -271,7 +277,7 @@ def test_one_shot_and_host_calls(dtype):
 
 # ------------------------------------------------------------------ float32 partial-sum kernel, direct (aligned) path
 
-@pytest.mark.parametrize("idx,nchans,ndm,nsamp", [(3, 517, 130, 2000), (4, 256, 200, 1500), (3, 64, 40, 5000), (3, 130, 70, 600)])
+@pytest.mark.parametrize("idx,nchans,ndm,nsamp", [(3, 517, 130, 2000), (4, 256, 200, 1500), (3, 64, 70, 5000), (3, 130, 70, 600)])
 def test_ps_kernel_reads_aligned_input_directly(idx, nchans, ndm, nsamp):
     """16-byte aligned X with strides that are multiples of four elements is staged by TMA straight from
     the caller's buffer (no re-pitch copy): several DM tiles, several time tiles, ragged tails, a
@@ -571,7 +577,7 @@ def test_many_beams_times_channels_stay_on_the_partial_sum_kernel():
     assert "dd_ps_u8_kernel" in plan.describe()
     plan.destroy()
     # a plan the partial-sum kernel cannot take says so
-    coarse = small(1, 64, 9, 2500, dm_step=40.0)
+    coarse = small(1, 64, 70, 2500, dm_step=40.0)                    # 4480 cells: not a tiny plan either
     pc = dd.Plan(dd.DD_F32, coarse.nchans, coarse.fch1, coarse.foff, coarse.tsamp, coarse.dm_list)
     assert pc.kernel_for(0x1000, 1 << 20, 0, 0x2000, 2500, 0, 2500, 1) == dd.DD_KERNEL_GENERIC
     assert "unavailable" in pc.describe() and pc.launches_for(0x1000, 1 << 20, 0, 0x2000, 2500, 0, 2500, 1) == 1
