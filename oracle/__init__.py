@@ -18,6 +18,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "dedisp_oracle.cpp")
+_SRC_POST = os.path.join(_HERE, "postproc_oracle.cpp")
 _SO = os.path.join(_HERE, "libdedisp_oracle.so")
 _lock = threading.Lock()
 _lib = None
@@ -27,11 +28,11 @@ def build(force: bool = False) -> str:
     """Compile the oracle shared object (no CUDA involved)."""
     with _lock:
         if (not force and os.path.exists(_SO)
-                and os.path.getmtime(_SO) >= os.path.getmtime(_SRC)):
+                and os.path.getmtime(_SO) >= max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_POST))):
             return _SO
         tmp = _SO + ".tmp.%d" % os.getpid()
         cmd = ["g++", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
-               "-std=c++17", "-o", tmp, _SRC]
+               "-std=c++17", "-o", tmp, _SRC, _SRC_POST]
         subprocess.run(cmd, check=True)
         os.replace(tmp, _SO)
         return _SO
@@ -68,6 +69,21 @@ def _load():
     lib.oracle_elements_u8.restype = None
     lib.oracle_elements_u8.argtypes = [C.c_void_p, C.c_int, C.c_int64, C.c_double, C.c_double,
                                        C.c_double, dp, ip, lp, C.c_int64, lp]
+    # post-processing (postproc_oracle.cpp)
+    lib.oracle_median_filter.restype = None
+    lib.oracle_median_filter.argtypes = [dp, C.c_int64, C.c_int, dp]
+    lib.oracle_fit_line.restype = None
+    lib.oracle_fit_line.argtypes = [dp, C.c_int64, dp, dp]
+    lib.oracle_detrend.restype = None
+    lib.oracle_detrend.argtypes = [dp, C.c_int64, C.c_double, C.c_double, dp, dp]
+    lib.oracle_normalise.restype = None
+    lib.oracle_normalise.argtypes = [dp, C.c_int64, C.c_double, dp]
+    lib.oracle_postprocess_rows.restype = None
+    lib.oracle_postprocess_rows.argtypes = [C.c_void_p, C.c_int, C.c_int64, C.c_int64, C.c_int64, C.c_int, C.c_int,
+                                            C.c_int, dp, dp]
+    lib.oracle_threshold.restype = C.c_int64
+    lib.oracle_threshold.argtypes = [dp, C.c_int, C.c_int, C.c_int64, C.c_double, dp, C.POINTER(C.c_int32),
+                                     C.POINTER(C.c_int32), lp, dp, C.c_int64]
     _lib = lib
     return lib
 
@@ -177,3 +193,76 @@ def num_threads() -> int:
         return len(os.sched_getaffinity(0))
     except AttributeError:
         return os.cpu_count() or 1
+
+
+# ------------------------------------------------------------------ post-processing
+
+def _f64(a):
+    return np.ascontiguousarray(np.asarray(a, dtype=np.float64))
+
+
+def median_filter(x, w) -> np.ndarray:
+    """eq 3.4 with the median, odd window w centred on each sample, ends clamped (R15)."""
+    x = _f64(x)
+    assert x.ndim == 1 and w >= 1 and w % 2 == 1
+    y = np.empty_like(x)
+    _load().oracle_median_filter(_dp(x), len(x), int(w), _dp(y))
+    return y
+
+
+def fit_line(y):
+    """Least-squares line through (t, y_t), t = 0..n-1 -> (intercept, slope)."""
+    y = _f64(y)
+    a, b = C.c_double(0.0), C.c_double(0.0)
+    _load().oracle_fit_line(_dp(y), len(y), C.byref(a), C.byref(b))
+    return float(a.value), float(b.value)
+
+
+def detrend(y, intercept, slope):
+    """y_t - (intercept + slope t) and its population standard deviation (R17) -> (r, sigma)."""
+    y = _f64(y)
+    r = np.empty_like(y)
+    s = C.c_double(0.0)
+    _load().oracle_detrend(_dp(y), len(y), float(intercept), float(slope), _dp(r), C.byref(s))
+    return r, float(s.value)
+
+
+def normalise(r, sigma) -> np.ndarray:
+    r = _f64(r)
+    z = np.empty_like(r)
+    _load().oracle_normalise(_dp(r), len(r), float(sigma), _dp(z))
+    return z
+
+
+def postprocess(D, median_window=0, detrend=True, normalise=True):
+    """§3.5 on series D [..., n] (float32 or int32, the dedispersion output) -> (z float64 same shape,
+    stats float64 [..., 3] = intercept, slope, sigma)."""
+    D = np.ascontiguousarray(D)
+    assert D.dtype in (np.float32, np.int32)
+    assert detrend or not normalise
+    n = D.shape[-1]
+    nrows = D.size // n if n else 0
+    z = np.empty(D.shape, dtype=np.float64)
+    stats = np.empty(D.shape[:-1] + (3,), dtype=np.float64)
+    _load().oracle_postprocess_rows(D.ctypes.data, int(D.dtype == np.int32), nrows, n, n, int(median_window),
+                                    int(bool(detrend)), int(bool(normalise)), _dp(z), _dp(stats))
+    return z, stats
+
+
+def threshold(z, nsigma, sigma=None, capacity=None):
+    """§3.6: samples of z [nbeams][ndm][n] above nsigma (times sigma [nbeams][ndm] when z is not normalised)
+    -> (beam, dm, t, value) arrays in (beam, dm, t) order."""
+    z = _f64(z)
+    assert z.ndim == 3
+    nb, ndm, n = z.shape
+    sg = None if sigma is None else _f64(sigma)
+    cap = int(capacity if capacity is not None else z.size)
+    b = np.empty(cap, dtype=np.int32)
+    d = np.empty(cap, dtype=np.int32)
+    t = np.empty(cap, dtype=np.int64)
+    v = np.empty(cap, dtype=np.float64)
+    cnt = _load().oracle_threshold(_dp(z), nb, ndm, n, float(nsigma), None if sg is None else _dp(sg),
+                                   b.ctypes.data_as(C.POINTER(C.c_int32)), d.ctypes.data_as(C.POINTER(C.c_int32)),
+                                   _lp(t), _dp(v), cap)
+    k = min(int(cnt), cap)
+    return b[:k], d[:k], t[:k], v[:k], int(cnt)
