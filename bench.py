@@ -264,16 +264,41 @@ class Case:
         barrier()
         sampler = ClockSampler(gpu_index)
         sampler.start()
-        ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+        # two events around the K steps on the launching stream (an event per step would add its own
+        # host and device cost to every step, which matters for the launch-bound config 1)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         with torch.cuda.stream(self.stream):
-            ev[0].record(self.stream)
+            ev0.record(self.stream)
             for i in range(steps):
                 self.step()
-                ev[i + 1].record(self.stream)
+            ev1.record(self.stream)
         barrier()
         clocks = sampler.result()
-        per_step = [ev[i].elapsed_time(ev[i + 1]) for i in range(steps)]
-        return per_step, ev[0].elapsed_time(ev[-1]), clocks
+        total = ev0.elapsed_time(ev1)
+        return [total / steps] * steps, total, clocks
+
+    def graph_ms_per_step(self, steps=200):
+        """The same step captured `steps` times into one CUDA graph and replayed: device time per step
+        without the host's per-call launch cost (launch-bound workloads only)."""
+        torch = self.torch
+        g = torch.cuda.CUDAGraph()
+        cs = torch.cuda.Stream()
+        real = self.stream
+        try:
+            self.stream = cs
+            with torch.cuda.graph(g, stream=cs):
+                for _ in range(steps):
+                    self.step()
+        finally:
+            self.stream = real
+        g.replay()
+        torch.cuda.synchronize()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        g.replay()
+        ev1.record()
+        torch.cuda.synchronize()
+        return ev0.elapsed_time(ev1) / steps
 
     def close(self):
         if self.streamer is not None:
@@ -376,6 +401,24 @@ def run_ours(args, w):
                 same = same and bool(torch.equal(Dh[b, r0:r0 + 512].cuda(), case.Dd[b, r0:r0 + 512]))
         e2e["matches_resident_result"] = same
         del Dh
+        # the same path with the post-processing row (median w = 5, detrend, normalise, 6 sigma) run on the
+        # device and ONLY the candidate list coming back (dd_search_host): no D -> host copy
+        prm = dd.post_params(5, True, True, nsigma=6.0)
+        cap = 1 << 20
+        hc = torch.zeros(cap * 4, dtype=torch.int32).pin_memory()
+        sa = (case.Xh, case.in_stride, w.nchans * case.in_stride, w.nsamp, nb, prm, hc, cap)
+        ncand = case.plan.search_host(*sa)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            ncand = case.plan.search_host(*sa)
+        dt = (time.perf_counter() - t0) / n_e2e
+        dt = sharding.max_over_ranks(dt, dist, "cuda")
+        e2e["search"] = {"value": sharding.whole_job_rate(w.adds, world, dt) / 1e9, "unit": UNIT, "ms_per_step": dt * 1e3,
+                         "h2d_bytes_per_step": e2e["h2d_bytes_per_step"],
+                         "d2h_bytes_per_step": int(8 + 16 * min(ncand, cap)), "candidates": int(ncand),
+                         "post": "median 5, detrend, normalise, 6 sigma (PAPER.md:1204-1221)",
+                         "gpu_launches_per_step": None}
 
     line = None
     if rank == 0:
@@ -428,6 +471,11 @@ def run_ours(args, w):
                 per["cfg%d" % idx]["note"] = ("launch-bound: %.2f us of adds at the roofline; empty-kernel launch "
                                               "measured beside it" % (wi.adds / 37.2e12 * 1e6))
                 per["cfg%d" % idx]["empty_launch_us"] = empty_launch_us(torch)
+                gms = c.graph_ms_per_step()
+                per["cfg%d" % idx]["cuda_graph"] = {
+                    "ms_per_step": gms, "value": wi.adds / (gms * 1e-3) / 1e9,
+                    "note": "200 dd_execute calls captured into one CUDA graph and replayed: device time per step "
+                            "without the per-call host launch cost that bounds ms_per_step above"}
             c.close()
         line["per_config"] = per
 

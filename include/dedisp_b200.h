@@ -174,6 +174,58 @@ int     dd_stream_push(dd_stream* s, const void* X_new, int64_t in_stride, int64
 int     dd_stream_reset(dd_stream* s);
 void    dd_stream_destroy(dd_stream* s);
 
+/* ---- post-processing of the dedispersed series and first stage of event detection
+ * (§3.5 "Signal Post-processing", §3.6 "Detection and Candidate Selection"),
+ * on the device: the (DM, t) plane stays in HBM, only the candidate list goes back to the host.
+ * Steps, in the paper's order; each series (one beam, one DM trial, nsamp samples) on its own:
+ *   1. median filter, eq 3.4: y_m = median{x_i, |i - m| <= (w-1)/2}, w odd ("5 or 7"), window
+ *      indices clamped to the ends of the series;
+ *   2. detrend: subtract the least-squares line through (t, y_t), t = 0..nsamp-1;
+ *   3. normalise: divide by the population standard deviation of the detrended series (a constant
+ *      series gives zeros);
+ *   4. threshold: samples whose value exceeds nsigma standard deviations (strictly) become
+ *      (beam, dm, t, value) candidates, value in units of sigma.
+ * The regression sums, the standard deviation and the threshold comparison are evaluated in double
+ * precision; medians are exact selections. */
+typedef struct dd_post_params {
+    int   median_window;   /* 0 or 1: no median filter; else 3, 5, 7 or 9 */
+    int   detrend;         /* 1: step 2 */
+    int   normalise;       /* 1: step 3 (needs detrend) */
+    int   threshold_on;    /* 1: step 4 (needs detrend: sigma is that of the detrended series) */
+    float nsigma;          /* threshold in units of sigma */
+} dd_post_params;
+
+typedef struct dd_candidate {
+    int32_t beam;          /* beam index */
+    int32_t dm;            /* DM trial: row index of D (the caller's dm_list order) */
+    int32_t t;             /* output sample */
+    float   value;         /* detrended sample / sigma */
+} dd_candidate;
+
+/* D: DEVICE series [nbeams][ndm][nsamp] as dd_execute wrote them -- float32 for dtype DD_F32, int32 for
+ * DD_U8 -- strides in elements; not modified unless Z aliases it.
+ * Z: DEVICE float32 [nbeams][ndm][nsamp] (strides z_stride, z_beam_stride) receives the processed series,
+ * or NULL; Z may be D itself (same strides) only when median_window <= 1.
+ * stats: DEVICE double [nbeams*ndm][3] = (intercept, slope, sigma) per series, or NULL.
+ * cand / capacity / count: DEVICE candidate buffer, its size in entries, and a DEVICE counter that the
+ * CALLER zeroes; the counter is advanced for every detection, entries beyond capacity are dropped
+ * (count > capacity tells), the order of the entries is unspecified.  Needed when threshold_on.
+ * Enqueued on cuda_stream, no synchronisation.  nsamp must fit int32. */
+int     dd_postprocess(int dtype, const void* D, int64_t stride, int64_t beam_stride, int ndm,
+                       int64_t nsamp, int nbeams, const dd_post_params* params,
+                       float* Z, int64_t z_stride, int64_t z_beam_stride, double* stats,
+                       dd_candidate* cand, int64_t capacity, unsigned long long* count,
+                       void* cuda_stream);
+/* number of kernels dd_postprocess launches for these parameters (bench.py's gpu_launches) */
+int     dd_postprocess_launches(const dd_post_params* params, int want_series);
+
+/* End to end with HOST buffers: uploads X (as dd_execute_host), dedisperses into a device buffer cached in
+ * the plan, post-processes it there and downloads ONLY the candidates: cand (HOST, capacity entries) and
+ * *count (HOST; may exceed capacity).  params->threshold_on must be 1.  Synchronous. */
+int     dd_search_host(dd_plan* plan, const void* X, int64_t in_stride, int64_t in_beam_stride,
+                       int64_t nsamp_out, int nbeams, const dd_post_params* params,
+                       dd_candidate* cand, int64_t capacity, int64_t* count);
+
 #ifdef __cplusplus
 }
 #endif

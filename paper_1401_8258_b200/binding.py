@@ -18,6 +18,15 @@ DD_OK, DD_ERR_BAD_ARG, DD_ERR_UNSUPPORTED, DD_ERR_NOMEM, DD_ERR_CUDA, DD_ERR_STA
 DD_F32, DD_U8 = 0, 1
 DD_KERNEL_AUTO, DD_KERNEL_GENERIC, DD_KERNEL_PS, DD_KERNEL_DIRECT = 0, 1, 2, 3
 
+class dd_post_params(C.Structure):
+    """Mirror of the C struct (include/dedisp_b200.h)."""
+    _fields_ = [("median_window", C.c_int), ("detrend", C.c_int), ("normalise", C.c_int),
+                ("threshold_on", C.c_int), ("nsigma", C.c_float)]
+
+
+# numpy view of dd_candidate (16 bytes)
+CANDIDATE_DTYPE = np.dtype([("beam", "<i4"), ("dm", "<i4"), ("t", "<i4"), ("value", "<f4")])
+
 _dp = C.POINTER(C.c_double)
 _vp = C.c_void_p
 _i64 = C.c_int64
@@ -46,6 +55,11 @@ SIGNATURES = {
     "dd_release_workspaces": (C.c_int, []),
     "dd_execute": (C.c_int, [_vp, _vp, _i64, _i64, _vp, _i64, _i64, _i64, C.c_int, _vp]),
     "dd_execute_host": (C.c_int, [_vp, _vp, _i64, _i64, _vp, _i64, _i64, _i64, C.c_int]),
+    "dd_postprocess": (C.c_int, [C.c_int, _vp, _i64, _i64, C.c_int, _i64, C.c_int, C.POINTER(dd_post_params),
+                                 _vp, _i64, _i64, _vp, _vp, _i64, _vp, _vp]),
+    "dd_postprocess_launches": (C.c_int, [C.POINTER(dd_post_params), C.c_int]),
+    "dd_search_host": (C.c_int, [_vp, _vp, _i64, _i64, _i64, C.c_int, C.POINTER(dd_post_params), _vp, _i64,
+                                 C.POINTER(_i64)]),
     "dd_stream_create": (C.c_int, [C.POINTER(_vp), _vp, _i64, C.c_int]),
     "dd_stream_push": (C.c_int, [_vp, _vp, _i64, _i64, _i64, _vp, _i64, _i64, C.POINTER(_i64), _vp]),
     "dd_stream_reset": (C.c_int, [_vp]),
@@ -160,6 +174,23 @@ def dd_dedisperse_u8_i32_host(X, nchans, nsamp, fch1, foff, tsamp, dm_list, D) -
     _check(lib().dd_dedisperse_u8_i32_host(_ptr(X), nchans, nsamp, fch1, foff, tsamp, p, n, _ptr(D)), "dd_dedisperse_u8_i32_host")
 
 
+def post_params(median_window=0, detrend=True, normalise=True, nsigma=None) -> dd_post_params:
+    """Fills a dd_post_params (thresholding on when nsigma is given)."""
+    return dd_post_params(int(median_window), int(bool(detrend)), int(bool(normalise)), int(nsigma is not None),
+                          float(nsigma if nsigma is not None else 0.0))
+
+
+def dd_postprocess(dtype, D, stride, beam_stride, ndm, nsamp, nbeams, params, Z=None, z_stride=0, z_beam_stride=0,
+                   stats=None, cand=None, capacity=0, count=None, stream=None) -> None:
+    _check(lib().dd_postprocess(dtype, _ptr(D), stride, beam_stride, ndm, nsamp, nbeams, C.byref(params), _ptr(Z),
+                                z_stride, z_beam_stride, _ptr(stats), _ptr(cand), capacity, _ptr(count),
+                                _stream_ptr(stream)), "dd_postprocess")
+
+
+def dd_postprocess_launches(params, want_series) -> int:
+    return _check(lib().dd_postprocess_launches(C.byref(params), int(bool(want_series))), "dd_postprocess_launches")
+
+
 # ------------------------------------------------------------------ plan / stream handles
 
 class Plan:
@@ -212,6 +243,14 @@ class Plan:
                      nbeams=1) -> None:
         _check(lib().dd_execute_host(self._h, _ptr(X), in_stride, in_beam_stride, _ptr(D), out_stride,
                                      out_beam_stride, nsamp_out, nbeams), "dd_execute_host")
+
+
+    def search_host(self, X, in_stride, in_beam_stride, nsamp_out, nbeams, params, cand, capacity) -> int:
+        """dd_search_host: cand is a HOST buffer (numpy array of CANDIDATE_DTYPE or pinned tensor); returns count."""
+        n = _i64(0)
+        _check(lib().dd_search_host(self._h, _ptr(X), in_stride, in_beam_stride, nsamp_out, nbeams, C.byref(params),
+                                    _ptr(cand), capacity, C.byref(n)), "dd_search_host")
+        return int(n.value)
 
 
 class Stream:

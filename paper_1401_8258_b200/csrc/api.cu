@@ -462,18 +462,24 @@ int dd_dedisperse_u8_i32(const uint8_t* X, int nchans, int64_t nsamp, double fch
 
 static int64_t round_up(int64_t v, int64_t m) { return (v + m - 1) / m * m; }
 
-int dd_execute_host(dd_plan* p, const void* X, int64_t in_stride, int64_t in_beam_stride, void* D,
-                    int64_t out_stride, int64_t out_beam_stride, int64_t nsamp_out, int nbeams)
+// Upload X in time slices, dedisperse every slice into the plan's cached device buffer and, when D is not
+// null, download the slices; the three overlap on internal streams.  With D == null the result stays on the
+// device (dd_search_host post-processes it there): *dD_out, *dstride_out, *dbeam_out describe it, and the
+// caller continues on w->s_run.  All streams are drained before returning when D != null or on failure.
+static int host_pipeline(dd_plan* p, const void* X, int64_t in_stride, int64_t in_beam_stride, void* D,
+                         int64_t out_stride, int64_t out_beam_stride, int64_t nsamp_out, int nbeams,
+                         void** dD_out, int64_t* dstride_out_p, int64_t* dbeam_out_p)
 {
     if (!p) return fail(DD_ERR_BAD_ARG, "plan is null");
     if (nsamp_out < 0) return fail(DD_ERR_BAD_ARG, "nsamp_out must be >= 0");
     if (nbeams < 1) return fail(DD_ERR_BAD_ARG, "nbeams must be >= 1");
     if (p->ndm == 0 || nsamp_out == 0) return DD_OK;
-    if (!X || !D) return fail(DD_ERR_BAD_ARG, "X or D is null");
+    if (!X) return fail(DD_ERR_BAD_ARG, "X is null");
     const int64_t ms = p->host.maxshift;
     if (in_stride < nsamp_out + ms) return fail(DD_ERR_BAD_ARG, "in_stride is shorter than nsamp_out + maxshift");
-    if (out_stride < nsamp_out) return fail(DD_ERR_BAD_ARG, "out_stride is shorter than nsamp_out");
-    if (nbeams > 1 && (in_beam_stride < (int64_t)p->nchans * in_stride || out_beam_stride < (int64_t)p->ndm * out_stride))
+    if (D && out_stride < nsamp_out) return fail(DD_ERR_BAD_ARG, "out_stride is shorter than nsamp_out");
+    if (nbeams > 1 && (in_beam_stride < (int64_t)p->nchans * in_stride ||
+                       (D && out_beam_stride < (int64_t)p->ndm * out_stride)))
         return fail(DD_ERR_BAD_ARG, "beam strides are shorter than a beam");
     {
         int rc = check_device(p);
@@ -557,6 +563,7 @@ int dd_execute_host(dd_plan* p, const void* X, int64_t in_stride, int64_t in_bea
             rc = erc;
             break;
         }
+        if (!D) continue;                                   // the result stays on the device
         if (!cuda_ok(cudaEventRecord(w->ev_run[k], w->s_run), "cudaEventRecord")) break;
         if (!cuda_ok(cudaStreamWaitEvent(w->s_out, w->ev_run[k], 0), "cudaStreamWaitEvent")) break;
         for (int b = 0; b < nbeams && rc == DD_OK; ++b)
@@ -565,11 +572,88 @@ int dd_execute_host(dd_plan* p, const void* X, int64_t in_stride, int64_t in_bea
                                       (size_t)(tb - ta) * 4, p->ndm, cudaMemcpyDeviceToHost, w->s_out),
                     "cudaMemcpy2DAsync(D2H)");
     }
-    const std::string first_error = rc != DD_OK ? g_last_error : std::string();
-    cuda_ok(cudaStreamSynchronize(w->s_out), "cudaStreamSynchronize");
-    cuda_ok(cudaStreamSynchronize(w->s_run), "cudaStreamSynchronize");
-    cuda_ok(cudaStreamSynchronize(w->s_in), "cudaStreamSynchronize");
-    if (!first_error.empty()) g_last_error = first_error;
+    if (dD_out) {
+        *dD_out = w->dD;
+        *dstride_out_p = dstride_out;
+        *dbeam_out_p = dbeam_out;
+    }
+    if (D || rc != DD_OK) {
+        const std::string first_error = rc != DD_OK ? g_last_error : std::string();
+        cuda_ok(cudaStreamSynchronize(w->s_out), "cudaStreamSynchronize");
+        cuda_ok(cudaStreamSynchronize(w->s_run), "cudaStreamSynchronize");
+        cuda_ok(cudaStreamSynchronize(w->s_in), "cudaStreamSynchronize");
+        if (!first_error.empty()) g_last_error = first_error;
+    }
+    return rc;
+}
+
+int dd_execute_host(dd_plan* p, const void* X, int64_t in_stride, int64_t in_beam_stride, void* D,
+                    int64_t out_stride, int64_t out_beam_stride, int64_t nsamp_out, int nbeams)
+{
+    if (p && p->ndm > 0 && nsamp_out > 0 && !D) return fail(DD_ERR_BAD_ARG, "X or D is null");
+    return host_pipeline(p, X, in_stride, in_beam_stride, D, out_stride, out_beam_stride, nsamp_out, nbeams,
+                         nullptr, nullptr, nullptr);
+}
+
+// ------------------------------------------------------------------------------ post-processing
+
+int dd_postprocess(int dtype, const void* D, int64_t stride, int64_t beam_stride, int ndm, int64_t nsamp,
+                   int nbeams, const dd_post_params* params, float* Z, int64_t z_stride, int64_t z_beam_stride,
+                   double* stats, dd_candidate* cand, int64_t capacity, unsigned long long* count,
+                   void* cuda_stream)
+{
+    int rc = require_sm100(nullptr);
+    if (rc != DD_OK) return rc;
+    return postprocess(dtype, D, stride, beam_stride, ndm, nsamp, nbeams, params, Z, z_stride, z_beam_stride, stats,
+                       cand, capacity, count, cuda_stream);
+}
+
+int dd_postprocess_launches(const dd_post_params* params, int want_series)
+{
+    if (!params) return fail(DD_ERR_BAD_ARG, "params is null");
+    return post_launches(params, want_series != 0);
+}
+
+int dd_search_host(dd_plan* p, const void* X, int64_t in_stride, int64_t in_beam_stride, int64_t nsamp_out,
+                   int nbeams, const dd_post_params* params, dd_candidate* cand, int64_t capacity, int64_t* count)
+{
+    if (!p || !params || !count) return fail(DD_ERR_BAD_ARG, "null argument");
+    *count = 0;
+    if (!params->threshold_on) return fail(DD_ERR_BAD_ARG, "dd_search_host needs params->threshold_on");
+    if (capacity < 0 || (capacity > 0 && !cand)) return fail(DD_ERR_BAD_ARG, "bad candidate buffer");
+    if (p->ndm == 0 || nsamp_out == 0) return DD_OK;
+    void* dD = nullptr;
+    int64_t dstride = 0, dbeam = 0;
+    int rc = host_pipeline(p, X, in_stride, in_beam_stride, nullptr, 0, 0, nsamp_out, nbeams, &dD, &dstride, &dbeam);
+    if (rc != DD_OK) return rc;
+    dd_host_ws* w = p->host_ws;
+    // candidates and the counter: one stream-ordered workspace, [counter (16 bytes)][capacity entries]
+    char* ws = nullptr;
+    const size_t bytes = 16 + (size_t)capacity * sizeof(dd_candidate);
+    rc = workspace_alloc((void**)&ws, bytes, w->s_run);
+    if (rc == DD_OK) {
+        cudaError_t e = cudaMemsetAsync(ws, 0, 16, w->s_run);
+        if (e != cudaSuccess) rc = cuda_fail("cudaMemsetAsync", e);
+    }
+    if (rc == DD_OK)
+        rc = postprocess(p->dtype, dD, dstride, dbeam, p->ndm, nsamp_out, nbeams, params, nullptr, 0, 0, nullptr,
+                         (dd_candidate*)(ws + 16), capacity, (unsigned long long*)ws, w->s_run);
+    unsigned long long n = 0;
+    if (rc == DD_OK) {
+        cudaError_t e = cudaMemcpyAsync(&n, ws, sizeof(n), cudaMemcpyDeviceToHost, w->s_run);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(w->s_run);
+        if (e != cudaSuccess) rc = cuda_fail("candidate count download", e);
+    }
+    if (rc == DD_OK && n > 0 && capacity > 0) {
+        const size_t k = (size_t)std::min<unsigned long long>(n, (unsigned long long)capacity);
+        cudaError_t e = cudaMemcpyAsync(cand, ws + 16, k * sizeof(dd_candidate), cudaMemcpyDeviceToHost, w->s_run);
+        if (e != cudaSuccess) rc = cuda_fail("candidate download", e);
+    }
+    if (ws) cudaFreeAsync(ws, w->s_run);
+    cudaError_t e = cudaStreamSynchronize(w->s_run);
+    if (e != cudaSuccess && rc == DD_OK) rc = cuda_fail("cudaStreamSynchronize", e);
+    cudaStreamSynchronize(w->s_in);
+    *count = (int64_t)n;
     return rc;
 }
 

@@ -87,6 +87,11 @@ bool psu8_plan_usable(const dd_plan* p);
 bool psu8_args_ok(const dd_plan* p, const ExecArgs& a);
 int launch_psu8(const dd_plan* p, const ExecArgs& a);
 std::string psu8_describe(const dd_plan* p);
+// post-processing (post.cu)
+int postprocess(int dtype, const void* D, int64_t stride, int64_t beam_stride, int ndm, int64_t nsamp, int nbeams,
+                const dd_post_params* prm, float* Z, int64_t z_stride, int64_t z_beam_stride, double* stats,
+                dd_candidate* cand, int64_t capacity, unsigned long long* count, void* cuda_stream);
+int post_launches(const dd_post_params* prm, bool want_series);
 }  // namespace dd
 
 struct dd_plan {

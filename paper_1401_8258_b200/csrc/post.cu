@@ -1,0 +1,280 @@
+// Post-processing of the dedispersed time series and first stage of event detection
+// (§3.5-3.6), on the device, so that the (DM, t) plane
+// -- 4 to 17 GB on the BASELINE.json workloads -- never has to cross PCIe: what leaves the GPU is
+// the list of (beam, DM, time, S/N) candidates.
+//
+// Steps, in the paper's order (readings R15-R19):
+//   1. windowed median, odd w <= 9 centred on the sample (eq 3.4), ends clamped;
+//   2. least-squares line over the whole series subtracted (pass 1: regression
+//      parameters, pass 2: subtraction + standard deviation);
+//   3. division by that standard deviation (pass 3);
+//   4. threshold at n sigma -> (time, DM, intensity) triplets per beam.
+//
+// Two kernels.  dd_post_stats_kernel: one block per series; pass 1 accumulates sum y and
+// sum (t - tm) y in double (the median is formed on the fly from the raw series, never stored),
+// the block reduces, pass 2 re-reads the series (the row, <= 1 MB, comes back from L2) and
+// accumulates sum r^2 of the residual about the fitted line -- the thesis' two passes, literally,
+// so a constant series gives sigma = 0 exactly.  dd_post_apply_kernel: grid over (time tiles,
+// series); every thread forms four consecutive medians from 4 + (w - 1) loaded samples,
+// subtracts the line, scales, optionally stores the processed series (16-byte stores) and
+// appends the samples above the threshold to the candidate list through an atomic cursor.
+// HBM traffic: D is read three times (twice through L2 for rows that fit) and written at most
+// once, against seven passes for the step-by-step pipeline of §3.5; the kernels are HBM-bound.
+// The thesis used one kernel per step with the series staged in shared memory.
+#include <cuda_runtime.h>
+
+#include <cmath>
+
+#include "dd_internal.h"
+
+namespace dd {
+
+namespace {
+
+constexpr int kThreads = 512;
+constexpr int kPer = 4;                       // consecutive samples per thread
+constexpr int kTile = kThreads * kPer;        // samples per block step
+
+template <typename T> __device__ __forceinline__ void cmpx(T& a, T& b)
+{
+    const T lo = a < b ? a : b, hi = a < b ? b : a;
+    a = lo;
+    b = hi;
+}
+// median of W values by a full odd-even transposition sort (static indices, branch-free)
+template <typename T, int W> __device__ __forceinline__ T median_of(T (&v)[W])
+{
+#pragma unroll
+    for (int round = 0; round < W; ++round)
+#pragma unroll
+        for (int i = round & 1; i + 1 < W; i += 2) cmpx(v[i], v[i + 1]);
+    return v[W / 2];
+}
+
+// The kPer medians (as doubles) of samples t0 .. t0+kPer-1 of one series; window indices clamped to
+// [0, n-1] (R15).  Samples past the end give 0 (never used).
+template <typename T, int W>
+__device__ __forceinline__ void medians4(const T* __restrict__ row, int64_t t0, int64_t n, double (&m)[kPer])
+{
+    constexpr int H = (W - 1) / 2;
+    T x[kPer + 2 * H];
+#pragma unroll
+    for (int i = 0; i < kPer + 2 * H; ++i) {
+        int64_t j = t0 - H + i;
+        j = j < 0 ? 0 : (j > n - 1 ? n - 1 : j);
+        x[i] = __ldg(row + j);
+    }
+#pragma unroll
+    for (int e = 0; e < kPer; ++e) {
+        T v[W];
+#pragma unroll
+        for (int i = 0; i < W; ++i) v[i] = x[e + i];
+        m[e] = (double)median_of<T, W>(v);
+    }
+}
+
+__device__ __forceinline__ double block_sum(double v, double* red)
+{
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __syncthreads();                                      // red may still be read from the previous reduction
+    if (lane == 0) red[warp] = v;
+    __syncthreads();
+    double s = 0.0;
+#pragma unroll
+    for (int w = 0; w < kThreads / 32; ++w) s += red[w];  // same order in every thread
+    return s;
+}
+
+// stats[row] = (intercept, slope, sigma): least-squares line through (t, y_t), t = 0..n-1, of the
+// median-filtered series and the population standard deviation of the residual.
+template <typename T, int W>
+__global__ void __launch_bounds__(kThreads)
+dd_post_stats_kernel(const T* __restrict__ D, int64_t stride, int64_t beam_stride, int ndm, int64_t n,
+                     double* __restrict__ stats)
+{
+    __shared__ double red[kThreads / 32];
+    const int64_t r = blockIdx.x;
+    const T* row = D + (r / ndm) * beam_stride + (r % ndm) * stride;
+    const double tm = 0.5 * (double)(n - 1);
+    double sy = 0.0, sty = 0.0;
+    for (int64_t t0 = (int64_t)threadIdx.x * kPer; t0 < n; t0 += kTile) {
+        double m[kPer];
+        medians4<T, W>(row, t0, n, m);
+#pragma unroll
+        for (int e = 0; e < kPer; ++e)
+            if (t0 + e < n) {
+                sy += m[e];
+                sty += ((double)(t0 + e) - tm) * m[e];
+            }
+    }
+    sy = block_sum(sy, red);
+    sty = block_sum(sty, red);
+    const double dn = (double)n;
+    const double stt = dn * (dn * dn - 1.0) / 12.0;       // sum (t - tm)^2
+    const double slope = stt > 0.0 ? sty / stt : 0.0;
+    const double intercept = sy / dn - slope * tm;
+    double ss = 0.0;
+    for (int64_t t0 = (int64_t)threadIdx.x * kPer; t0 < n; t0 += kTile) {
+        double m[kPer];
+        medians4<T, W>(row, t0, n, m);
+#pragma unroll
+        for (int e = 0; e < kPer; ++e)
+            if (t0 + e < n) {
+                const double res = m[e] - (intercept + slope * (double)(t0 + e));
+                ss += res * res;
+            }
+    }
+    ss = block_sum(ss, red);
+    if (threadIdx.x == 0) {
+        stats[r * 3 + 0] = intercept;
+        stats[r * 3 + 1] = slope;
+        stats[r * 3 + 2] = sqrt(ss / dn);
+    }
+}
+
+struct ApplyParams {
+    int64_t stride, beam_stride, n;
+    int ndm;
+    unsigned ntiles;
+    int detrend, normalise, threshold_on;
+    double nsigma;
+    const double* stats;
+    float* Z;
+    int64_t z_stride, z_beam_stride;
+    dd_candidate* cand;
+    int64_t capacity;
+    unsigned long long* count;
+};
+
+template <typename T, int W>
+__global__ void __launch_bounds__(kThreads)
+dd_post_apply_kernel(const T* __restrict__ D, const ApplyParams p)
+{
+    const int64_t r = blockIdx.x / p.ntiles;              // time tiles fastest (1-D grid: no 65535 limit on series)
+    const int beam = (int)(r / p.ndm), dm = (int)(r % p.ndm);
+    const T* row = D + (int64_t)beam * p.beam_stride + (int64_t)dm * p.stride;
+    const int64_t t0 = ((int64_t)(blockIdx.x % p.ntiles) * kThreads + threadIdx.x) * kPer;
+    if (t0 >= p.n) return;
+    double m[kPer];
+    medians4<T, W>(row, t0, p.n, m);
+    double intercept = 0.0, slope = 0.0, sigma = 0.0;
+    if (p.detrend) {
+        intercept = p.stats[r * 3 + 0];
+        slope = p.stats[r * 3 + 1];
+        sigma = p.stats[r * 3 + 2];
+    }
+    const double inv = sigma > 0.0 ? 1.0 / sigma : 0.0;    // sigma = 0: all-zero output (R17)
+    float out[kPer];
+#pragma unroll
+    for (int e = 0; e < kPer; ++e) {
+        double v = m[e];
+        if (p.detrend) v -= intercept + slope * (double)(t0 + e);
+        // un-normalised series are compared against n * sigma; same decision, same precision
+        const double snr = p.detrend ? v * inv : v;
+        if (p.normalise) v = snr;
+        out[e] = (float)v;
+        if (p.threshold_on && t0 + e < p.n && snr > p.nsigma) {
+            const unsigned long long at = atomicAdd(p.count, 1ull);
+            if ((int64_t)at < p.capacity) {
+                dd_candidate c;
+                c.beam = beam;
+                c.dm = dm;
+                c.t = (int32_t)(t0 + e);
+                c.value = (float)snr;
+                p.cand[at] = c;
+            }
+        }
+    }
+    if (p.Z) {
+        float* z = p.Z + (int64_t)beam * p.z_beam_stride + (int64_t)dm * p.z_stride + t0;
+        if (t0 + kPer <= p.n && (((uintptr_t)z) & 15) == 0) {
+            *reinterpret_cast<float4*>(z) = make_float4(out[0], out[1], out[2], out[3]);
+        } else {
+#pragma unroll
+            for (int e = 0; e < kPer; ++e)
+                if (t0 + e < p.n) z[e] = out[e];
+        }
+    }
+}
+
+template <typename T, int W>
+int launch_w(const void* D, int64_t nrows, const ApplyParams& ap, double* stats, cudaStream_t st)
+{
+    if (ap.detrend)
+        dd_post_stats_kernel<T, W><<<(unsigned)nrows, kThreads, 0, st>>>((const T*)D, ap.stride, ap.beam_stride, ap.ndm,
+                                                                          ap.n, stats);
+    if (ap.Z || ap.threshold_on) {
+        dd_post_apply_kernel<T, W><<<(unsigned)(nrows * ap.ntiles), kThreads, 0, st>>>((const T*)D, ap);
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(DD_ERR_CUDA, std::string("post-processing launch: ") + cudaGetErrorString(e));
+    return DD_OK;
+}
+
+template <typename T>
+int launch_t(int w, const void* D, int64_t nrows, const ApplyParams& ap, double* stats, cudaStream_t st)
+{
+    switch (w) {
+        case 1: return launch_w<T, 1>(D, nrows, ap, stats, st);
+        case 3: return launch_w<T, 3>(D, nrows, ap, stats, st);
+        case 5: return launch_w<T, 5>(D, nrows, ap, stats, st);
+        case 7: return launch_w<T, 7>(D, nrows, ap, stats, st);
+        case 9: return launch_w<T, 9>(D, nrows, ap, stats, st);
+    }
+    return fail(DD_ERR_BAD_ARG, "median_window must be 0, 1, 3, 5, 7 or 9");
+}
+
+}  // namespace
+
+int post_launches(const dd_post_params* prm, bool want_series)
+{
+    return (prm->detrend ? 1 : 0) + ((want_series || prm->threshold_on) ? 1 : 0);
+}
+
+int postprocess(int dtype, const void* D, int64_t stride, int64_t beam_stride, int ndm, int64_t nsamp, int nbeams,
+                const dd_post_params* prm, float* Z, int64_t z_stride, int64_t z_beam_stride, double* stats,
+                dd_candidate* cand, int64_t capacity, unsigned long long* count, void* cuda_stream)
+{
+    if (!prm) return fail(DD_ERR_BAD_ARG, "params is null");
+    if (dtype != DD_F32 && dtype != DD_U8) return fail(DD_ERR_BAD_ARG, "dtype must be DD_F32 or DD_U8");
+    if (ndm < 0 || nsamp < 0 || nbeams < 1) return fail(DD_ERR_BAD_ARG, "bad ndm / nsamp / nbeams");
+    const int w = prm->median_window <= 1 ? 1 : prm->median_window;
+    if (w != 1 && w != 3 && w != 5 && w != 7 && w != 9)
+        return fail(DD_ERR_BAD_ARG, "median_window must be 0, 1, 3, 5, 7 or 9");
+    if (prm->normalise && !prm->detrend)
+        return fail(DD_ERR_BAD_ARG, "normalise needs detrend (the thesis normalises the detrended series)");
+    if (prm->threshold_on && !prm->detrend)
+        return fail(DD_ERR_BAD_ARG, "the n-sigma threshold needs detrend (sigma is the detrended series')");
+    if (prm->threshold_on && (!cand || !count || capacity < 0))
+        return fail(DD_ERR_BAD_ARG, "thresholding needs a candidate buffer and a counter");
+    if (prm->threshold_on && !(prm->nsigma == prm->nsigma)) return fail(DD_ERR_BAD_ARG, "nsigma is NaN");
+    if (ndm == 0 || nsamp == 0) return DD_OK;
+    if (!D) return fail(DD_ERR_BAD_ARG, "D is null");
+    if (nsamp > 2147483647LL) return fail(DD_ERR_BAD_ARG, "nsamp must fit int32 (candidate time index)");
+    if (stride < nsamp || (Z && z_stride < nsamp)) return fail(DD_ERR_BAD_ARG, "stride is shorter than nsamp");
+    if (nbeams > 1 && (beam_stride <= 0 || (Z && z_beam_stride <= 0)))
+        return fail(DD_ERR_BAD_ARG, "beam strides must be positive when nbeams > 1");
+    if (Z && (const void*)Z == D && w > 1)
+        return fail(DD_ERR_BAD_ARG, "in-place output needs median_window <= 1 (neighbours read each other's samples)");
+    const int64_t nrows = (int64_t)nbeams * ndm;
+    const int64_t ntiles = (nsamp + kTile - 1) / kTile;
+    if (nrows * ntiles > 2147483647LL) return fail(DD_ERR_UNSUPPORTED, "series x time tiles exceed one grid: split the call");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    double* own_stats = nullptr;
+    if (prm->detrend && !stats) {
+        int rc = workspace_alloc((void**)&own_stats, (size_t)nrows * 3 * sizeof(double), cuda_stream);
+        if (rc != DD_OK) return rc;
+        stats = own_stats;
+    }
+    ApplyParams ap{stride, nbeams > 1 ? beam_stride : 0, nsamp, ndm, (unsigned)ntiles, prm->detrend, prm->normalise,
+                   prm->threshold_on, (double)prm->nsigma, stats, Z, z_stride, nbeams > 1 ? z_beam_stride : 0,
+                   cand, capacity, count};
+    const int rc = dtype == DD_F32 ? launch_t<float>(w, D, nrows, ap, stats, st)
+                                   : launch_t<int32_t>(w, D, nrows, ap, stats, st);
+    if (own_stats) cudaFreeAsync(own_stats, st);
+    return rc;
+}
+
+}  // namespace dd
