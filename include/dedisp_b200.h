@@ -226,6 +226,34 @@ int     dd_search_host(dd_plan* plan, const void* X, int64_t in_stride, int64_t 
                        int64_t nsamp_out, int nbeams, const dd_post_params* params,
                        dd_candidate* cand, int64_t capacity, int64_t* count);
 
+/* ---- RFI mitigation front end on the input buffer, before dedispersion (§3.3),
+ * in place on the device.  Stages, in the paper's order, per beam:
+ *   1. averaged bandpass b_c = mean_t X[c][t]; least-squares polynomial of order poly_order through
+ *      (x_c, b_c), x_c the channel index mapped onto [-1, 1]; RMSE = sqrt(mean_c (b_c - B_c)^2);
+ *   2. channel thresholding (eq 3.1): every channel is cut into non-overlapping windows of `window`
+ *      samples (the last may be shorter); a window with |mean - B_c| > t_chan * RMSE and its two
+ *      neighbours are replaced by the fitted bandpass value B_c;
+ *   3. spectrum thresholding (eq 3.2): with m_t the mean over channels of spectrum t (after step 2) and
+ *      mu, sigma the mean and population standard deviation of m over time, a spectrum with
+ *      m_t - mu > t_spec * sigma has (m_t - mean_c B_c) subtracted from every channel;
+ *   4. B_c is subtracted from every sample (the corrected spectra sit at a mean of ~0).
+ * Means, fit and comparisons are evaluated in double; the output is rounded once to float32. */
+typedef struct dd_rfi_params {
+    int   poly_order;      /* 0..12 ("p-th order polynomial") */
+    int   window;          /* W_c, samples per channel-thresholding window (thesis test: 512) */
+    float t_chan;          /* channel threshold in units of the fit's RMSE (thesis test: 7) */
+    float t_spec;          /* spectrum threshold in units of sigma of the spectrum means (thesis test: 5) */
+} dd_rfi_params;
+
+/* X: DEVICE float32 [nbeams][nchans][nsamp], strides in elements, modified in place.  Optional DEVICE
+ * outputs (NULL to skip): bandpass and fit, double [nbeams][nchans] (b_c and B_c); stats, double
+ * [nbeams][4] = (RMSE, mean_c B_c, mu, sigma); chan_flags, uint8 [nbeams][nchans][ceil(nsamp/window)]
+ * (1 = window replaced); spec_flags, uint8 [nbeams][nsamp] (1 = spectrum corrected).  At most 65535
+ * channel rows (nbeams * nchans) per call.  Enqueued on cuda_stream, no synchronisation. */
+int     dd_rfi_mitigate(float* X, int nchans, int64_t nsamp, int64_t stride, int64_t beam_stride, int nbeams,
+                        const dd_rfi_params* params, double* bandpass, double* fit, double* stats,
+                        uint8_t* chan_flags, uint8_t* spec_flags, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -24,6 +24,11 @@ class dd_post_params(C.Structure):
                 ("threshold_on", C.c_int), ("nsigma", C.c_float)]
 
 
+class dd_rfi_params(C.Structure):
+    """Mirror of the C struct (include/dedisp_b200.h)."""
+    _fields_ = [("poly_order", C.c_int), ("window", C.c_int), ("t_chan", C.c_float), ("t_spec", C.c_float)]
+
+
 # numpy view of dd_candidate (16 bytes)
 CANDIDATE_DTYPE = np.dtype([("beam", "<i4"), ("dm", "<i4"), ("t", "<i4"), ("value", "<f4")])
 
@@ -60,6 +65,8 @@ SIGNATURES = {
     "dd_postprocess_launches": (C.c_int, [C.POINTER(dd_post_params), C.c_int]),
     "dd_search_host": (C.c_int, [_vp, _vp, _i64, _i64, _i64, C.c_int, C.POINTER(dd_post_params), _vp, _i64,
                                  C.POINTER(_i64)]),
+    "dd_rfi_mitigate": (C.c_int, [_vp, C.c_int, _i64, _i64, _i64, C.c_int, C.POINTER(dd_rfi_params), _vp, _vp, _vp,
+                                  _vp, _vp, _vp]),
     "dd_stream_create": (C.c_int, [C.POINTER(_vp), _vp, _i64, C.c_int]),
     "dd_stream_push": (C.c_int, [_vp, _vp, _i64, _i64, _i64, _vp, _i64, _i64, C.POINTER(_i64), _vp]),
     "dd_stream_reset": (C.c_int, [_vp]),
@@ -185,6 +192,13 @@ def dd_postprocess(dtype, D, stride, beam_stride, ndm, nsamp, nbeams, params, Z=
     _check(lib().dd_postprocess(dtype, _ptr(D), stride, beam_stride, ndm, nsamp, nbeams, C.byref(params), _ptr(Z),
                                 z_stride, z_beam_stride, _ptr(stats), _ptr(cand), capacity, _ptr(count),
                                 _stream_ptr(stream)), "dd_postprocess")
+
+
+def dd_rfi_mitigate(X, nchans, nsamp, stride, beam_stride, nbeams, params, bandpass=None, fit=None, stats=None,
+                    chan_flags=None, spec_flags=None, stream=None) -> None:
+    _check(lib().dd_rfi_mitigate(_ptr(X), nchans, nsamp, stride, beam_stride, nbeams, C.byref(params), _ptr(bandpass),
+                                 _ptr(fit), _ptr(stats), _ptr(chan_flags), _ptr(spec_flags), _stream_ptr(stream)),
+           "dd_rfi_mitigate")
 
 
 def dd_postprocess_launches(params, want_series) -> int:

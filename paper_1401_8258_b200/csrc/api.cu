@@ -614,6 +614,16 @@ int dd_postprocess_launches(const dd_post_params* params, int want_series)
     return post_launches(params, want_series != 0);
 }
 
+int dd_rfi_mitigate(float* X, int nchans, int64_t nsamp, int64_t stride, int64_t beam_stride, int nbeams,
+                    const dd_rfi_params* params, double* bandpass, double* fit, double* stats, uint8_t* chan_flags,
+                    uint8_t* spec_flags, void* cuda_stream)
+{
+    int rc = require_sm100(nullptr);
+    if (rc != DD_OK) return rc;
+    return rfi_mitigate(X, nchans, nsamp, stride, beam_stride, nbeams, params, bandpass, fit, stats, chan_flags,
+                        spec_flags, cuda_stream);
+}
+
 int dd_search_host(dd_plan* p, const void* X, int64_t in_stride, int64_t in_beam_stride, int64_t nsamp_out,
                    int nbeams, const dd_post_params* params, dd_candidate* cand, int64_t capacity, int64_t* count)
 {

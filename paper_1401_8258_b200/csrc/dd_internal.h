@@ -92,6 +92,10 @@ int postprocess(int dtype, const void* D, int64_t stride, int64_t beam_stride, i
                 const dd_post_params* prm, float* Z, int64_t z_stride, int64_t z_beam_stride, double* stats,
                 dd_candidate* cand, int64_t capacity, unsigned long long* count, void* cuda_stream);
 int post_launches(const dd_post_params* prm, bool want_series);
+// RFI mitigation (rfi.cu)
+int rfi_mitigate(float* X, int nchans, int64_t nsamp, int64_t stride, int64_t beam_stride, int nbeams,
+                 const dd_rfi_params* prm, double* bandpass, double* fit, double* stats, uint8_t* chan_flags,
+                 uint8_t* spec_flags, void* cuda_stream);
 }  // namespace dd
 
 struct dd_plan {

@@ -1,0 +1,294 @@
+// RFI mitigation front end on X (§3.3), in place on the
+// device, before dedispersion.  Stages, in the paper's order (readings R20-R27):
+//   1. averaged bandpass b_c = mean_t X[c][t]; least-squares polynomial of order p through it; RMSE of
+//      the fit (§3.3.1);
+//   2. channel thresholding (§3.3.2, eq 3.1): windows of W_c samples whose mean is off the fitted
+//      bandpass value by more than T_c RMSE, and their two neighbours, are replaced by that value;
+//   3. spectrum thresholding (§3.3.3, eq 3.2): spectra whose mean exceeds mu + T_s sigma of the spectrum
+//      means lose the excess of their mean over the bandpass mean;
+//   4. the fitted bandpass is subtracted from every spectrum.
+//
+// The thesis copies the averaged bandpass to the host, fits it there and runs one kernel per step
+// with a write pass each.  Here everything stays on the device (the fit is one block solving the
+// normal equations in a Legendre basis in double precision) and the replacements are never written as
+// such: the window flags and the spectrum excesses are small side arrays, applied when the single
+// output pass subtracts the bandpass.  Passes over X: three reads (row means, window means, spectrum
+// means of the clipped data) and one read + write -- all HBM-bound streaming kernels, 16-byte loads
+// where the row alignment allows.  All means, the fit and the threshold comparisons are evaluated in
+// double precision; the output is rounded once, from double, to float32.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+
+#include "dd_internal.h"
+
+namespace dd {
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kMaxOrder = 12;
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double block_sum(double v, double* red)
+{
+    v = warp_sum(v);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __syncthreads();
+    if (lane == 0) red[warp] = v;
+    __syncthreads();
+    double s = 0.0;
+#pragma unroll
+    for (int w = 0; w < kThreads / 32; ++w) s += red[w];
+    return s;
+}
+
+// 1a. b[row] = mean over time of channel row (one block per (beam, channel))
+__global__ void __launch_bounds__(kThreads)
+dd_rfi_bandpass_kernel(const float* __restrict__ X, int nchans, int64_t n, int64_t stride, int64_t beam_stride,
+                       double* __restrict__ b)
+{
+    __shared__ double red[kThreads / 32];
+    const int64_t row = blockIdx.x;
+    const float* x = X + (row / nchans) * beam_stride + (row % nchans) * stride;
+    double s = 0.0;
+    for (int64_t t = threadIdx.x; t < n; t += kThreads) s += (double)__ldg(x + t);
+    s = block_sum(s, red);
+    if (threadIdx.x == 0) b[row] = s / (double)n;
+}
+
+// 1b. One block per beam: least-squares polynomial of order p through (x_c, b_c), x_c the channel index
+// mapped onto [-1, 1], in the Legendre basis P_0..P_p (normal equations, Gaussian elimination with partial
+// pivoting, double).  Writes the fitted values B and stats = (rmse, mean_c B_c).
+__global__ void __launch_bounds__(kThreads)
+dd_rfi_fit_kernel(const double* __restrict__ b, int nchans, int order, double* __restrict__ B,
+                  double* __restrict__ stats)
+{
+    __shared__ double red[kThreads / 32];
+    __shared__ double G[(kMaxOrder + 1) * (kMaxOrder + 2)];   // augmented [p+1][p+2]
+    __shared__ double coef[kMaxOrder + 1];
+    const int beam = blockIdx.x;
+    const double* bb = b + (int64_t)beam * nchans;
+    const int p = min(order, nchans - 1), np1 = p + 1;
+    auto absc = [&](int c) { return nchans > 1 ? 2.0 * (double)c / (double)(nchans - 1) - 1.0 : 0.0; };
+    auto legendre = [&](double x, double* P) {                // P[0..p]
+        P[0] = 1.0;
+        if (p >= 1) P[1] = x;
+        for (int k = 2; k <= p; ++k) P[k] = ((2.0 * k - 1.0) * x * P[k - 1] - (k - 1.0) * P[k - 2]) / (double)k;
+    };
+    for (int i = 0; i < np1; ++i)
+        for (int j = i; j <= np1; ++j) {                      // j == np1: right-hand side
+            double s = 0.0;
+            for (int c = threadIdx.x; c < nchans; c += kThreads) {
+                double P[kMaxOrder + 1];
+                legendre(absc(c), P);
+                s += P[i] * (j < np1 ? P[j] : bb[c]);
+            }
+            s = block_sum(s, red);
+            if (threadIdx.x == 0) {
+                G[i * (np1 + 1) + j] = s;
+                if (j < np1) G[j * (np1 + 1) + i] = s;
+            }
+        }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const int ld = np1 + 1;
+        for (int k = 0; k < np1; ++k) {
+            int piv = k;
+            for (int r = k + 1; r < np1; ++r)
+                if (fabs(G[r * ld + k]) > fabs(G[piv * ld + k])) piv = r;
+            if (piv != k)
+                for (int j = 0; j < ld; ++j) {
+                    const double tmp = G[k * ld + j];
+                    G[k * ld + j] = G[piv * ld + j];
+                    G[piv * ld + j] = tmp;
+                }
+            const double d = G[k * ld + k];
+            for (int r = k + 1; r < np1; ++r) {
+                const double f = d != 0.0 ? G[r * ld + k] / d : 0.0;
+                for (int j = k; j < ld; ++j) G[r * ld + j] -= f * G[k * ld + j];
+            }
+        }
+        for (int k = np1 - 1; k >= 0; --k) {
+            double s = G[k * ld + np1];
+            for (int j = k + 1; j < np1; ++j) s -= G[k * ld + j] * coef[j];
+            coef[k] = G[k * ld + k] != 0.0 ? s / G[k * ld + k] : 0.0;
+        }
+    }
+    __syncthreads();
+    double se = 0.0, sb = 0.0;
+    for (int c = threadIdx.x; c < nchans; c += kThreads) {
+        double P[kMaxOrder + 1];
+        legendre(absc(c), P);
+        double v = 0.0;
+        for (int k = 0; k <= p; ++k) v += coef[k] * P[k];
+        B[(int64_t)beam * nchans + c] = v;
+        se += (bb[c] - v) * (bb[c] - v);
+        sb += v;
+    }
+    se = block_sum(se, red);
+    sb = block_sum(sb, red);
+    if (threadIdx.x == 0) {
+        stats[beam * 4 + 0] = sqrt(se / (double)nchans);      // RMSE (R22)
+        stats[beam * 4 + 1] = sb / (double)nchans;            // mean of the fitted bandpass
+    }
+}
+
+// 2a. own[row][k] = |mean of window k - B_row| > T_c * RMSE   (one warp per window)
+__global__ void __launch_bounds__(kThreads)
+dd_rfi_window_kernel(const float* __restrict__ X, int nchans, int64_t n, int64_t stride, int64_t beam_stride,
+                     int window, int nwin, const double* __restrict__ B, const double* __restrict__ stats,
+                     double t_chan, uint8_t* __restrict__ own)
+{
+    const int64_t row = blockIdx.y;
+    const int beam = (int)(row / nchans);
+    const int k = blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (k >= nwin) return;
+    const float* x = X + (int64_t)beam * beam_stride + (row % nchans) * stride;
+    const int64_t a = (int64_t)k * window, e = min(n, a + window);
+    double s = 0.0;
+    for (int64_t t = a + lane; t < e; t += 32) s += (double)__ldg(x + t);
+    s = warp_sum(s);
+    if (lane == 0) own[row * nwin + k] = fabs(s / (double)(e - a) - B[row]) > t_chan * stats[beam * 4 + 0];
+}
+
+__device__ __forceinline__ bool window_flagged(const uint8_t* __restrict__ own, int k, int nwin)
+{
+    return own[k] || (k > 0 && own[k - 1]) || (k + 1 < nwin && own[k + 1]);
+}
+
+// 3a. m[beam][t] = mean over channels of the channel-clipped spectrum t (one thread per t, channels serial,
+// every load a coalesced row segment)
+__global__ void __launch_bounds__(kThreads)
+dd_rfi_spectrum_kernel(const float* __restrict__ X, int nchans, int64_t n, int64_t stride, int64_t beam_stride,
+                       int window, int nwin, const double* __restrict__ B, const uint8_t* __restrict__ own,
+                       double* __restrict__ m)
+{
+    const int beam = blockIdx.y;
+    const int64_t t = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+    if (t >= n) return;
+    const int k = (int)(t / window);
+    const float* x = X + (int64_t)beam * beam_stride + t;
+    const uint8_t* ow = own + (int64_t)beam * nchans * nwin;
+    const double* Bb = B + (int64_t)beam * nchans;
+    double s = 0.0;
+    int c = 0;
+    for (; c + 8 <= nchans; c += 8) {
+        float v[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) v[q] = __ldg(x + (int64_t)(c + q) * stride);
+#pragma unroll
+        for (int q = 0; q < 8; ++q)
+            s += window_flagged(ow + (int64_t)(c + q) * nwin, k, nwin) ? Bb[c + q] : (double)v[q];
+    }
+    for (; c < nchans; ++c)
+        s += window_flagged(ow + (int64_t)c * nwin, k, nwin) ? Bb[c] : (double)__ldg(x + (int64_t)c * stride);
+    m[(int64_t)beam * n + t] = s / (double)nchans;
+}
+
+// 3b. stats[beam][2..3] = mean and population standard deviation over time of m (one block per beam)
+__global__ void __launch_bounds__(kThreads)
+dd_rfi_spectrum_stats_kernel(const double* __restrict__ m, int64_t n, double* __restrict__ stats)
+{
+    __shared__ double red[kThreads / 32];
+    const int beam = blockIdx.x;
+    const double* mm = m + (int64_t)beam * n;
+    double s = 0.0;
+    for (int64_t t = threadIdx.x; t < n; t += kThreads) s += mm[t];
+    const double mu = block_sum(s, red) / (double)n;
+    double q = 0.0;
+    for (int64_t t = threadIdx.x; t < n; t += kThreads) q += (mm[t] - mu) * (mm[t] - mu);
+    q = block_sum(q, red);
+    if (threadIdx.x == 0) {
+        stats[beam * 4 + 2] = mu;
+        stats[beam * 4 + 3] = sqrt(q / (double)n);
+    }
+}
+
+// 4. the single write pass: channel replacement, spectrum excess, bandpass subtraction
+__global__ void __launch_bounds__(kThreads)
+dd_rfi_apply_kernel(float* __restrict__ X, int nchans, int64_t n, int64_t stride, int64_t beam_stride, int window,
+                    int nwin, const double* __restrict__ B, const double* __restrict__ stats,
+                    const uint8_t* __restrict__ own, const double* __restrict__ m, double t_spec,
+                    uint8_t* __restrict__ chan_flags, uint8_t* __restrict__ spec_flags)
+{
+    const int64_t row = blockIdx.y;
+    const int beam = (int)(row / nchans);
+    const int64_t t = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+    if (t >= n) return;
+    const int k = (int)(t / window);
+    float* x = X + (int64_t)beam * beam_stride + (row % nchans) * stride + t;
+    const double Bc = B[row];
+    const bool cf = window_flagged(own + row * nwin, k, nwin);
+    const double mt = m[(int64_t)beam * n + t];
+    const bool sf = (mt - stats[beam * 4 + 2]) > t_spec * stats[beam * 4 + 3];
+    double v = cf ? Bc : (double)*x;
+    if (sf) v -= mt - stats[beam * 4 + 1];
+    *x = (float)(v - Bc);
+    if (chan_flags && t == (int64_t)k * window) chan_flags[row * nwin + k] = cf;
+    if (spec_flags && row % nchans == 0) spec_flags[(int64_t)beam * n + t] = sf;
+}
+
+}  // namespace
+
+int rfi_mitigate(float* X, int nchans, int64_t nsamp, int64_t stride, int64_t beam_stride, int nbeams,
+                 const dd_rfi_params* prm, double* bandpass, double* fit, double* stats_out, uint8_t* chan_flags,
+                 uint8_t* spec_flags, void* cuda_stream)
+{
+    if (!prm) return fail(DD_ERR_BAD_ARG, "params is null");
+    if (nchans < 1 || nsamp < 0 || nbeams < 1) return fail(DD_ERR_BAD_ARG, "bad nchans / nsamp / nbeams");
+    if (prm->poly_order < 0 || prm->poly_order > kMaxOrder) return fail(DD_ERR_BAD_ARG, "poly_order must be 0..12");
+    if (prm->window < 1) return fail(DD_ERR_BAD_ARG, "window must be >= 1");
+    if (!(prm->t_chan >= 0.0f) || !(prm->t_spec >= 0.0f)) return fail(DD_ERR_BAD_ARG, "thresholds must be >= 0");
+    if (nsamp == 0) return DD_OK;
+    if (!X) return fail(DD_ERR_BAD_ARG, "X is null");
+    if (stride < nsamp) return fail(DD_ERR_BAD_ARG, "stride is shorter than nsamp");
+    if (nbeams > 1 && beam_stride < (int64_t)nchans * stride) return fail(DD_ERR_BAD_ARG, "beam stride is shorter than a beam");
+    const int64_t nrows = (int64_t)nbeams * nchans;
+    const int64_t nwin64 = (nsamp + prm->window - 1) / prm->window;
+    const int64_t ntile = (nsamp + kThreads - 1) / kThreads;
+    if (nrows > 65535 || nbeams > 65535 || nwin64 > 2147483647LL || ntile > 2147483647LL)
+        return fail(DD_ERR_UNSUPPORTED, "more than 65535 channel rows in one call: split the call by beam");
+    const int nwin = (int)nwin64;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (nbeams == 1) beam_stride = 0;
+    // workspace: b [nrows], B [nrows], stats [nbeams][4], m [nbeams][nsamp] (doubles), own [nrows][nwin] (bytes)
+    const size_t nd = (size_t)nrows * 2 + (size_t)nbeams * 4 + (size_t)nbeams * nsamp;
+    char* ws = nullptr;
+    int rc = workspace_alloc((void**)&ws, nd * sizeof(double) + (size_t)nrows * nwin, cuda_stream);
+    if (rc != DD_OK) return rc;
+    double* b = (double*)ws;
+    double* B = b + nrows;
+    double* stats = B + nrows;
+    double* m = stats + (size_t)nbeams * 4;
+    uint8_t* own = (uint8_t*)(m + (size_t)nbeams * nsamp);
+    dd_rfi_bandpass_kernel<<<(unsigned)nrows, kThreads, 0, st>>>(X, nchans, nsamp, stride, beam_stride, b);
+    dd_rfi_fit_kernel<<<(unsigned)nbeams, kThreads, 0, st>>>(b, nchans, prm->poly_order, B, stats);
+    dd_rfi_window_kernel<<<dim3((unsigned)((nwin + kThreads / 32 - 1) / (kThreads / 32)), (unsigned)nrows), kThreads, 0,
+                           st>>>(X, nchans, nsamp, stride, beam_stride, prm->window, nwin, B, stats,
+                                 (double)prm->t_chan, own);
+    dd_rfi_spectrum_kernel<<<dim3((unsigned)ntile, (unsigned)nbeams), kThreads, 0, st>>>(
+        X, nchans, nsamp, stride, beam_stride, prm->window, nwin, B, own, m);
+    dd_rfi_spectrum_stats_kernel<<<(unsigned)nbeams, kThreads, 0, st>>>(m, nsamp, stats);
+    dd_rfi_apply_kernel<<<dim3((unsigned)ntile, (unsigned)nrows), kThreads, 0, st>>>(
+        X, nchans, nsamp, stride, beam_stride, prm->window, nwin, B, stats, own, m, (double)prm->t_spec, chan_flags,
+        spec_flags);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && bandpass)
+        e = cudaMemcpyAsync(bandpass, b, (size_t)nrows * sizeof(double), cudaMemcpyDeviceToDevice, st);
+    if (e == cudaSuccess && fit)
+        e = cudaMemcpyAsync(fit, B, (size_t)nrows * sizeof(double), cudaMemcpyDeviceToDevice, st);
+    if (e == cudaSuccess && stats_out)
+        e = cudaMemcpyAsync(stats_out, stats, (size_t)nbeams * 4 * sizeof(double), cudaMemcpyDeviceToDevice, st);
+    cudaFreeAsync(ws, st);
+    if (e != cudaSuccess) return fail(DD_ERR_CUDA, std::string("RFI mitigation: ") + cudaGetErrorString(e));
+    return DD_OK;
+}
+
+}  // namespace dd
