@@ -254,6 +254,45 @@ int     dd_rfi_mitigate(float* X, int nchans, int64_t nsamp, int64_t stride, int
                         const dd_rfi_params* params, double* bandpass, double* fit, double* stats,
                         uint8_t* chan_flags, uint8_t* spec_flags, void* cuda_stream);
 
+/* ---- approximate variants (float32), built from the exact kernels on reduced data -----------------
+ * A. Time binning: trials with DM >= 2 DM_diag run on the input summed over
+ *    2^k adjacent samples, k = floor(log2(DM / DM_diag)) capped at max_level, with sampling time
+ *    2^k tsamp in the delay formula; DM_diag is the DM at which the delay across the LAST channel is one
+ *    sample (dd_diagonal_dm), or the caller's value.  dm_list must be non-decreasing. */
+double  dd_diagonal_dm(int nchans, double fch1, double foff, double tsamp);    /* host only; inf for 1 channel */
+/* Y[r][i] = X[r][2i] + X[r][2i+1], i < n_in / 2; X, Y: DEVICE float32 rows, strides in elements */
+int     dd_downsample2_f32(const float* X, float* Y, int64_t nrows, int64_t n_in, int64_t stride_in,
+                           int64_t stride_out, void* cuda_stream);
+typedef struct dd_timebin dd_timebin;
+int     dd_timebin_create(dd_timebin** out, int nchans, double fch1, double foff, double tsamp,
+                          const double* dm_list, int ndm, double dm_diag /* <= 0: dd_diagonal_dm */,
+                          int max_level);
+void    dd_timebin_destroy(dd_timebin* t);
+/* number of levels; level_of_trial (HOST int32 [ndm], may be NULL) receives k per trial */
+int     dd_timebin_levels(const dd_timebin* t, int32_t* level_of_trial);
+/* full-rate samples every input row must hold for nsamp_out (full-rate) output samples */
+int64_t dd_timebin_input_samples(const dd_timebin* t, int64_t nsamp_out);
+/* X: DEVICE [nchans][n_in] (stride in_stride); D: DEVICE [ndm][out_stride]: row d receives
+ * nsamp_out >> level(d) samples, sample i covering full-rate samples [2^k i, 2^k (i+1)); the rest of
+ * the row is not written. */
+int     dd_timebin_execute(dd_timebin* t, const float* X, int64_t in_stride, int64_t n_in, float* D,
+                           int64_t out_stride, int64_t nsamp_out, void* cuda_stream);
+
+/* B. Subband dedispersion (§2.1.3).  Step 1: every block of chans_per_subband channels is
+ *    dedispersed as a filterbank of its own (reference = its first channel) at one nominal DM per block
+ *    of dms_per_nominal consecutive trials (the block's middle trial).  Step 2: for every nominal DM the
+ *    subband series form a filterbank of ceil(nchans / chans_per_subband) channels (fch1' = fch1,
+ *    foff' = chans_per_subband * foff) that is dedispersed at each trial of the block.  dm_list must be
+ *    non-decreasing.  Input rows must hold nsamp_out + dd_subband_max_shift samples. */
+typedef struct dd_subband dd_subband;
+int     dd_subband_create(dd_subband** out, int nchans, double fch1, double foff, double tsamp,
+                          const double* dm_list, int ndm, int chans_per_subband, int dms_per_nominal);
+void    dd_subband_destroy(dd_subband* s);
+int64_t dd_subband_max_shift(const dd_subband* s);
+/* X: DEVICE [nchans][in_stride]; D: DEVICE [ndm][out_stride], rows in dm_list order */
+int     dd_subband_execute(dd_subband* s, const float* X, int64_t in_stride, float* D, int64_t out_stride,
+                           int64_t nsamp_out, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

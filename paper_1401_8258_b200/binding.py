@@ -67,6 +67,19 @@ SIGNATURES = {
                                  C.POINTER(_i64)]),
     "dd_rfi_mitigate": (C.c_int, [_vp, C.c_int, _i64, _i64, _i64, C.c_int, C.POINTER(dd_rfi_params), _vp, _vp, _vp,
                                   _vp, _vp, _vp]),
+    "dd_diagonal_dm": (C.c_double, [C.c_int, C.c_double, C.c_double, C.c_double]),
+    "dd_downsample2_f32": (C.c_int, [_vp, _vp, _i64, _i64, _i64, _i64, _vp]),
+    "dd_timebin_create": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_double, C.c_double, C.c_double, _dp, C.c_int,
+                                    C.c_double, C.c_int]),
+    "dd_timebin_destroy": (None, [_vp]),
+    "dd_timebin_levels": (C.c_int, [_vp, _vp]),
+    "dd_timebin_input_samples": (_i64, [_vp, _i64]),
+    "dd_timebin_execute": (C.c_int, [_vp, _vp, _i64, _i64, _vp, _i64, _i64, _vp]),
+    "dd_subband_create": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_double, C.c_double, C.c_double, _dp, C.c_int,
+                                    C.c_int, C.c_int]),
+    "dd_subband_destroy": (None, [_vp]),
+    "dd_subband_max_shift": (_i64, [_vp]),
+    "dd_subband_execute": (C.c_int, [_vp, _vp, _i64, _vp, _i64, _i64, _vp]),
     "dd_stream_create": (C.c_int, [C.POINTER(_vp), _vp, _i64, C.c_int]),
     "dd_stream_push": (C.c_int, [_vp, _vp, _i64, _i64, _i64, _vp, _i64, _i64, C.POINTER(_i64), _vp]),
     "dd_stream_reset": (C.c_int, [_vp]),
@@ -293,3 +306,69 @@ class Stream:
 
     def reset(self) -> None:
         _check(lib().dd_stream_reset(self._h), "dd_stream_reset")
+
+
+# ------------------------------------------------------------------ approximate variants (f2)
+
+def dd_diagonal_dm(nchans, fch1, foff, tsamp) -> float:
+    return float(lib().dd_diagonal_dm(nchans, fch1, foff, tsamp))
+
+
+def dd_downsample2_f32(X, Y, nrows, n_in, stride_in, stride_out, stream=None) -> None:
+    _check(lib().dd_downsample2_f32(_ptr(X), _ptr(Y), nrows, n_in, stride_in, stride_out, _stream_ptr(stream)),
+           "dd_downsample2_f32")
+
+
+class TimeBin:
+    """Owns a ``dd_timebin*`` (time-binned dedispersion)."""
+
+    def __init__(self, nchans, fch1, foff, tsamp, dm_list, dm_diag=0.0, max_level=8):
+        a, p, n = _dms(dm_list)
+        h = _vp()
+        _check(lib().dd_timebin_create(C.byref(h), nchans, fch1, foff, tsamp, p, n, dm_diag, max_level),
+               "dd_timebin_create")
+        self._h, self.ndm = h, n
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib().dd_timebin_destroy(self._h)
+            self._h = None
+
+    __del__ = destroy
+
+    def levels(self) -> np.ndarray:
+        out = np.zeros(self.ndm, dtype=np.int32)
+        _check(lib().dd_timebin_levels(self._h, out.ctypes.data), "dd_timebin_levels")
+        return out
+
+    def input_samples(self, nsamp_out) -> int:
+        return _check(lib().dd_timebin_input_samples(self._h, nsamp_out), "dd_timebin_input_samples")
+
+    def execute(self, X, in_stride, n_in, D, out_stride, nsamp_out, stream=None) -> None:
+        _check(lib().dd_timebin_execute(self._h, _ptr(X), in_stride, n_in, _ptr(D), out_stride, nsamp_out,
+                                        _stream_ptr(stream)), "dd_timebin_execute")
+
+
+class Subband:
+    """Owns a ``dd_subband*`` (two-step subband dedispersion)."""
+
+    def __init__(self, nchans, fch1, foff, tsamp, dm_list, chans_per_subband, dms_per_nominal):
+        a, p, n = _dms(dm_list)
+        h = _vp()
+        _check(lib().dd_subband_create(C.byref(h), nchans, fch1, foff, tsamp, p, n, chans_per_subband,
+                                       dms_per_nominal), "dd_subband_create")
+        self._h, self.ndm = h, n
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib().dd_subband_destroy(self._h)
+            self._h = None
+
+    __del__ = destroy
+
+    def max_shift(self) -> int:
+        return _check(lib().dd_subband_max_shift(self._h), "dd_subband_max_shift")
+
+    def execute(self, X, in_stride, D, out_stride, nsamp_out, stream=None) -> None:
+        _check(lib().dd_subband_execute(self._h, _ptr(X), in_stride, _ptr(D), out_stride, nsamp_out,
+                                        _stream_ptr(stream)), "dd_subband_execute")
