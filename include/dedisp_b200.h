@@ -293,6 +293,20 @@ int64_t dd_subband_max_shift(const dd_subband* s);
 int     dd_subband_execute(dd_subband* s, const float* X, int64_t in_stride, float* D, int64_t out_stride,
                            int64_t nsamp_out, void* cuda_stream);
 
+/* ---- coherent multi-beam beamformer (ch. 5: eq 5.1, Alg. 2) feeding the dedisperser
+ * on the device.  b(f, t, beam) = sum_a W[f][beam][a] * v[f][t][a]; output = detected power |b|^2.
+ * V: DEVICE uint8 [nchans][nsamp][nants] (antenna fastest, four antennas per 32-bit word);
+ *    each byte: low nibble = real part, high nibble = imaginary part, 4-bit two's complement (-8..7);
+ *    nants must be a multiple of 4.
+ * W: DEVICE float32 pairs (re, im), [nchans][nbeams][nants]: the weights that point the beams, fixed over
+ *    the buffer; no conjugation is applied.
+ * P: DEVICE float32 [nbeams][nchans][nsamp] with strides out_stride (channel rows) and out_beam_stride,
+ *    i.e. exactly the X layout of dd_execute with nbeams beams.
+ * The products run on the tensor cores (fp16 operands -- the 4-bit voltages exactly, the weights as two
+ * fp16 terms -- with float32 accumulation): |P - exact| <= 1e-5 (sum_a |W||v|)^2.  Enqueued on cuda_stream. */
+int     dd_beamform_power_u4(const uint8_t* V, int nants, int nchans, int64_t nsamp, const float* W, int nbeams,
+                             float* P, int64_t out_stride, int64_t out_beam_stride, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -80,6 +80,7 @@ SIGNATURES = {
     "dd_subband_destroy": (None, [_vp]),
     "dd_subband_max_shift": (_i64, [_vp]),
     "dd_subband_execute": (C.c_int, [_vp, _vp, _i64, _vp, _i64, _i64, _vp]),
+    "dd_beamform_power_u4": (C.c_int, [_vp, C.c_int, C.c_int, _i64, _vp, C.c_int, _vp, _i64, _i64, _vp]),
     "dd_stream_create": (C.c_int, [C.POINTER(_vp), _vp, _i64, C.c_int]),
     "dd_stream_push": (C.c_int, [_vp, _vp, _i64, _i64, _i64, _vp, _i64, _i64, C.POINTER(_i64), _vp]),
     "dd_stream_reset": (C.c_int, [_vp]),
@@ -212,6 +213,11 @@ def dd_rfi_mitigate(X, nchans, nsamp, stride, beam_stride, nbeams, params, bandp
     _check(lib().dd_rfi_mitigate(_ptr(X), nchans, nsamp, stride, beam_stride, nbeams, C.byref(params), _ptr(bandpass),
                                  _ptr(fit), _ptr(stats), _ptr(chan_flags), _ptr(spec_flags), _stream_ptr(stream)),
            "dd_rfi_mitigate")
+
+
+def dd_beamform_power_u4(V, nants, nchans, nsamp, W, nbeams, P, out_stride, out_beam_stride, stream=None) -> None:
+    _check(lib().dd_beamform_power_u4(_ptr(V), nants, nchans, nsamp, _ptr(W), nbeams, _ptr(P), out_stride,
+                                      out_beam_stride, _stream_ptr(stream)), "dd_beamform_power_u4")
 
 
 def dd_postprocess_launches(params, want_series) -> int:

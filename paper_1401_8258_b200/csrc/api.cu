@@ -624,6 +624,14 @@ int dd_rfi_mitigate(float* X, int nchans, int64_t nsamp, int64_t stride, int64_t
                         spec_flags, cuda_stream);
 }
 
+int dd_beamform_power_u4(const uint8_t* V, int nants, int nchans, int64_t nsamp, const float* W, int nbeams, float* P,
+                         int64_t out_stride, int64_t out_beam_stride, void* cuda_stream)
+{
+    int rc = require_sm100(nullptr);
+    if (rc != DD_OK) return rc;
+    return beamform_power_u4(V, nants, nchans, nsamp, W, nbeams, P, out_stride, out_beam_stride, cuda_stream);
+}
+
 int dd_search_host(dd_plan* p, const void* X, int64_t in_stride, int64_t in_beam_stride, int64_t nsamp_out,
                    int nbeams, const dd_post_params* params, dd_candidate* cand, int64_t capacity, int64_t* count)
 {
