@@ -478,6 +478,12 @@ def run_ours(args, w):
                             "without the per-call host launch cost that bounds ms_per_step above"}
             c.close()
         line["per_config"] = per
+        hbm_peak = None
+        try:
+            hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs")
+        except (OSError, ValueError):
+            pass
+        line["next_rows"] = next_rows(dd, torch, hbm_peak)
 
     if rank == 0:
         if not args.no_cpu:
@@ -496,6 +502,93 @@ def finish_timing(total_ms, steps, units_per_rank, world, dist, device):
     total_ms = sharding.max_over_ranks(total_ms, dist, device)
     ms_per_step = total_ms / steps
     return ms_per_step, sharding.whole_job_rate(units_per_rank, world, ms_per_step * 1e-3) / 1e9
+
+
+def _timed_ms(torch, fn, reps=5, warm=2):
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(reps):
+        fn()
+    b.record()
+    torch.cuda.synchronize()
+    return a.elapsed_time(b) / reps
+
+
+def next_rows(dd, torch, hbm_peak):
+    """The SURVEY 8(f) rows beside the hot path, each timed on the device at a BASELINE.json-sized shape with
+    its own roofline: f1 / f3 / f4 are HBM-bound streaming kernels (achieved = algorithmic bytes / time against
+    the measured HBM copy bandwidth), f2 is reported as its speed-up over the exact kernel on the same input."""
+    rows = {}
+    peak = hbm_peak or 6453.4
+    g = torch.Generator(device="cuda").manual_seed(1401)
+    # f1: post-processing of config 3's (DM, t) plane, candidates only
+    w = synth.WORKLOADS[3]
+    D = torch.randn((w.ndm, w.nsamp), dtype=torch.float32, device="cuda", generator=g)
+    cap = 1 << 20
+    cand = torch.zeros(4 * cap, dtype=torch.int32, device="cuda")
+    cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    prm = dd.post_params(5, True, True, nsigma=6.0)
+    ms = _timed_ms(torch, lambda: dd.dd_postprocess(dd.DD_F32, D, w.nsamp, 0, w.ndm, w.nsamp, 1, prm, None, 0, 0, None,
+                                                    cand, cap, cnt))
+    by = D.numel() * 4
+    rows["f1_postprocess"] = {"shape": "config 3 output, %d series x %d samples float32; median 5, detrend, normalise, 6 sigma -> candidates" % (w.ndm, w.nsamp),
+                              "ms": ms, "algorithmic_bytes": by, "bound": "hbm", "achieved_gbs": by / ms / 1e6,
+                              "peak_gbs": peak, "frac": by / ms / 1e6 / peak, "gpu_launches": dd.dd_postprocess_launches(prm, False),
+                              "note": "algorithmic = D read once; the kernels read it three times (fit pass 1, pass 2, apply), twice through L2 for rows that fit"}
+    del D
+    # f3: RFI mitigation of config 3's input buffer, in place
+    n_in = w.nsamp + 14845
+    X = torch.randn((w.nchans, n_in), dtype=torch.float32, device="cuda", generator=g).add_(20.0)
+    rp = dd.dd_rfi_params(4, 512, 7.0, 5.0)
+    ms = _timed_ms(torch, lambda: dd.dd_rfi_mitigate(X, w.nchans, n_in, n_in, 0, 1, rp))
+    by = X.numel() * 8
+    rows["f3_rfi"] = {"shape": "config 3 input, %d channels x %d samples float32; order 4, window 512, thresholds 7 / 5" % (w.nchans, n_in),
+                      "ms": ms, "algorithmic_bytes": by, "bound": "hbm", "achieved_gbs": by / ms / 1e6, "peak_gbs": peak,
+                      "frac": by / ms / 1e6 / peak, "gpu_launches": 6,
+                      "note": "algorithmic = X read once + written once; the kernels read it four times (row means, window means, spectrum means, apply)"}
+    del X
+    # f4: beamformer, BEST-II parameters of PAPER.md:1653 (32 antennas, 1024 channels, 16 beams) over 2^16 samples
+    na, nch, nb, nt = 32, 1024, 16, 1 << 16
+    V = torch.randint(0, 256, (nch, nt, na), dtype=torch.uint8, device="cuda", generator=g)
+    W = torch.randn((nch, nb, na, 2), dtype=torch.float32, device="cuda", generator=g)
+    P = torch.empty((nb, nch, nt), dtype=torch.float32, device="cuda")
+    ms = _timed_ms(torch, lambda: dd.dd_beamform_power_u4(V, na, nch, nt, W, nb, P, nt, nch * nt))
+    by = V.numel() + P.numel() * 4
+    flops = 8.0 * na * nb * nch * nt
+    rows["f4_beamformer"] = {"shape": "%d antennas (4-bit complex) x %d channels x %d samples -> %d beams, detected power float32" % (na, nch, nt, nb),
+                             "ms": ms, "algorithmic_bytes": by, "bound": "hbm", "achieved_gbs": by / ms / 1e6, "peak_gbs": peak,
+                             "frac": by / ms / 1e6 / peak, "tflops": flops / ms / 1e9, "gpu_launches": 2,
+                             "note": "8 Na Nb flops per (channel, sample) on the tensor cores (mma.sync fp16 x2, fp32 accumulate)"}
+    del V, W, P
+    # f2: subband (32 channels per subband, 16 trials per nominal DM) vs the exact kernel, config 2's shape as float32
+    w2 = synth.scaled(synth.WORKLOADS[2], dtype="f32")
+    sb = dd.Subband(w2.nchans, w2.fch1, w2.foff, w2.tsamp, w2.dm_list, 32, 16)
+    total = (w2.nsamp + sb.max_shift() + 63) // 64 * 64
+    X = torch.randn((w2.nchans, total), dtype=torch.float32, device="cuda", generator=g)
+    D = torch.empty((w2.ndm, w2.nsamp), dtype=torch.float32, device="cuda")
+    ms_sb = _timed_ms(torch, lambda: sb.execute(X, total, D, w2.nsamp, w2.nsamp), reps=3, warm=1)
+    plan = dd.Plan(dd.DD_F32, w2.nchans, w2.fch1, w2.foff, w2.tsamp, w2.dm_list)
+    ms_ex = _timed_ms(torch, lambda: plan.execute(X, total, 0, D, w2.nsamp, 0, w2.nsamp, 1), reps=3, warm=1)
+    rows["f2_subband"] = {"shape": "config 2's shape as float32 (1024 ch x 1024 trials x 2^17 samples), 32 channels per subband, 16 trials per nominal DM",
+                          "ms": ms_sb, "exact_ms": ms_ex, "speedup_over_exact": ms_ex / ms_sb,
+                          "adds_ratio": (w2.nchans * 64 + 32 * w2.ndm) / (w2.nchans * w2.ndm),
+                          "note": "approximate method (PAPER.md:823): same kernels on reduced data; 96 plans, 96 launches"}
+    sb.destroy(); plan.destroy()
+    tb = dd.TimeBin(w2.nchans, w2.fch1, w2.foff, w2.tsamp, w2.dm_list * 8.0, 0.0, 8)       # DMs up to 818: four levels
+    n_in = tb.input_samples(w2.nsamp)
+    n_in_p = (n_in + 63) // 64 * 64
+    X = torch.randn((w2.nchans, n_in_p), dtype=torch.float32, device="cuda", generator=g)
+    ms_tb = _timed_ms(torch, lambda: tb.execute(X, n_in_p, n_in, D, w2.nsamp, w2.nsamp), reps=3, warm=1)
+    plan = dd.Plan(dd.DD_F32, w2.nchans, w2.fch1, w2.foff, w2.tsamp, w2.dm_list * 8.0)
+    ms_ex = _timed_ms(torch, lambda: plan.execute(X, n_in_p, 0, D, w2.nsamp, 0, w2.nsamp, 1), reps=3, warm=1)
+    rows["f2_timebin"] = {"shape": "1024 ch x 1024 trials (DM 0..818, step 0.8) x 2^17 samples float32, levels %s" % sorted(set(tb.levels().tolist())),
+                          "ms": ms_tb, "exact_ms": ms_ex, "speedup_over_exact": ms_ex / ms_tb,
+                          "note": "approximate method (PAPER.md:736, 813-819): trials above 2 DM_diag on input summed over 2^k samples"}
+    tb.destroy(); plan.destroy()
+    return rows
 
 
 def empty_launch_us(torch, n=200):

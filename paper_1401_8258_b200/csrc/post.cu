@@ -10,16 +10,15 @@
 //   3. division by that standard deviation (pass 3);
 //   4. threshold at n sigma -> (time, DM, intensity) triplets per beam.
 //
-// Two kernels.  dd_post_stats_kernel: one block per series; pass 1 accumulates sum y and
-// sum (t - tm) y in double (the median is formed on the fly from the raw series, never stored),
-// the block reduces, pass 2 re-reads the series (the row, <= 1 MB, comes back from L2) and
-// accumulates sum r^2 of the residual about the fitted line -- the thesis' two passes, literally,
-// so a constant series gives sigma = 0 exactly.  dd_post_apply_kernel: grid over (time tiles,
-// series); every thread forms four consecutive medians from 4 + (w - 1) loaded samples,
-// subtracts the line, scales, optionally stores the processed series (16-byte stores) and
-// appends the samples above the threshold to the candidate list through an atomic cursor.
-// HBM traffic: D is read three times (twice through L2 for rows that fit) and written at most
-// once, against seven passes for the step-by-step pipeline of §3.5; the kernels are HBM-bound.
+// Two kernels.  dd_post_stats_kernel: one block per series, ONE pass: sum u, sum (t - tm) u and
+// sum u^2 of u = y - y_0 in double (the median is formed on the fly from the raw series, never
+// stored); slope, intercept and the residual's standard deviation follow from the normal equations
+// (the thesis' two passes give the same numbers; the offset y_0 keeps a constant series at sigma = 0
+// exactly).  dd_post_apply_kernel: grid over (time tiles, series); every thread forms four
+// consecutive medians from 4 + (w - 1) loaded samples, subtracts the line, scales, optionally stores
+// the processed series (16-byte stores) and appends the samples above the threshold to the
+// candidate list through an atomic cursor.  HBM traffic: D is read twice and written at most once,
+// against seven passes for the step-by-step pipeline of §3.5; the kernels are HBM-bound.
 // The thesis used one kernel per step with the series staged in shared memory.
 #include <cuda_runtime.h>
 
@@ -58,11 +57,17 @@ __device__ __forceinline__ void medians4(const T* __restrict__ row, int64_t t0, 
 {
     constexpr int H = (W - 1) / 2;
     T x[kPer + 2 * H];
+    if (t0 >= H && t0 + kPer + H <= n) {                  // interior: no clamping
+        const T* src = row + (t0 - H);
 #pragma unroll
-    for (int i = 0; i < kPer + 2 * H; ++i) {
-        int64_t j = t0 - H + i;
-        j = j < 0 ? 0 : (j > n - 1 ? n - 1 : j);
-        x[i] = __ldg(row + j);
+        for (int i = 0; i < kPer + 2 * H; ++i) x[i] = __ldg(src + i);
+    } else {
+#pragma unroll
+        for (int i = 0; i < kPer + 2 * H; ++i) {
+            int64_t j = t0 - H + i;
+            j = j < 0 ? 0 : (j > n - 1 ? n - 1 : j);
+            x[i] = __ldg(row + j);
+        }
     }
 #pragma unroll
     for (int e = 0; e < kPer; ++e) {
@@ -88,7 +93,10 @@ __device__ __forceinline__ double block_sum(double v, double* red)
 }
 
 // stats[row] = (intercept, slope, sigma): least-squares line through (t, y_t), t = 0..n-1, of the
-// median-filtered series and the population standard deviation of the residual.
+// median-filtered series and the population standard deviation of the residual, from ONE pass:
+// with u_t = y_t - y_0 (the offset removes the level, so a constant series gives exact zeros) and
+// tc = t - (n-1)/2,  slope = sum tc u / sum tc^2,  mean = y_0 + sum u / n,
+// SS_res = sum u^2 - (sum u)^2 / n - slope^2 sum tc^2  (the normal equations' residual), all in double.
 template <typename T, int W>
 __global__ void __launch_bounds__(kThreads)
 dd_post_stats_kernel(const T* __restrict__ D, int64_t stride, int64_t beam_stride, int ndm, int64_t n,
@@ -98,37 +106,34 @@ dd_post_stats_kernel(const T* __restrict__ D, int64_t stride, int64_t beam_strid
     const int64_t r = blockIdx.x;
     const T* row = D + (r / ndm) * beam_stride + (r % ndm) * stride;
     const double tm = 0.5 * (double)(n - 1);
-    double sy = 0.0, sty = 0.0;
+    double first[kPer];
+    medians4<T, W>(row, 0, n, first);
+    const double y0 = first[0];
+    double su = 0.0, stu = 0.0, suu = 0.0;
     for (int64_t t0 = (int64_t)threadIdx.x * kPer; t0 < n; t0 += kTile) {
         double m[kPer];
         medians4<T, W>(row, t0, n, m);
 #pragma unroll
         for (int e = 0; e < kPer; ++e)
             if (t0 + e < n) {
-                sy += m[e];
-                sty += ((double)(t0 + e) - tm) * m[e];
+                const double u = m[e] - y0;
+                su += u;
+                stu += ((double)(t0 + e) - tm) * u;
+                suu += u * u;
             }
     }
-    sy = block_sum(sy, red);
-    sty = block_sum(sty, red);
-    const double dn = (double)n;
-    const double stt = dn * (dn * dn - 1.0) / 12.0;       // sum (t - tm)^2
-    const double slope = stt > 0.0 ? sty / stt : 0.0;
-    const double intercept = sy / dn - slope * tm;
-    double ss = 0.0;
-    for (int64_t t0 = (int64_t)threadIdx.x * kPer; t0 < n; t0 += kTile) {
-        double m[kPer];
-        medians4<T, W>(row, t0, n, m);
-#pragma unroll
-        for (int e = 0; e < kPer; ++e)
-            if (t0 + e < n) {
-                const double res = m[e] - (intercept + slope * (double)(t0 + e));
-                ss += res * res;
-            }
-    }
-    ss = block_sum(ss, red);
+    su = block_sum(su, red);
+    stu = block_sum(stu, red);
+    suu = block_sum(suu, red);
     if (threadIdx.x == 0) {
-        stats[r * 3 + 0] = intercept;
+        const double dn = (double)n;
+        const double stt = dn * (dn * dn - 1.0) / 12.0;   // sum (t - tm)^2
+        const double slope = stt > 0.0 ? stu / stt : 0.0;
+        const double ss_tot = suu - su * su / dn;
+        double ss = ss_tot - slope * slope * stt;
+        // a series that is a straight line to rounding (ss / ss_tot ~ 1e-16) has no residual to normalise
+        if (!(ss > 1e-24 * fmax(ss_tot, suu))) ss = 0.0;
+        stats[r * 3 + 0] = y0 + su / dn - slope * tm;
         stats[r * 3 + 1] = slope;
         stats[r * 3 + 2] = sqrt(ss / dn);
     }

@@ -13,8 +13,7 @@
 // normal equations in a Legendre basis in double precision) and the replacements are never written as
 // such: the window flags and the spectrum excesses are small side arrays, applied when the single
 // output pass subtracts the bandpass.  Passes over X: three reads (row means, window means, spectrum
-// means of the clipped data) and one read + write -- all HBM-bound streaming kernels, 16-byte loads
-// where the row alignment allows.  All means, the fit and the threshold comparisons are evaluated in
+// means of the clipped data) and one read + write -- all HBM-bound streaming kernels.  All means, the fit and the threshold comparisons are evaluated in
 // double precision; the output is rounded once, from double, to float32.
 #include <cuda_runtime.h>
 
@@ -158,38 +157,60 @@ dd_rfi_window_kernel(const float* __restrict__ X, int nchans, int64_t n, int64_t
     if (lane == 0) own[row * nwin + k] = fabs(s / (double)(e - a) - B[row]) > t_chan * stats[beam * 4 + 0];
 }
 
-__device__ __forceinline__ bool window_flagged(const uint8_t* __restrict__ own, int k, int nwin)
+// 2b. flag[row][k] = own[k-1] | own[k] | own[k+1]  ("neighbouring blocks are also flagged", R24)
+__global__ void __launch_bounds__(kThreads)
+dd_rfi_flags_kernel(const uint8_t* __restrict__ own, int64_t nrows, int nwin, uint8_t* __restrict__ flag)
 {
-    return own[k] || (k > 0 && own[k - 1]) || (k + 1 < nwin && own[k + 1]);
+    const int64_t total = nrows * nwin;
+    for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < total; i += (int64_t)gridDim.x * kThreads) {
+        const int k = (int)(i % nwin);
+        flag[i] = own[i] | (k > 0 ? own[i - 1] : 0) | (k + 1 < nwin ? own[i + 1] : 0);
+    }
 }
 
-// 3a. m[beam][t] = mean over channels of the channel-clipped spectrum t (one thread per t, channels serial,
-// every load a coalesced row segment)
-__global__ void __launch_bounds__(kThreads)
+constexpr int kSpecT = 128;                   // spectra per block of the spectrum-mean kernel
+constexpr int kSpecQ = kThreads * 4 / kSpecT; // channel slices per block (threads = kSpecT x kSpecQ)
+
+// 3a. m[beam][t] = mean over channels of the channel-clipped spectrum t.  Block = 128 spectra x 8 channel
+// slices; a thread sums its slice's channels in ascending order (every load a coalesced row segment), the
+// slices' partial sums meet in shared memory and are added in slice order.
+__global__ void __launch_bounds__(kSpecT * kSpecQ)
 dd_rfi_spectrum_kernel(const float* __restrict__ X, int nchans, int64_t n, int64_t stride, int64_t beam_stride,
-                       int window, int nwin, const double* __restrict__ B, const uint8_t* __restrict__ own,
+                       int window, int nwin, const double* __restrict__ B, const uint8_t* __restrict__ flag,
                        double* __restrict__ m)
 {
-    const int beam = blockIdx.y;
-    const int64_t t = (int64_t)blockIdx.x * kThreads + threadIdx.x;
-    if (t >= n) return;
-    const int k = (int)(t / window);
-    const float* x = X + (int64_t)beam * beam_stride + t;
-    const uint8_t* ow = own + (int64_t)beam * nchans * nwin;
+    __shared__ double part[kSpecQ][kSpecT];
+    const int beam = blockIdx.y, tx = threadIdx.x, q = threadIdx.y;
+    const int64_t t = (int64_t)blockIdx.x * kSpecT + tx;
+    const int64_t tc = min(t, n - 1);
+    const int k = (int)(tc / window);
+    const float* x = X + (int64_t)beam * beam_stride + tc;
+    const uint8_t* fl = flag + (int64_t)beam * nchans * nwin + k;
     const double* Bb = B + (int64_t)beam * nchans;
+    const int cq = (nchans + kSpecQ - 1) / kSpecQ;
+    const int c_lo = min(nchans, q * cq), c_hi = min(nchans, c_lo + cq);
     double s = 0.0;
-    int c = 0;
-    for (; c + 8 <= nchans; c += 8) {
+    int c = c_lo;
+    for (; c + 8 <= c_hi; c += 8) {
         float v[8];
+        uint8_t f[8];
 #pragma unroll
-        for (int q = 0; q < 8; ++q) v[q] = __ldg(x + (int64_t)(c + q) * stride);
+        for (int j = 0; j < 8; ++j) {
+            v[j] = __ldg(x + (int64_t)(c + j) * stride);
+            f[j] = __ldg(fl + (int64_t)(c + j) * nwin);
+        }
 #pragma unroll
-        for (int q = 0; q < 8; ++q)
-            s += window_flagged(ow + (int64_t)(c + q) * nwin, k, nwin) ? Bb[c + q] : (double)v[q];
+        for (int j = 0; j < 8; ++j) s += f[j] ? Bb[c + j] : (double)v[j];
     }
-    for (; c < nchans; ++c)
-        s += window_flagged(ow + (int64_t)c * nwin, k, nwin) ? Bb[c] : (double)__ldg(x + (int64_t)c * stride);
-    m[(int64_t)beam * n + t] = s / (double)nchans;
+    for (; c < c_hi; ++c) s += __ldg(fl + (int64_t)c * nwin) ? Bb[c] : (double)__ldg(x + (int64_t)c * stride);
+    part[q][tx] = s;
+    __syncthreads();
+    if (q == 0 && t < n) {
+        double tot = part[0][tx];
+#pragma unroll
+        for (int j = 1; j < kSpecQ; ++j) tot += part[j][tx];
+        m[(int64_t)beam * n + t] = tot / (double)nchans;
+    }
 }
 
 // 3b. stats[beam][2..3] = mean and population standard deviation over time of m (one block per beam)
@@ -211,28 +232,58 @@ dd_rfi_spectrum_stats_kernel(const double* __restrict__ m, int64_t n, double* __
     }
 }
 
-// 4. the single write pass: channel replacement, spectrum excess, bandpass subtraction
+// 4. the single write pass: channel replacement, spectrum excess, bandpass subtraction; four consecutive
+// samples per thread (16-byte accesses when the row allows)
 __global__ void __launch_bounds__(kThreads)
 dd_rfi_apply_kernel(float* __restrict__ X, int nchans, int64_t n, int64_t stride, int64_t beam_stride, int window,
                     int nwin, const double* __restrict__ B, const double* __restrict__ stats,
-                    const uint8_t* __restrict__ own, const double* __restrict__ m, double t_spec,
+                    const uint8_t* __restrict__ flag, const double* __restrict__ m, double t_spec,
                     uint8_t* __restrict__ chan_flags, uint8_t* __restrict__ spec_flags)
 {
     const int64_t row = blockIdx.y;
     const int beam = (int)(row / nchans);
-    const int64_t t = (int64_t)blockIdx.x * kThreads + threadIdx.x;
-    if (t >= n) return;
-    const int k = (int)(t / window);
-    float* x = X + (int64_t)beam * beam_stride + (row % nchans) * stride + t;
-    const double Bc = B[row];
-    const bool cf = window_flagged(own + row * nwin, k, nwin);
-    const double mt = m[(int64_t)beam * n + t];
-    const bool sf = (mt - stats[beam * 4 + 2]) > t_spec * stats[beam * 4 + 3];
-    double v = cf ? Bc : (double)*x;
-    if (sf) v -= mt - stats[beam * 4 + 1];
-    *x = (float)(v - Bc);
-    if (chan_flags && t == (int64_t)k * window) chan_flags[row * nwin + k] = cf;
-    if (spec_flags && row % nchans == 0) spec_flags[(int64_t)beam * n + t] = sf;
+    const int64_t t0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4;
+    if (t0 >= n) return;
+    float* x = X + (int64_t)beam * beam_stride + (row % nchans) * stride + t0;
+    const double Bc = B[row], mu = stats[beam * 4 + 2], level = t_spec * stats[beam * 4 + 3], bmean = stats[beam * 4 + 1];
+    const double* mt = m + (int64_t)beam * n + t0;
+    const uint8_t* fl = flag + row * nwin;
+    int k = (int)(t0 / window);
+    int64_t next = (int64_t)(k + 1) * window;              // first sample of the next window
+    const bool vec = t0 + 4 <= n && ((((uintptr_t)x) & 15) == 0);
+    float v[4];
+    if (vec) {
+        const float4 q = *reinterpret_cast<const float4*>(x);
+        v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
+    } else {
+#pragma unroll
+        for (int e = 0; e < 4; ++e) v[e] = t0 + e < n ? x[e] : 0.0f;
+    }
+    bool cf = fl[k];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        const int64_t t = t0 + e;
+        if (t >= n) break;
+        if (t >= next) {
+            ++k;
+            next += window;
+            cf = fl[k];
+        }
+        const double me = mt[e];
+        const bool sf = (me - mu) > level;
+        double val = cf ? Bc : (double)v[e];
+        if (sf) val -= me - bmean;
+        v[e] = (float)(val - Bc);
+        if (chan_flags && t == (int64_t)k * window) chan_flags[row * nwin + k] = cf;
+        if (spec_flags && row % nchans == 0) spec_flags[(int64_t)beam * n + t] = sf;
+    }
+    if (vec) {
+        *reinterpret_cast<float4*>(x) = make_float4(v[0], v[1], v[2], v[3]);
+    } else {
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+            if (t0 + e < n) x[e] = v[e];
+    }
 }
 
 }  // namespace
@@ -252,32 +303,36 @@ int rfi_mitigate(float* X, int nchans, int64_t nsamp, int64_t stride, int64_t be
     if (nbeams > 1 && beam_stride < (int64_t)nchans * stride) return fail(DD_ERR_BAD_ARG, "beam stride is shorter than a beam");
     const int64_t nrows = (int64_t)nbeams * nchans;
     const int64_t nwin64 = (nsamp + prm->window - 1) / prm->window;
-    const int64_t ntile = (nsamp + kThreads - 1) / kThreads;
-    if (nrows > 65535 || nbeams > 65535 || nwin64 > 2147483647LL || ntile > 2147483647LL)
+    const int64_t ntile = (nsamp + 4 * kThreads - 1) / (4 * kThreads);
+    const int64_t nspec = (nsamp + kSpecT - 1) / kSpecT;
+    if (nrows > 65535 || nbeams > 65535 || nwin64 > 2147483647LL || nspec > 2147483647LL)
         return fail(DD_ERR_UNSUPPORTED, "more than 65535 channel rows in one call: split the call by beam");
     const int nwin = (int)nwin64;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (nbeams == 1) beam_stride = 0;
-    // workspace: b [nrows], B [nrows], stats [nbeams][4], m [nbeams][nsamp] (doubles), own [nrows][nwin] (bytes)
+    // workspace: b [nrows], B [nrows], stats [nbeams][4], m [nbeams][nsamp] (doubles), own and flag [nrows][nwin] (bytes)
     const size_t nd = (size_t)nrows * 2 + (size_t)nbeams * 4 + (size_t)nbeams * nsamp;
     char* ws = nullptr;
-    int rc = workspace_alloc((void**)&ws, nd * sizeof(double) + (size_t)nrows * nwin, cuda_stream);
+    int rc = workspace_alloc((void**)&ws, nd * sizeof(double) + (size_t)2 * nrows * nwin, cuda_stream);
     if (rc != DD_OK) return rc;
     double* b = (double*)ws;
     double* B = b + nrows;
     double* stats = B + nrows;
     double* m = stats + (size_t)nbeams * 4;
     uint8_t* own = (uint8_t*)(m + (size_t)nbeams * nsamp);
+    uint8_t* flag = own + (size_t)nrows * nwin;
     dd_rfi_bandpass_kernel<<<(unsigned)nrows, kThreads, 0, st>>>(X, nchans, nsamp, stride, beam_stride, b);
     dd_rfi_fit_kernel<<<(unsigned)nbeams, kThreads, 0, st>>>(b, nchans, prm->poly_order, B, stats);
     dd_rfi_window_kernel<<<dim3((unsigned)((nwin + kThreads / 32 - 1) / (kThreads / 32)), (unsigned)nrows), kThreads, 0,
                            st>>>(X, nchans, nsamp, stride, beam_stride, prm->window, nwin, B, stats,
                                  (double)prm->t_chan, own);
-    dd_rfi_spectrum_kernel<<<dim3((unsigned)ntile, (unsigned)nbeams), kThreads, 0, st>>>(
-        X, nchans, nsamp, stride, beam_stride, prm->window, nwin, B, own, m);
+    dd_rfi_flags_kernel<<<(unsigned)std::min<int64_t>((nrows * nwin + kThreads - 1) / kThreads, 4096), kThreads, 0, st>>>(
+        own, nrows, nwin, flag);
+    dd_rfi_spectrum_kernel<<<dim3((unsigned)nspec, (unsigned)nbeams), dim3(kSpecT, kSpecQ), 0, st>>>(
+        X, nchans, nsamp, stride, beam_stride, prm->window, nwin, B, flag, m);
     dd_rfi_spectrum_stats_kernel<<<(unsigned)nbeams, kThreads, 0, st>>>(m, nsamp, stats);
     dd_rfi_apply_kernel<<<dim3((unsigned)ntile, (unsigned)nrows), kThreads, 0, st>>>(
-        X, nchans, nsamp, stride, beam_stride, prm->window, nwin, B, stats, own, m, (double)prm->t_spec, chan_flags,
+        X, nchans, nsamp, stride, beam_stride, prm->window, nwin, B, stats, flag, m, (double)prm->t_spec, chan_flags,
         spec_flags);
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess && bandpass)

@@ -141,9 +141,12 @@ def test_edges_and_argument_errors():
     for n in (1, 2, 3, 6):
         D = series(n, 1, 3, n)
         for w in (0, 3, 9):
-            Z, st, c, count = run_post(D, dd.post_params(w, True, True, nsigma=0.5))
-            z, stats = oracle.postprocess(D, median_window=w)
-            check_series(Z, z, stats, np.abs(D).max(), True, extra=1e-6)
+            # two points always lie on their fitted line: the residual is rounding noise, which neither side can
+            # normalise meaningfully (the device calls it sigma = 0); compare the detrended series there
+            nrm = n != 2
+            Z, st, c, count = run_post(D, dd.post_params(w, True, nrm, nsigma=0.5))
+            z, stats = oracle.postprocess(D, median_window=w, normalise=nrm)
+            check_series(Z, z, stats, np.abs(D).max(), nrm, extra=1e-6)
     D = np.full((1, 2, 3000), 42.5, dtype=np.float32)
     Z, st, c, count = run_post(D, dd.post_params(7, True, True, nsigma=1.0))
     assert not Z.any() and count == 0 and np.all(st[..., 2] == 0.0) and np.all(st[..., 0] == 42.5)
