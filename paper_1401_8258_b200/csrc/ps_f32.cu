@@ -13,10 +13,16 @@
 //   1. has the four channel vectors (eq 2.14) in shared memory, copied there by the
 //      TMA engine (cp.async.bulk + mbarrier, three stages ahead);
 //   2. forms one row per pattern,  P[u] = ((x0[u] + x1[u+r1]) + x2[u+r2]) + x3[u+r3],  in shared
-//      memory (all warps, 64 consecutive u per warp step);
+//      memory.  All rows of a tile sit on one grid of 32-word chunks of u.  A warp takes a "segment":
+//      a run of up to 8 patterns that need the same chunk and in which every r_k takes at most two
+//      adjacent values a_k, a_k + 1 (adjacent trials move a relative delay by less than a sample).  It
+//      loads both candidates x_k[u + a_k], x_k[u + a_k + 1] of every channel into REGISTERS once
+//      (2 G - 1 shared-memory loads per lane) and forms the row words of all patterns of the run from
+//      them: per pattern G - 1 selects (predicates from one R2P), G - 1 adds and one store, no
+//      further load -- against G loads per row word when every row is formed on its own;
 //   3. adds, for every trial d and sample t of the tile, ONE word:  acc += P_{pattern(d)}[t + s(d,c0)].
-// Step 3 costs one shared-memory word per FOUR channel-adds; step 2 adds about (patterns / KB)
-// * 5/4 words per channel-add.  Descriptors (windows, patterns, per-trial row offsets) are built on
+// Step 3 costs one shared-memory word per FOUR channel-adds; step 2 one store per row word plus
+// (2 G + 7) / 32 loads per segment word.  Descriptors (windows, segments, per-trial row offsets) are built on
 // the host at plan time from the exact delay table; nothing is approximated, and the order of
 // the additions depends only on the plan (groups in ascending channel order, inside a group the
 // expression above), never on the tile, so batch / streaming / one-shot results are identical.
@@ -57,19 +63,30 @@ constexpr int kThreads = 32 * kWarps;
 // 64 trials x 512 samples or 128 trials x 256 samples per block; chosen per plan by the cost model
 constexpr int kAccPerLane = 64;
 constexpr int kKBMax = 8 * kWarps;
-constexpr int kXStages = 3;
-constexpr int kMaxSmem = 200 * 1024;
+constexpr int kXStages = 3;               // staged groups in flight
+constexpr int kPB = 3;                    // partial-sum buffers: step 2 may run two groups ahead of step 3
+constexpr int kMaxSmem = 224 * 1024;
 
 // descriptor layout (ints), one per (trial tile, channel group)
-constexpr int kChunk = 64;                // words of a partial-sum row formed per warp step
-constexpr int kDNChunks = 0;              // kChunk-word steps of the partial-sum phase
+constexpr int kCW = 32;                   // words of a chunk: one u per lane
+constexpr int kPad = 64;                  // spare words behind the staged vectors (chunk-aligned rows read past them)
+constexpr int kDNSegs = 0;                // number of segments (work items of step 2)
 constexpr int kDBytes = 1;                // bytes of this descriptor that are in use (multiple of 16)
+constexpr int kDEnt = 2;                  // first int of the segment blocks
 constexpr int kDBase = 4;                 // [8]  first staged word of channel k, relative to t0 (multiple of 4)
 constexpr int kDLen = 12;                 // [8]  words to stage (multiple of 4; 0 for a missing channel)
 constexpr int kDTrial = 20;               // [KB] flat word offset of trial j's first operand in the partial sums
-// kDTrial + KB:                             [nchunks][G] uint16 word offset, from the stage's first staged word, of
-                                          //      the operand of lane 0 in channel k (zero pad if missing); 16-bit
-                                          //      entries because a warp-uniform LDS.128 still costs four data cycles
+// kDTrial + KB:                             [12] uint16 x 17: warp w takes segments wstart[w] .. wstart[w+1]-1
+// kDTrial + KB + 12 (= kDEnt):              [nsegs][8] segment blocks.  A segment is a run of at most kNP patterns that
+//                                                need the same chunk and in which every r_k takes at most two values,
+//                                                a_k and a_k + 1:
+//                   [4] uint16 x 8: word offset, from the stage's first word, of lane 0's operand x_k[u + a_k]
+//                                   (a missing channel, and k >= G, points at the zero pad)
+//                   [4] uint16 x 8: one entry per pattern: bit k-1 = (r_k == a_k + 1), k = 1..G-1; bits 7-15 = 1 + word
+//                                   offset / 32 of the pattern's 32 row words in the partial-sum buffer; 0 = no pattern
+constexpr int kDWarpInts = 12;
+constexpr int kNP = 8;                    // patterns per segment
+constexpr int kSegInts = 8;
 
 struct PsParams {
     const float* X;
@@ -81,20 +98,30 @@ struct PsParams {
     int64_t in_stride, in_beam_stride, out_stride, out_beam_stride;
 };
 
+// One row word of a pattern: ((x0 + x1) + x2) + ... with x_k = b[k] where bit k-1 of the pattern's entry e is set
+// (r_k = a_k + 1), else a[k].  The association depends on nothing but G.
+template <int G> __device__ __forceinline__ float pattern_sum(const float (&a)[G], const float (&b)[G], uint32_t e)
+{
+    float s = a[0];
+#pragma unroll
+    for (int k = 1; k < G; ++k) s += (e >> (k - 1)) & 1u ? b[k] : a[k];
+    return s;
+}
+
 template <int G, int KW>
 __global__ void __launch_bounds__(kThreads + 32, 1)
 dd_ps_f32_kernel(const PsParams p)
 {
-    constexpr int NK = kAccPerLane / KW, KB = KW * kWarps, TB = 32 * NK, kDChunk = kDTrial + KB;
+    constexpr int NK = kAccPerLane / KW, KB = KW * kWarps, TB = 32 * NK;
     extern __shared__ __align__(128) uint8_t smem_raw[];
-    const int xstage = G * p.xw + kChunk;                                      // words; the last kChunk stay zero
+    const int xstage = G * p.xw + kPad;                                        // words; the last kPad stay zero
     float* Xs = reinterpret_cast<float*>(smem_raw);                            // [kXStages][xstage]
     float* Ps = Xs + kXStages * xstage;                                        // [2][psw]
-    int32_t* Ds = reinterpret_cast<int32_t*>(Ps + 2 * p.psw);                  // [kXStages][desc_ints]
+    int32_t* Ds = reinterpret_cast<int32_t*>(Ps + kPB * p.psw);                  // [kXStages][desc_ints]
     uint64_t* full = reinterpret_cast<uint64_t*>(Ds + kXStages * p.desc_ints); // [kXStages]
     uint64_t* empty = full + kXStages;                                         // [kXStages]
     uint64_t* ready = empty + kXStages;                                        // [2] partial sums complete
-    uint64_t* freeb = ready + 2;                                               // [2] partial sums consumed
+    uint64_t* freeb = ready + kPB;                                               // [2] partial sums consumed
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int tile = blockIdx.x;                          // trial tiles fastest: neighbours share L2 lines
@@ -107,14 +134,14 @@ dd_ps_f32_kernel(const PsParams p)
             mbar_init(&full[s], 1);
             mbar_init(&empty[s], kWarps);
         }
-        for (int b = 0; b < 2; ++b) {
+        for (int b = 0; b < kPB; ++b) {
             mbar_init(&ready[b], kWarps);
             mbar_init(&freeb[b], kWarps);
         }
         mbar_fence_init();
     }
-    if (threadIdx.x < kXStages * kChunk)
-        Xs[(threadIdx.x / kChunk) * xstage + G * p.xw + (threadIdx.x % kChunk)] = 0.0f;
+    if (threadIdx.x < kXStages * kPad)
+        Xs[(threadIdx.x / kPad) * xstage + G * p.xw + (threadIdx.x % kPad)] = 0.0f;
     __syncthreads();
 
     if (warp == kWarps) {
@@ -151,40 +178,35 @@ dd_ps_f32_kernel(const PsParams p)
     }
 
     // -------------------------------------------------------------------- consumer warps
-    // Step 2: the pattern rows of group g into partial-sum buffer `buf`; a warp step forms kChunk
-    // consecutive words (lane l: words l and l + 32) from one descriptor entry of G byte offsets.
+    // Step 2: the pattern rows of group g into partial-sum buffer `buf`.  The rows sit on a common grid of
+    // chunks of 32 consecutive u (one per lane).  A segment is a run of patterns that need the same chunk and
+    // whose relative delays take at most two adjacent values per channel: the warp loads both candidates
+    // x_k[u + a_k], x_k[u + a_k + 1] of every channel into registers ONCE (2 G - 1 loads) and then forms the
+    // row words of every pattern of the run from registers -- per pattern and word G - 1 selects, G - 1 adds
+    // and one store, no further shared-memory read.  The host split the segments evenly over the 16 warps.
     auto pre = [&](int st, int buf) {
         const int32_t* ds = Ds + st * p.desc_ints;
         const uint32_t xa = smem_u32(Xs + st * xstage) + lane * 4;
-        float* ps = Ps + buf * p.psw + lane;
-        const int nchunks = ds[kDNChunks];
-        const uint32_t* ct = reinterpret_cast<const uint32_t*>(ds + kDChunk);
-        for (int c = warp; c < nchunks; c += kWarps) {
-            uint32_t pk[G / 2];
-            if (G == 4) {
-                const uint2 v = *reinterpret_cast<const uint2*>(ct + c * 2);
-                pk[0] = v.x; pk[1] = v.y;
-            } else {
-                const uint4 v = *reinterpret_cast<const uint4*>(ct + c * 4);
-                pk[0] = v.x; pk[1] = v.y; pk[G / 2 - 2] = v.z; pk[G / 2 - 1] = v.w;
-            }
-            int o[G];
-#pragma unroll
-            for (int q = 0; q < G / 2; ++q) {
-                o[2 * q] = (int)(pk[q] & 0xffffu) * 4;
-                o[2 * q + 1] = (int)(pk[q] >> 16) * 4;
-            }
-            float lo[G], hi[G];
+        const uint32_t pa = smem_u32(Ps + buf * p.psw) + lane * 4 - kCW * 4;    // entries hold 1 + chunk index
+        const uint16_t* ws = reinterpret_cast<const uint16_t*>(ds + kDTrial + KB);
+        const uint4* blk = reinterpret_cast<const uint4*>(ds + kDTrial + KB + kDWarpInts);
+        const int cend = ws[warp + 1];
+        for (int c = ws[warp]; c < cend; ++c) {
+            const uint4 o = blk[2 * c], en = blk[2 * c + 1];
+            const uint32_t ow[4] = {o.x, o.y, o.z, o.w}, ew[4] = {en.x, en.y, en.z, en.w};
+            float a[G], b[G];
 #pragma unroll
             for (int k = 0; k < G; ++k) {
-                lo[k] = lds_f32(xa + o[k]);
-                hi[k] = lds_f32(xa + o[k] + 128);
+                const uint32_t ad = xa + ((ow[k >> 1] >> (16 * (k & 1))) & 0xffffu) * 4;
+                a[k] = lds_f32(ad);
+                b[k] = k ? lds_f32(ad + 4) : 0.0f;
             }
-            float slo = lo[0], shi = hi[0];
 #pragma unroll
-            for (int k = 1; k < G; ++k) { slo += lo[k]; shi += hi[k]; }
-            ps[c * kChunk] = slo;
-            ps[c * kChunk + 32] = shi;
+            for (int i = 0; i < kNP; ++i) {
+                const uint32_t e = ew[i >> 1] >> (16 * (i & 1));               // entry of the run's i-th pattern
+                if (!(e & 0xff80u)) break;
+                sts_f32(pa + (e & 0xff80u), pattern_sum<G>(a, b, e));
+            }
         }
     };
 
@@ -204,13 +226,14 @@ dd_ps_f32_kernel(const PsParams p)
 
     int st = 0, sn = 1 % kXStages, phn = kXStages == 1 ? 1 : 0;
     for (int g = 0; g < ng; ++g) {
-        const int b = g & 1;
+        const int b = g % kPB, bn = (g + 1) % kPB;
         if (g + 1 < ng) {
             mbar_wait(&full[sn], phn);
-            if (g >= 1) mbar_wait(&freeb[b ^ 1], ((g - 1) >> 1) & 1);      // step 3 of g-1 is done everywhere
-            pre(sn, b ^ 1);
+            // buffer bn was last read by step 3 of group g + 1 - kPB: done everywhere?
+            if (g + 1 >= kPB) mbar_wait(&freeb[bn], ((g + 1 - kPB) / kPB) & 1);
+            pre(sn, bn);
             __syncwarp();
-            if (lane == 0) mbar_arrive(&ready[b ^ 1]);
+            if (lane == 0) mbar_arrive(&ready[bn]);
         }
         // Step 3: one word per trial, sample and group
         int tro[KW];
@@ -220,7 +243,7 @@ dd_ps_f32_kernel(const PsParams p)
             tro[4 * q] = tr.x; tro[4 * q + 1] = tr.y; tro[4 * q + 2] = tr.z; tro[4 * q + 3] = tr.w;
         }
         const float* ps = Ps + b * p.psw + lane;
-        mbar_wait(&ready[b], (g >> 1) & 1);                                // step 2 of g is done everywhere
+        mbar_wait(&ready[b], (g / kPB) & 1);                                // step 2 of g is done everywhere
 #pragma unroll
         for (int j = 0; j < KW; ++j) {
             const float* r = ps + tro[j];
@@ -275,39 +298,174 @@ PsKernel ps_kernel_for(int G, int kw)
 
 struct PsShape { bool fits = false; int64_t psw = 0, xw = 0; int desc_ints = 0; size_t smem = 0; double cost = 0; };
 
-// Shared-memory need and modelled shared-memory wavefronts per output tile for group size G:
-// step 3 costs KB * NK per group, step 2 (2 G + 2 + G / 2) per kChunk words of pattern rows.
+// Placement of the pattern rows of one (tile, group) on the common grid of kCW-word chunks, and the work
+// list of step 2.  Chunk c covers u0 + kCW c .. + kCW - 1 with u0 the smallest s(d, c0) of the tile; row r
+// occupies chunks cb[r] .. ce[r] and sits at word rowbase[r] of the partial-sum buffer.  Items = (chunk,
+// row) pairs in chunk-major order, rows in order of first appearance; a segment is a run of items of one
+// chunk; warp w takes segments wstart[w] .. wstart[w+1]-1, cut so that every warp gets about the same cost.
+// Orders the patterns of a (tile, group) so that neighbours differ in few r_k: by the sum of the relative
+// delays, then lexicographically.  (Where the r_k only jitter between two adjacent integers with the
+// fractional part of s(d, c0), the patterns form a chain along which one r_k changes at a time; where they
+// grow with the trial, this is the order of first appearance.)  slot[] is renumbered accordingly.
+void ps_chain_order(std::vector<PsRow>& rows, int* slot, int kb)
+{
+    const int nr = (int)rows.size();
+    std::vector<int> idx(nr), inv(nr);
+    for (int r = 0; r < nr; ++r) idx[r] = r;
+    auto weight = [&](int r) { int w = 0; for (int k = 0; k < kPsGMax - 1; ++k) w += rows[r].key[k]; return w; };
+    std::sort(idx.begin(), idx.end(), [&](int a, int b) {
+        const int wa = weight(a), wb = weight(b);
+        if (wa != wb) return wa < wb;
+        for (int k = 0; k < kPsGMax - 1; ++k)
+            if (rows[a].key[k] != rows[b].key[k]) return rows[a].key[k] < rows[b].key[k];
+        return a < b;
+    });
+    std::vector<PsRow> out(nr);
+    for (int r = 0; r < nr; ++r) { out[r] = rows[idx[r]]; inv[idx[r]] = r; }
+    rows.swap(out);
+    for (int j = 0; j < kb; ++j) slot[j] = inv[slot[j]];
+}
+
+struct PsSeg { int chunk, first, count; int a[kPsGMax - 1]; };
+struct PsLayout {
+    int u0 = 0, flat = 0, npw = 0;
+    std::vector<int> cb, ce, rowbase, item_chunk, item_row;
+    std::vector<PsSeg> segs;
+    int wstart[kWarps + 1];
+};
+
+void ps_layout(const std::vector<PsRow>& rows, int G, int kTB, PsLayout& L)
+{
+    const int nr = (int)rows.size();
+    L.cb.assign(nr, 0);
+    L.ce.assign(nr, 0);
+    L.rowbase.assign(nr, 0);
+    L.u0 = rows[0].umin;
+    for (const PsRow& r : rows) L.u0 = std::min(L.u0, r.umin);
+    L.flat = 0;
+    int nch = 0;
+    for (int r = 0; r < nr; ++r) {
+        L.cb[r] = (rows[r].umin - L.u0) / kCW;
+        L.ce[r] = (rows[r].umax + kTB - 1 - L.u0) / kCW;
+        L.rowbase[r] = L.flat;
+        L.flat += kCW * (L.ce[r] - L.cb[r] + 1);
+        nch = std::max(nch, L.ce[r] + 1);
+    }
+    L.item_chunk.clear();
+    L.item_row.clear();
+    for (int c = 0; c < nch; ++c)
+        for (int r = 0; r < nr; ++r)
+            if (c >= L.cb[r] && c <= L.ce[r]) {
+                L.item_chunk.push_back(c);
+                L.item_row.push_back(r);
+            }
+    // segments: greedy runs; a run ends at a new chunk, at kNP patterns, when some r_k would span more than two
+    // adjacent values, and where the cost so far says the next warp should start (loading a run's operands
+    // costs about as much as three pattern words)
+    const int header = 3;
+    const int ni = (int)L.item_row.size();
+    L.npw = ni;
+    L.segs.clear();
+    int lo[kPsGMax - 1], hi[kPsGMax - 1];
+    auto fits_run = [&](int r) {
+        for (int k = 0; k < G - 1; ++k)
+            if (std::max(hi[k], rows[r].key[k]) - std::min(lo[k], rows[r].key[k]) > 1) return false;
+        return true;
+    };
+    // first pass: runs without balancing, to know the total cost
+    int total = 0;
+    {
+        int cnt = 0;
+        for (int i = 0; i < ni; ++i) {
+            const int r = L.item_row[i];
+            const bool start = i == 0 || L.item_chunk[i] != L.item_chunk[i - 1] || cnt == kNP || !fits_run(r);
+            if (start) {
+                total += header;
+                cnt = 0;
+                for (int k = 0; k < G - 1; ++k) lo[k] = hi[k] = rows[r].key[k];
+            }
+            for (int k = 0; k < G - 1; ++k) {
+                lo[k] = std::min(lo[k], rows[r].key[k]);
+                hi[k] = std::max(hi[k], rows[r].key[k]);
+            }
+            ++cnt;
+            ++total;
+        }
+    }
+    int w = 0, acc = 0;
+    L.wstart[0] = 0;
+    for (int i = 0; i < ni; ++i) {
+        const int r = L.item_row[i];
+        bool start = i == 0 || L.item_chunk[i] != L.item_chunk[i - 1] || L.segs.back().count == kNP || !fits_run(r);
+        if (start) acc += header;                        // (the operands reloaded after a balancing cut are not counted)
+        if (i > 0 && w < kWarps - 1 && (int64_t)acc * kWarps >= (int64_t)total * (w + 1)) {
+            L.wstart[++w] = (int)L.segs.size();
+            start = true;
+        }
+        if (start) {
+            PsSeg sg;
+            sg.chunk = L.item_chunk[i];
+            sg.first = i;
+            sg.count = 0;
+            for (int k = 0; k < kPsGMax - 1; ++k) sg.a[k] = 0;
+            L.segs.push_back(sg);
+            for (int k = 0; k < G - 1; ++k) lo[k] = hi[k] = rows[r].key[k];
+        }
+        for (int k = 0; k < G - 1; ++k) {
+            lo[k] = std::min(lo[k], rows[r].key[k]);
+            hi[k] = std::max(hi[k], rows[r].key[k]);
+            L.segs.back().a[k] = lo[k];
+        }
+        ++L.segs.back().count;
+        ++acc;
+    }
+    while (w < kWarps) L.wstart[++w] = (int)L.segs.size();
+}
+
+// Shared-memory need and modelled cost per output tile for group size G and tile shape kw.  Shared-memory
+// wavefronts: step 3 takes KB * NK + KB per group (one word per trial and sample, the row offsets), step 2
+// 2 G + 9 per segment (two 16-byte block reads, the operands) and one store per pattern word.  Issue slots:
+// step 3 about 2.8 per word, a segment about 30 + 4 G, a pattern word about 5 + 3 (G - 1) instructions; four
+// schedulers.  The cost is the larger of the two.
 PsShape shape_for(const HostTable& h, int G, int kw)
 {
     PsShape o;
     const int kKB = kw * kWarps, kNK = kAccPerLane / kw, kTB = 32 * kNK, kDChunk = kDTrial + kKB;
     const int ntiles = (h.ndm + kKB - 1) / kKB, ngroups = (h.nchans + G - 1) / G;
     const int64_t spread = max_tile_spread(h, kKB);
-    o.xw = (kTB + spread + 3 + 3) / 4 * 4 + kChunk;
+    o.xw = (kTB + spread + 3 + 3) / 4 * 4 + kPad;
     const int workers = ps_workers(ntiles);
-    std::vector<int64_t> wpsw(workers, 0), wchunks(workers, 0);
+    std::vector<int64_t> wpsw(workers, 0), wsegs(workers, 0), wpw(workers, 0), wmax(workers, 0);
     ps_parallel_tiles(ntiles, workers, [&](int tb, int te, int wk) {
         std::vector<PsRow> rows;
+        PsLayout L;
         int slot[kKBMax];
         for (int tile = tb; tile < te; ++tile)
             for (int g = 0; g < ngroups; ++g) {
                 ps_classify(h, G, kKB, tile, g, rows, slot);
-                int64_t w = 0;
-                for (const PsRow& r : rows) w += ((int64_t)r.umax - r.umin + kTB + kChunk - 1) / kChunk * kChunk;
-                wpsw[wk] = std::max(wpsw[wk], w);
-                wchunks[wk] += w / kChunk;
+                ps_chain_order(rows, slot, kKB);
+                ps_layout(rows, G, kTB, L);
+                wpsw[wk] = std::max<int64_t>(wpsw[wk], L.flat);
+                wmax[wk] = std::max<int64_t>(wmax[wk], (int64_t)L.segs.size());
+                wsegs[wk] += (int64_t)L.segs.size();
+                wpw[wk] += L.npw;
             }
     });
-    int64_t chunks = 0;
+    int64_t segs = 0, pw = 0, maxsegs = 0;
     for (int wk = 0; wk < workers; ++wk) {
         o.psw = std::max(o.psw, wpsw[wk]);
-        chunks += wchunks[wk];
+        maxsegs = std::max(maxsegs, wmax[wk]);
+        segs += wsegs[wk];
+        pw += wpw[wk];
     }
-    o.desc_ints = (kDChunk + (G / 2) * (int)(o.psw / kChunk) + 3) / 4 * 4;
-    o.smem = (size_t)kXStages * (G * o.xw + kChunk) * 4 + (size_t)2 * o.psw * 4 +
-             (size_t)kXStages * o.desc_ints * 4 + (2 * kXStages + 4) * 8;
-    o.fits = G * o.xw + kChunk < 65536 && o.smem <= (size_t)kMaxSmem;
-    o.cost = (double)ntiles * ngroups * kKB * kNK + (double)chunks * (2 * G + 2 + G / 2);
+    o.desc_ints = (int)(kDChunk + kDWarpInts + kSegInts * maxsegs + 4);
+    o.smem = (size_t)kXStages * (G * o.xw + kPad) * 4 + (size_t)kPB * o.psw * 4 +
+             (size_t)kXStages * o.desc_ints * 4 + (2 * kXStages + 2 * kPB) * 8;
+    o.fits = G * o.xw + kPad < 65536 && o.psw / kCW <= 511 && maxsegs < 65536 && o.smem <= (size_t)kMaxSmem;
+    const double tg = (double)ntiles * ngroups;
+    const double lsu = tg * (kKB * kNK + kKB) + (double)segs * (2 * G + 9) + (double)pw;
+    const double issue = (tg * 2.8 * kKB * kNK + (30.0 + 4.0 * G) * segs + (5.0 + 3.0 * (G - 1)) * pw) / 4.0;
+    o.cost = std::max(lsu / 0.85, issue / 0.8);
     return o;
 }
 
@@ -361,18 +519,20 @@ int build_ps_plan(dd_plan* p)
         destroy_ps_plan(p);
         return fail(DD_ERR_NOMEM, "ps descriptor allocation failed");
     }
-    const int zero_pad = G * t->xw;                       // word offset of the stage's kChunk zero words
+    const int zero_pad = G * t->xw;                       // word offset of the stage's kPad zero words
     bool bounds_ok = true;                                // every shared-memory offset written below is in range
     const int workers = ps_workers(ntiles);
     std::vector<char> wok(workers, 1);
     ps_parallel_tiles(ntiles, workers, [&](int tb, int te, int wk) {
     std::vector<PsRow> rows;
+    PsLayout L;
     int slot[kKBMax];
-    std::vector<int> rowbase;
     bool bounds_ok = true;
     for (int tile = tb; tile < te; ++tile)
         for (int g = 0; g < ngroups; ++g) {
             ps_classify(h, G, kKB, tile, g, rows, slot);
+            ps_chain_order(rows, slot, kKB);
+            ps_layout(rows, G, kTB, L);
             int32_t* ds = &desc[((size_t)tile * ngroups + g) * desc_ints];
             const int c0 = g * G, nk = std::min(G, nch - c0);
             const int dfirst = tile * kKB, dlast = std::min(tile * kKB + kKB, ndm) - 1;
@@ -383,32 +543,48 @@ int build_ps_plan(dd_plan* p)
                 ds[kDBase + k] = base[k];
                 ds[kDLen + k] = (smax + kTB - base[k] + 3) / 4 * 4;
             }
-            int flat = 0;
-            rowbase.assign(rows.size(), 0);
-            for (size_t r = 0; r < rows.size(); ++r) {
-                rowbase[r] = flat;
-                const int ulen = rows[r].umax - rows[r].umin + kTB;
-                // word e of the flat partial-sum buffer (rowbase <= e < rowbase + ulen) is
-                // u = umin + (e - rowbase); channel k supplies x_k[u + r_k], staged at word
-                // (u + r_k - base_k) of its vector
-                for (int c = 0; c < (ulen + kChunk - 1) / kChunk; ++c) {
-                    uint16_t* ce = reinterpret_cast<uint16_t*>(ds + kDChunk) + G * (flat / kChunk + c);
-                    for (int k = 0; k < G; ++k) {
-                        const int rk = k == 0 ? 0 : rows[r].key[k - 1];
-                        const int off = k < nk ? k * t->xw + rows[r].umin + kChunk * c + rk - base[k] : zero_pad;
-                        // every lane's two reads (words off + l and off + l + 32) stay inside the stage
-                        bounds_ok = bounds_ok && off >= 0 && off + kChunk <= G * t->xw + kChunk;
-                        ce[k] = (uint16_t)off;
-                    }
+            // word e of row r's storage is u = u0 + kCW cb[r] + e; channel k supplies x_k[u + r_k], staged at word
+            // (u + r_k - base_k) of its vector.  The first chunk of a row starts up to kCW - 1 words before the
+            // row's first valid u and its last chunk ends as many after: those words read neighbouring staged
+            // data (for k = 0 never below the stage: u >= u0 >= base_0) and are never used by step 3.
+            const int nsegs = (int)L.segs.size();
+            const int ent0 = kDChunk + kDWarpInts;
+            uint16_t* ws = reinterpret_cast<uint16_t*>(ds + kDChunk);
+            for (int w = 0; w <= kWarps; ++w) ws[w] = (uint16_t)L.wstart[w];
+            for (int sg = 0; sg < nsegs; ++sg) {
+                const PsSeg& S = L.segs[sg];
+                uint16_t* o16 = reinterpret_cast<uint16_t*>(ds + ent0 + kSegInts * sg);
+                uint16_t* e16 = o16 + 8;
+                for (int k = 0; k < 8; ++k) {
+                    const int ak = k == 0 ? 0 : (k < G ? S.a[k - 1] : 0);
+                    const int off = k < nk ? k * t->xw + L.u0 + kCW * S.chunk + ak - base[k] : zero_pad;
+                    // both candidates of every lane (words off + l and off + l + 1) stay inside the stage
+                    bounds_ok = bounds_ok && off >= 0 && off + 1 + kCW <= G * t->xw + kPad;
+                    o16[k] = (uint16_t)off;
                 }
-                flat += (ulen + kChunk - 1) / kChunk * kChunk;
+                bounds_ok = bounds_ok && S.count >= 1 && S.count <= kNP;
+                for (int i = 0; i < S.count; ++i) {
+                    const int r = L.item_row[S.first + i];
+                    const int store = L.rowbase[r] + kCW * (S.chunk - L.cb[r]);
+                    bounds_ok = bounds_ok && store >= 0 && store + kCW <= t->psw && store / kCW < 511;
+                    uint32_t bits = 0;
+                    for (int k = 1; k < G; ++k) {
+                        const int dk = rows[r].key[k - 1] - S.a[k - 1];
+                        bounds_ok = bounds_ok && (dk == 0 || dk == 1);
+                        bits |= (uint32_t)(dk & 1) << (k - 1);
+                    }
+                    e16[i] = (uint16_t)(bits | (uint32_t)(store / kCW + 1) << 7);
+                }
             }
-            ds[kDNChunks] = flat / kChunk;
-            ds[kDBytes] = (4 * kDChunk + 2 * G * (flat / kChunk) + 15) / 16 * 16;
+            bounds_ok = bounds_ok && ent0 + kSegInts * nsegs + 4 <= desc_ints && nsegs < 65536;
+            ds[kDNSegs] = nsegs;
+            ds[kDEnt] = ent0;
+            ds[kDBytes] = (4 * (ent0 + kSegInts * nsegs) + 15) / 16 * 16;
             for (int j = 0; j < kKB; ++j) {
                 const int d = std::min(tile * kKB + j, ndm - 1);
                 const int s0 = h.shift[(size_t)d * nch + c0];
-                ds[kDTrial + j] = rowbase[slot[j]] + (s0 - rows[slot[j]].umin);
+                const int r = slot[j];
+                ds[kDTrial + j] = L.rowbase[r] + (s0 - (L.u0 + kCW * L.cb[r]));
                 bounds_ok = bounds_ok && ds[kDTrial + j] >= 0 && ds[kDTrial + j] + kTB <= t->psw;
             }
         }
