@@ -57,6 +57,7 @@ constexpr int kThreads = 32 * kWarps;
 constexpr int kAccPerLane = 64;
 constexpr int kKBMax = 8 * kWarps;
 constexpr int kXStages = 3;
+constexpr int kPB = 3;                    // partial-sum buffers: step 2 may run two groups ahead of step 3
 constexpr int kMaxSmem = 200 * 1024;
 constexpr int kFlushGroups = 64;          // 64 groups * 4 channels * 255 = 65280 < 65536
 constexpr int kChunk = 64;                // even-u words (= 128 samples) a warp step writes ...
@@ -72,10 +73,6 @@ constexpr int kDTrial = 12;               // [KB] word offset of trial j's first
                                           //      aligned word lane 0 reads in channel k (zero pad if missing);
                                           //      [4], [5] first even-u / odd-u word the step writes (even numbers)
 
-__device__ __forceinline__ void consumer_barrier()
-{
-    asm volatile("bar.sync 1, %0;" ::"n"(kThreads) : "memory");
-}
 struct PsU8Params {
     int32_t* D;
     const int32_t* desc;
@@ -93,10 +90,12 @@ dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
     extern __shared__ __align__(128) uint8_t smem_raw[];
     const int xstage = p.xstage;                                               // bytes: 16 rows of xwb, 256 zero bytes, slack
     uint8_t* Xs = smem_raw;                                                    // [kXStages][xstage]
-    uint32_t* Ps = reinterpret_cast<uint32_t*>(Xs + kXStages * xstage);        // [2][psw]
-    int32_t* Ds = reinterpret_cast<int32_t*>(Ps + 2 * p.psw);                  // [kXStages][desc_ints]
+    uint32_t* Ps = reinterpret_cast<uint32_t*>(Xs + kXStages * xstage);        // [kPB][psw]
+    int32_t* Ds = reinterpret_cast<int32_t*>(Ps + kPB * p.psw);                // [kXStages][desc_ints]
     uint64_t* full = reinterpret_cast<uint64_t*>(Ds + kXStages * p.desc_ints); // [kXStages]
     uint64_t* empty = full + kXStages;                                         // [kXStages]
+    uint64_t* ready = empty + kXStages;                                        // [kPB] partial sums complete
+    uint64_t* freeb = ready + kPB;                                             // [kPB] partial sums consumed
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t xs0 = smem_u32(Xs);
@@ -109,6 +108,10 @@ dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
         for (int s = 0; s < kXStages; ++s) {
             mbar_init(&full[s], 1);
             mbar_init(&empty[s], kWarps);
+        }
+        for (int b = 0; b < kPB; ++b) {
+            mbar_init(&ready[b], kWarps);
+            mbar_init(&freeb[b], kWarps);
         }
         mbar_fence_init();
     }
@@ -229,9 +232,13 @@ dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
         ++nflush;
     };
 
+    // Warps synchronise through split-phase barriers, not a block barrier: ready[b] completes when all 16
+    // warps have written their part of partial-sum buffer b, freeb[b] when all have consumed it; with three
+    // buffers a warp only waits if another one is more than a whole group behind.
     mbar_wait(&full[0], 0);
     pre(0, 0);
-    consumer_barrier();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&ready[0]);
 
     // st: stage of group g; sn / phn: stage and phase parity of group g + 1
     int st = 0, sn = 1 % kXStages, phn = kXStages == 1 ? 1 : 0;
@@ -242,9 +249,14 @@ dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
         const int g1 = min(ng, g0 + kFlushGroups);
 #pragma unroll 1
         for (int g = g0; g < g1; ++g) {
+            const int b = g % kPB, bn = (g + 1) % kPB;
             if (g + 1 < ng) {
                 mbar_wait(&full[sn], phn);
-                pre(sn, (g + 1) & 1);
+                // buffer bn was last read by step 3 of group g + 1 - kPB: done everywhere?
+                if (g + 1 >= kPB) mbar_wait(&freeb[bn], ((g + 1 - kPB) / kPB) & 1);
+                pre(sn, bn);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&ready[bn]);
             }
             // Step 3: one word per trial, sample pair and group
             int tro[KW];
@@ -253,7 +265,8 @@ dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
                 const int4 tr = *reinterpret_cast<const int4*>(Ds + st * p.desc_ints + kDTrial + warp * KW + 4 * q);
                 tro[4 * q] = tr.x; tro[4 * q + 1] = tr.y; tro[4 * q + 2] = tr.z; tro[4 * q + 3] = tr.w;
             }
-            const uint32_t* ps = Ps + (g & 1) * p.psw + lane;
+            const uint32_t* ps = Ps + b * p.psw + lane;
+            mbar_wait(&ready[b], (g / kPB) & 1);         // step 2 of g is done everywhere
 #pragma unroll
             for (int j = 0; j < KW; ++j) {
                 const uint32_t* r = ps + tro[j];
@@ -261,8 +274,10 @@ dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
                 for (int i = 0; i < NK; ++i) acc[j][i] += r[32 * i];
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[st]);      // stage st (vectors and descriptor) may be refilled
-            consumer_barrier();                          // partial sums of g+1 complete, those of g consumed
+            if (lane == 0) {
+                mbar_arrive(&freeb[b]);
+                mbar_arrive(&empty[st]);                 // stage st (vectors and descriptor) may be refilled
+            }
             st = sn;
             if (++sn == kXStages) { sn = 0; phn ^= 1; }
         }
@@ -328,8 +343,8 @@ static int try_build_psu8(dd_plan* p, int kw)
         max_steps = std::max(max_steps, wsteps[wk]);
     }
     const int desc_ints = kDChunk + kCE * (int)max_steps;
-    const size_t smem = (size_t)kXStages * xstage + (size_t)2 * psw * 4 +
-                        (size_t)kXStages * desc_ints * 4 + 2 * kXStages * 8;
+    const size_t smem = (size_t)kXStages * xstage + (size_t)kPB * psw * 4 +
+                        (size_t)kXStages * desc_ints * 4 + (2 * kXStages + 2 * kPB) * 8;
     if (smem > (size_t)kMaxSmem) {                        // too many patterns for shared memory
         p->ps_why = "the delay patterns of a trial tile do not fit shared memory (per-trial delay steps too coarse)";
         return DD_OK;
