@@ -537,7 +537,7 @@ def next_rows(dd, torch, hbm_peak):
     rows["f1_postprocess"] = {"shape": "config 3 output, %d series x %d samples float32; median 5, detrend, normalise, 6 sigma -> candidates" % (w.ndm, w.nsamp),
                               "ms": ms, "algorithmic_bytes": by, "bound": "hbm", "achieved_gbs": by / ms / 1e6,
                               "peak_gbs": peak, "frac": by / ms / 1e6 / peak, "gpu_launches": dd.dd_postprocess_launches(prm, False),
-                              "note": "algorithmic = D read once; the kernels read it three times (fit pass 1, pass 2, apply), twice through L2 for rows that fit"}
+                              "note": "algorithmic = D read once; the kernels read it twice (regression statistics, apply)"}
     del D
     # f3: RFI mitigation of config 3's input buffer, in place
     n_in = w.nsamp + 14845
@@ -547,8 +547,8 @@ def next_rows(dd, torch, hbm_peak):
     by = X.numel() * 8
     rows["f3_rfi"] = {"shape": "config 3 input, %d channels x %d samples float32; order 4, window 512, thresholds 7 / 5" % (w.nchans, n_in),
                       "ms": ms, "algorithmic_bytes": by, "bound": "hbm", "achieved_gbs": by / ms / 1e6, "peak_gbs": peak,
-                      "frac": by / ms / 1e6 / peak, "gpu_launches": 6,
-                      "note": "algorithmic = X read once + written once; the kernels read it four times (row means, window means, spectrum means, apply)"}
+                      "frac": by / ms / 1e6 / peak, "gpu_launches": 8,
+                      "note": "algorithmic = X read once + written once; the kernels read it three times (window sums, spectrum means, apply)"}
     del X
     # f4: beamformer, BEST-II parameters of PAPER.md:1653 (32 antennas, 1024 channels, 16 beams) over 2^16 samples
     na, nch, nb, nt = 32, 1024, 16, 1 << 16

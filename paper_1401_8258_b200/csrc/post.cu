@@ -40,14 +40,26 @@ template <typename T> __device__ __forceinline__ void cmpx(T& a, T& b)
     a = lo;
     b = hi;
 }
-// median of W values by a full odd-even transposition sort (static indices, branch-free)
+template <typename T> __device__ __forceinline__ T mn(T a, T b) { return a < b ? a : b; }
+template <typename T> __device__ __forceinline__ T mx(T a, T b) { return a < b ? b : a; }
+// median of W values: selection only (the result is one of the inputs), static indices, branch-free.
+// W = 3 and 5 use the short min / max forms (4 and 10 operations: the median of five is the median of
+// the fifth value, the larger of the two pair minima and the smaller of the two pair maxima); the
+// other windows a full odd-even transposition sort.
 template <typename T, int W> __device__ __forceinline__ T median_of(T (&v)[W])
 {
+    if constexpr (W == 3) {
+        return mx(mn(v[0], v[1]), mn(mx(v[0], v[1]), v[2]));
+    } else if constexpr (W == 5) {
+        const T lo = mx(mn(v[0], v[1]), mn(v[2], v[3])), hi = mn(mx(v[0], v[1]), mx(v[2], v[3]));
+        return mx(mn(lo, hi), mn(mx(lo, hi), v[4]));
+    } else {
 #pragma unroll
-    for (int round = 0; round < W; ++round)
+        for (int round = 0; round < W; ++round)
 #pragma unroll
-        for (int i = round & 1; i + 1 < W; i += 2) cmpx(v[i], v[i + 1]);
-    return v[W / 2];
+            for (int i = round & 1; i + 1 < W; i += 2) cmpx(v[i], v[i + 1]);
+        return v[W / 2];
+    }
 }
 
 // The kPer medians (as doubles) of samples t0 .. t0+kPer-1 of one series; window indices clamped to
@@ -57,7 +69,20 @@ __device__ __forceinline__ void medians4(const T* __restrict__ row, int64_t t0, 
 {
     constexpr int H = (W - 1) / 2;
     T x[kPer + 2 * H];
-    if (t0 >= H && t0 + kPer + H <= n) {                  // interior: no clamping
+    static_assert(sizeof(T) == 4 && kPer == 4 && H <= 4, "the aligned path loads three 16-byte vectors");
+    if (t0 >= 4 && t0 + 8 <= n && ((uintptr_t)(row + t0) & 15) == 0) {
+        // interior, 16-byte aligned: the thread's four samples and the aligned vectors on either side
+        // (the neighbours' own samples: L1 hits) instead of 4 + 2 H scalar loads
+        const int4* src = reinterpret_cast<const int4*>(row + t0);
+        const int4 l = __ldg(src - 1), c = __ldg(src), r = __ldg(src + 1);
+        const int w12[12] = {l.x, l.y, l.z, l.w, c.x, c.y, c.z, c.w, r.x, r.y, r.z, r.w};
+#pragma unroll
+        for (int i = 0; i < kPer + 2 * H; ++i) {
+            union { int i; T t; } u;
+            u.i = w12[4 - H + i];
+            x[i] = u.t;
+        }
+    } else if (t0 >= H && t0 + kPer + H <= n) {           // interior: no clamping
         const T* src = row + (t0 - H);
 #pragma unroll
         for (int i = 0; i < kPer + 2 * H; ++i) x[i] = __ldg(src + i);

@@ -12,9 +12,10 @@
 // with a write pass each.  Here everything stays on the device (the fit is one block solving the
 // normal equations in a Legendre basis in double precision) and the replacements are never written as
 // such: the window flags and the spectrum excesses are small side arrays, applied when the single
-// output pass subtracts the bandpass.  Passes over X: three reads (row means, window means, spectrum
-// means of the clipped data) and one read + write -- all HBM-bound streaming kernels.  All means, the fit and the threshold comparisons are evaluated in
-// double precision; the output is rounded once, from double, to float32.
+// output pass subtracts the bandpass.  Passes over X: two reads (window sums -- from which both the
+// averaged bandpass and the window means follow -- and the spectrum means of the clipped data) and one
+// read + write -- all HBM-bound streaming kernels.  All means, the fit and the threshold comparisons are
+// evaluated in double precision; the output is rounded once, from double, to float32.
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -48,18 +49,42 @@ __device__ __forceinline__ double block_sum(double v, double* red)
     return s;
 }
 
-// 1a. b[row] = mean over time of channel row (one block per (beam, channel))
+// 1a. wsum[row][k] = sum of window k of channel row (one warp per window): the ONLY pass over X before the
+// flags are known -- the averaged bandpass and the window means of stage 2 both follow from these sums.
 __global__ void __launch_bounds__(kThreads)
-dd_rfi_bandpass_kernel(const float* __restrict__ X, int nchans, int64_t n, int64_t stride, int64_t beam_stride,
-                       double* __restrict__ b)
+dd_rfi_window_sums_kernel(const float* __restrict__ X, int nchans, int64_t n, int64_t stride, int64_t beam_stride,
+                          int window, int nwin, double* __restrict__ wsum)
 {
-    __shared__ double red[kThreads / 32];
-    const int64_t row = blockIdx.x;
+    const int64_t row = blockIdx.y;
+    const int k = blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (k >= nwin) return;
     const float* x = X + (row / nchans) * beam_stride + (row % nchans) * stride;
+    const int64_t a = (int64_t)k * window, e = min(n, a + window);
     double s = 0.0;
-    for (int64_t t = threadIdx.x; t < n; t += kThreads) s += (double)__ldg(x + t);
-    s = block_sum(s, red);
-    if (threadIdx.x == 0) b[row] = s / (double)n;
+    if ((window & 3) == 0 && e - a == window && (((uintptr_t)(x + a)) & 15) == 0) {
+        const float4* x4 = reinterpret_cast<const float4*>(x + a);
+        for (int i = lane; i < window / 4; i += 32) {
+            const float4 v = __ldg(x4 + i);
+            s += ((double)v.x + (double)v.y) + ((double)v.z + (double)v.w);
+        }
+    } else {
+        for (int64_t t = a + lane; t < e; t += 32) s += (double)__ldg(x + t);
+    }
+    s = warp_sum(s);
+    if (lane == 0) wsum[row * nwin + k] = s;
+}
+
+// 1a'. b[row] = mean over time of channel row = (sum of its window sums) / n  (one warp per row, fixed order)
+__global__ void __launch_bounds__(kThreads)
+dd_rfi_bandpass_kernel(const double* __restrict__ wsum, int64_t nrows, int nwin, int64_t n, double* __restrict__ b)
+{
+    const int64_t row = (int64_t)blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (row >= nrows) return;
+    double s = 0.0;
+    for (int k = lane; k < nwin; k += 32) s += wsum[row * nwin + k];
+    s = warp_sum(s);
+    if (lane == 0) b[row] = s / (double)n;
 }
 
 // 1b. One block per beam: least-squares polynomial of order p through (x_c, b_c), x_c the channel index
@@ -139,32 +164,25 @@ dd_rfi_fit_kernel(const double* __restrict__ b, int nchans, int order, double* _
     }
 }
 
-// 2a. own[row][k] = |mean of window k - B_row| > T_c * RMSE   (one warp per window)
+// 2. flag[row][k] = own[k-1] | own[k] | own[k+1],  own[k] = |mean of window k - B_row| > T_c * RMSE
+// ("neighbouring blocks are also flagged", R24); the last, shorter window counts with its own length (R23).
 __global__ void __launch_bounds__(kThreads)
-dd_rfi_window_kernel(const float* __restrict__ X, int nchans, int64_t n, int64_t stride, int64_t beam_stride,
-                     int window, int nwin, const double* __restrict__ B, const double* __restrict__ stats,
-                     double t_chan, uint8_t* __restrict__ own)
-{
-    const int64_t row = blockIdx.y;
-    const int beam = (int)(row / nchans);
-    const int k = blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-    if (k >= nwin) return;
-    const float* x = X + (int64_t)beam * beam_stride + (row % nchans) * stride;
-    const int64_t a = (int64_t)k * window, e = min(n, a + window);
-    double s = 0.0;
-    for (int64_t t = a + lane; t < e; t += 32) s += (double)__ldg(x + t);
-    s = warp_sum(s);
-    if (lane == 0) own[row * nwin + k] = fabs(s / (double)(e - a) - B[row]) > t_chan * stats[beam * 4 + 0];
-}
-
-// 2b. flag[row][k] = own[k-1] | own[k] | own[k+1]  ("neighbouring blocks are also flagged", R24)
-__global__ void __launch_bounds__(kThreads)
-dd_rfi_flags_kernel(const uint8_t* __restrict__ own, int64_t nrows, int nwin, uint8_t* __restrict__ flag)
+dd_rfi_flags_kernel(const double* __restrict__ wsum, int64_t nrows, int nchans, int nwin, int window, int64_t n,
+                    const double* __restrict__ B, const double* __restrict__ stats, double t_chan,
+                    uint8_t* __restrict__ flag, uint8_t* __restrict__ chan_flags)
 {
     const int64_t total = nrows * nwin;
     for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < total; i += (int64_t)gridDim.x * kThreads) {
+        const int64_t row = i / nwin;
         const int k = (int)(i % nwin);
-        flag[i] = own[i] | (k > 0 ? own[i - 1] : 0) | (k + 1 < nwin ? own[i + 1] : 0);
+        const double Bc = B[row], level = t_chan * stats[(row / nchans) * 4 + 0];
+        auto own = [&](int kk) {
+            const int64_t a = (int64_t)kk * window, e = min(n, a + window);
+            return fabs(wsum[row * nwin + kk] / (double)(e - a) - Bc) > level;
+        };
+        const bool f = own(k) || (k > 0 && own(k - 1)) || (k + 1 < nwin && own(k + 1));
+        flag[i] = f;
+        if (chan_flags) chan_flags[i] = f;
     }
 }
 
@@ -232,24 +250,44 @@ dd_rfi_spectrum_stats_kernel(const double* __restrict__ m, int64_t n, double* __
     }
 }
 
+// 3c. per spectrum: excess[t] = m_t - mean_c B_c if the spectrum is flagged (m_t - mu > T_s sigma), else 0;
+// any4[t / 4] = some spectrum of the group of four is flagged (lets the write pass skip the excesses)
+__global__ void __launch_bounds__(kThreads)
+dd_rfi_excess_kernel(const double* __restrict__ m, int64_t n, const double* __restrict__ stats, double t_spec,
+                     double* __restrict__ excess, uint8_t* __restrict__ any4, uint8_t* __restrict__ spec_flags)
+{
+    const int beam = blockIdx.y;
+    const int64_t g = (int64_t)blockIdx.x * kThreads + threadIdx.x, t0 = 4 * g;
+    if (t0 >= n) return;
+    const double mu = stats[beam * 4 + 2], level = t_spec * stats[beam * 4 + 3], bmean = stats[beam * 4 + 1];
+    bool any = false;
+    for (int e = 0; e < 4 && t0 + e < n; ++e) {
+        const double me = m[(int64_t)beam * n + t0 + e];
+        const bool sf = (me - mu) > level;
+        excess[(int64_t)beam * n + t0 + e] = sf ? me - bmean : 0.0;
+        if (spec_flags) spec_flags[(int64_t)beam * n + t0 + e] = sf;
+        any = any || sf;
+    }
+    any4[(int64_t)beam * ((n + 3) / 4) + g] = any;
+}
+
 // 4. the single write pass: channel replacement, spectrum excess, bandpass subtraction; four consecutive
-// samples per thread (16-byte accesses when the row allows)
+// samples per thread (16-byte accesses when the row allows); every value is formed in double and rounded once
 __global__ void __launch_bounds__(kThreads)
 dd_rfi_apply_kernel(float* __restrict__ X, int nchans, int64_t n, int64_t stride, int64_t beam_stride, int window,
-                    int nwin, const double* __restrict__ B, const double* __restrict__ stats,
-                    const uint8_t* __restrict__ flag, const double* __restrict__ m, double t_spec,
-                    uint8_t* __restrict__ chan_flags, uint8_t* __restrict__ spec_flags)
+                    int nwin, const double* __restrict__ B, const uint8_t* __restrict__ flag,
+                    const double* __restrict__ excess, const uint8_t* __restrict__ any4)
 {
     const int64_t row = blockIdx.y;
     const int beam = (int)(row / nchans);
-    const int64_t t0 = ((int64_t)blockIdx.x * kThreads + threadIdx.x) * 4;
+    const int64_t g = (int64_t)blockIdx.x * kThreads + threadIdx.x, t0 = 4 * g;
     if (t0 >= n) return;
     float* x = X + (int64_t)beam * beam_stride + (row % nchans) * stride + t0;
-    const double Bc = B[row], mu = stats[beam * 4 + 2], level = t_spec * stats[beam * 4 + 3], bmean = stats[beam * 4 + 1];
-    const double* mt = m + (int64_t)beam * n + t0;
+    const double Bc = B[row];
     const uint8_t* fl = flag + row * nwin;
-    int k = (int)(t0 / window);
-    int64_t next = (int64_t)(k + 1) * window;              // first sample of the next window
+    const int k0 = (int)(t0 / window), k1 = (int)(min(t0 + 3, n - 1) / window);
+    const bool cf0 = fl[k0], cf1 = k1 != k0 ? (bool)fl[k1] : cf0;
+    const int64_t next = (int64_t)(k0 + 1) * window;       // first sample of the next window
     const bool vec = t0 + 4 <= n && ((((uintptr_t)x) & 15) == 0);
     float v[4];
     if (vec) {
@@ -259,23 +297,17 @@ dd_rfi_apply_kernel(float* __restrict__ X, int nchans, int64_t n, int64_t stride
 #pragma unroll
         for (int e = 0; e < 4; ++e) v[e] = t0 + e < n ? x[e] : 0.0f;
     }
-    bool cf = fl[k];
+    double ex[4] = {0.0, 0.0, 0.0, 0.0};
+    if (any4[(int64_t)beam * ((n + 3) / 4) + g]) {
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+            if (t0 + e < n) ex[e] = excess[(int64_t)beam * n + t0 + e];
+    }
 #pragma unroll
     for (int e = 0; e < 4; ++e) {
-        const int64_t t = t0 + e;
-        if (t >= n) break;
-        if (t >= next) {
-            ++k;
-            next += window;
-            cf = fl[k];
-        }
-        const double me = mt[e];
-        const bool sf = (me - mu) > level;
-        double val = cf ? Bc : (double)v[e];
-        if (sf) val -= me - bmean;
+        const bool cf = t0 + e >= next ? cf1 : cf0;
+        const double val = (cf ? Bc : (double)v[e]) - ex[e];
         v[e] = (float)(val - Bc);
-        if (chan_flags && t == (int64_t)k * window) chan_flags[row * nwin + k] = cf;
-        if (spec_flags && row % nchans == 0) spec_flags[(int64_t)beam * n + t] = sf;
     }
     if (vec) {
         *reinterpret_cast<float4*>(x) = make_float4(v[0], v[1], v[2], v[3]);
@@ -310,30 +342,35 @@ int rfi_mitigate(float* X, int nchans, int64_t nsamp, int64_t stride, int64_t be
     const int nwin = (int)nwin64;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (nbeams == 1) beam_stride = 0;
-    // workspace: b [nrows], B [nrows], stats [nbeams][4], m [nbeams][nsamp] (doubles), own and flag [nrows][nwin] (bytes)
-    const size_t nd = (size_t)nrows * 2 + (size_t)nbeams * 4 + (size_t)nbeams * nsamp;
+    // workspace (doubles): b [nrows], B [nrows], stats [nbeams][4], m and excess [nbeams][nsamp], wsum [nrows][nwin];
+    // (bytes): flag [nrows][nwin], any4 [nbeams][ceil(nsamp / 4)]
+    const int64_t ng4 = (nsamp + 3) / 4;
+    const size_t nd = (size_t)nrows * 2 + (size_t)nbeams * 4 + (size_t)2 * nbeams * nsamp + (size_t)nrows * nwin;
     char* ws = nullptr;
-    int rc = workspace_alloc((void**)&ws, nd * sizeof(double) + (size_t)2 * nrows * nwin, cuda_stream);
+    int rc = workspace_alloc((void**)&ws, nd * sizeof(double) + (size_t)nrows * nwin + (size_t)nbeams * ng4, cuda_stream);
     if (rc != DD_OK) return rc;
     double* b = (double*)ws;
     double* B = b + nrows;
     double* stats = B + nrows;
     double* m = stats + (size_t)nbeams * 4;
-    uint8_t* own = (uint8_t*)(m + (size_t)nbeams * nsamp);
-    uint8_t* flag = own + (size_t)nrows * nwin;
-    dd_rfi_bandpass_kernel<<<(unsigned)nrows, kThreads, 0, st>>>(X, nchans, nsamp, stride, beam_stride, b);
+    double* excess = m + (size_t)nbeams * nsamp;
+    double* wsum = excess + (size_t)nbeams * nsamp;
+    uint8_t* flag = (uint8_t*)(wsum + (size_t)nrows * nwin);
+    uint8_t* any4 = flag + (size_t)nrows * nwin;
+    constexpr int kWPB = kThreads / 32;                    // warps per block
+    dd_rfi_window_sums_kernel<<<dim3((unsigned)((nwin + kWPB - 1) / kWPB), (unsigned)nrows), kThreads, 0, st>>>(
+        X, nchans, nsamp, stride, beam_stride, prm->window, nwin, wsum);
+    dd_rfi_bandpass_kernel<<<(unsigned)((nrows + kWPB - 1) / kWPB), kThreads, 0, st>>>(wsum, nrows, nwin, nsamp, b);
     dd_rfi_fit_kernel<<<(unsigned)nbeams, kThreads, 0, st>>>(b, nchans, prm->poly_order, B, stats);
-    dd_rfi_window_kernel<<<dim3((unsigned)((nwin + kThreads / 32 - 1) / (kThreads / 32)), (unsigned)nrows), kThreads, 0,
-                           st>>>(X, nchans, nsamp, stride, beam_stride, prm->window, nwin, B, stats,
-                                 (double)prm->t_chan, own);
     dd_rfi_flags_kernel<<<(unsigned)std::min<int64_t>((nrows * nwin + kThreads - 1) / kThreads, 4096), kThreads, 0, st>>>(
-        own, nrows, nwin, flag);
+        wsum, nrows, nchans, nwin, prm->window, nsamp, B, stats, (double)prm->t_chan, flag, chan_flags);
     dd_rfi_spectrum_kernel<<<dim3((unsigned)nspec, (unsigned)nbeams), dim3(kSpecT, kSpecQ), 0, st>>>(
         X, nchans, nsamp, stride, beam_stride, prm->window, nwin, B, flag, m);
     dd_rfi_spectrum_stats_kernel<<<(unsigned)nbeams, kThreads, 0, st>>>(m, nsamp, stats);
+    dd_rfi_excess_kernel<<<dim3((unsigned)((ng4 + kThreads - 1) / kThreads), (unsigned)nbeams), kThreads, 0, st>>>(
+        m, nsamp, stats, (double)prm->t_spec, excess, any4, spec_flags);
     dd_rfi_apply_kernel<<<dim3((unsigned)ntile, (unsigned)nrows), kThreads, 0, st>>>(
-        X, nchans, nsamp, stride, beam_stride, prm->window, nwin, B, stats, flag, m, (double)prm->t_spec, chan_flags,
-        spec_flags);
+        X, nchans, nsamp, stride, beam_stride, prm->window, nwin, B, flag, excess, any4);
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess && bandpass)
         e = cudaMemcpyAsync(bandpass, b, (size_t)nrows * sizeof(double), cudaMemcpyDeviceToDevice, st);
