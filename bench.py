@@ -541,10 +541,18 @@ def next_rows(dd, torch, hbm_peak):
     del D
     # f3: RFI mitigation of config 3's input buffer, in place
     n_in = w.nsamp + 14845
-    X = torch.randn((w.nchans, n_in), dtype=torch.float32, device="cuda", generator=g).add_(20.0)
+    n_pad = (n_in + 63) // 64 * 64                       # row stride as the dedisperser's input buffer has it
+    # noise on a bandpass with channel-to-channel gain scatter (so that the fit's RMSE is a bandpass property, not the
+    # noise of a window mean), narrowband RFI in three channels and two broadband bursts (the recipe of PAPER.md:1176-1185)
+    X = torch.randn((w.nchans, n_pad), dtype=torch.float32, device="cuda", generator=g).add_(20.0)
+    X.add_(torch.randn((w.nchans, 1), dtype=torch.float32, device="cuda", generator=g).mul_(0.3))
+    for c in (100, 1777, 3000):
+        X[c, 50000:90000].add_(5.0)
+    for t in (123456, 200000):
+        X[:, t:t + 4].add_(3.0)
     rp = dd.dd_rfi_params(4, 512, 7.0, 5.0)
-    ms = _timed_ms(torch, lambda: dd.dd_rfi_mitigate(X, w.nchans, n_in, n_in, 0, 1, rp))
-    by = X.numel() * 8
+    ms = _timed_ms(torch, lambda: dd.dd_rfi_mitigate(X, w.nchans, n_in, n_pad, 0, 1, rp))
+    by = w.nchans * n_in * 8
     rows["f3_rfi"] = {"shape": "config 3 input, %d channels x %d samples float32; order 4, window 512, thresholds 7 / 5" % (w.nchans, n_in),
                       "ms": ms, "algorithmic_bytes": by, "bound": "hbm", "achieved_gbs": by / ms / 1e6, "peak_gbs": peak,
                       "frac": by / ms / 1e6 / peak, "gpu_launches": 8,

@@ -138,12 +138,13 @@ dd_post_stats_kernel(const T* __restrict__ D, int64_t stride, int64_t beam_strid
     for (int64_t t0 = (int64_t)threadIdx.x * kPer; t0 < n; t0 += kTile) {
         double m[kPer];
         medians4<T, W>(row, t0, n, m);
+        const double tc0 = (double)t0 - tm;               // (one integer conversion per four samples)
 #pragma unroll
         for (int e = 0; e < kPer; ++e)
             if (t0 + e < n) {
                 const double u = m[e] - y0;
                 su += u;
-                stu += ((double)(t0 + e) - tm) * u;
+                stu += (tc0 + (double)e) * u;
                 suu += u * u;
             }
     }
@@ -178,53 +179,61 @@ struct ApplyParams {
     unsigned long long* count;
 };
 
+constexpr int kApplyJ = 4;                     // block steps per thread of the apply kernel (amortises the row set-up)
+
 template <typename T, int W>
 __global__ void __launch_bounds__(kThreads)
 dd_post_apply_kernel(const T* __restrict__ D, const ApplyParams p)
 {
-    const int64_t r = blockIdx.x / p.ntiles;              // time tiles fastest (1-D grid: no 65535 limit on series)
-    const int beam = (int)(r / p.ndm), dm = (int)(r % p.ndm);
+    const unsigned r = blockIdx.x / p.ntiles;             // time tiles fastest (1-D grid: no 65535 limit on series)
+    const int beam = (int)(r / (unsigned)p.ndm), dm = (int)(r - (unsigned)beam * (unsigned)p.ndm);
     const T* row = D + (int64_t)beam * p.beam_stride + (int64_t)dm * p.stride;
-    const int64_t t0 = ((int64_t)(blockIdx.x % p.ntiles) * kThreads + threadIdx.x) * kPer;
-    if (t0 >= p.n) return;
-    double m[kPer];
-    medians4<T, W>(row, t0, p.n, m);
     double intercept = 0.0, slope = 0.0, sigma = 0.0;
     if (p.detrend) {
-        intercept = p.stats[r * 3 + 0];
-        slope = p.stats[r * 3 + 1];
-        sigma = p.stats[r * 3 + 2];
+        intercept = p.stats[(int64_t)r * 3 + 0];
+        slope = p.stats[(int64_t)r * 3 + 1];
+        sigma = p.stats[(int64_t)r * 3 + 2];
     }
     const double inv = sigma > 0.0 ? 1.0 / sigma : 0.0;    // sigma = 0: all-zero output (R17)
-    float out[kPer];
+    float* zrow = p.Z ? p.Z + (int64_t)beam * p.z_beam_stride + (int64_t)dm * p.z_stride : nullptr;
+    const int64_t tile0 = (int64_t)(blockIdx.x - r * p.ntiles) * kApplyJ;
+#pragma unroll 1
+    for (int j = 0; j < kApplyJ; ++j) {
+        const int64_t t0 = ((tile0 + j) * kThreads + threadIdx.x) * kPer;
+        if (t0 >= p.n) return;
+        double m[kPer];
+        medians4<T, W>(row, t0, p.n, m);
+        const double td0 = (double)t0;                     // exact; t0 + e as td0 + e is exact too
+        float out[kPer];
 #pragma unroll
-    for (int e = 0; e < kPer; ++e) {
-        double v = m[e];
-        if (p.detrend) v -= intercept + slope * (double)(t0 + e);
-        // un-normalised series are compared against n * sigma; same decision, same precision
-        const double snr = p.detrend ? v * inv : v;
-        if (p.normalise) v = snr;
-        out[e] = (float)v;
-        if (p.threshold_on && t0 + e < p.n && snr > p.nsigma) {
-            const unsigned long long at = atomicAdd(p.count, 1ull);
-            if ((int64_t)at < p.capacity) {
-                dd_candidate c;
-                c.beam = beam;
-                c.dm = dm;
-                c.t = (int32_t)(t0 + e);
-                c.value = (float)snr;
-                p.cand[at] = c;
+        for (int e = 0; e < kPer; ++e) {
+            double v = m[e];
+            if (p.detrend) v -= intercept + slope * (td0 + (double)e);
+            // un-normalised series are compared against n * sigma; same decision, same precision
+            const double snr = p.detrend ? v * inv : v;
+            if (p.normalise) v = snr;
+            out[e] = (float)v;
+            if (p.threshold_on && t0 + e < p.n && snr > p.nsigma) {
+                const unsigned long long at = atomicAdd(p.count, 1ull);
+                if ((int64_t)at < p.capacity) {
+                    dd_candidate c;
+                    c.beam = beam;
+                    c.dm = dm;
+                    c.t = (int32_t)(t0 + e);
+                    c.value = (float)snr;
+                    p.cand[at] = c;
+                }
             }
         }
-    }
-    if (p.Z) {
-        float* z = p.Z + (int64_t)beam * p.z_beam_stride + (int64_t)dm * p.z_stride + t0;
-        if (t0 + kPer <= p.n && (((uintptr_t)z) & 15) == 0) {
-            *reinterpret_cast<float4*>(z) = make_float4(out[0], out[1], out[2], out[3]);
-        } else {
+        if (zrow) {
+            float* z = zrow + t0;
+            if (t0 + kPer <= p.n && (((uintptr_t)z) & 15) == 0) {
+                *reinterpret_cast<float4*>(z) = make_float4(out[0], out[1], out[2], out[3]);
+            } else {
 #pragma unroll
-            for (int e = 0; e < kPer; ++e)
-                if (t0 + e < p.n) z[e] = out[e];
+                for (int e = 0; e < kPer; ++e)
+                    if (t0 + e < p.n) z[e] = out[e];
+            }
         }
     }
 }
@@ -289,7 +298,7 @@ int postprocess(int dtype, const void* D, int64_t stride, int64_t beam_stride, i
     if (Z && (const void*)Z == D && w > 1)
         return fail(DD_ERR_BAD_ARG, "in-place output needs median_window <= 1 (neighbours read each other's samples)");
     const int64_t nrows = (int64_t)nbeams * ndm;
-    const int64_t ntiles = (nsamp + kTile - 1) / kTile;
+    const int64_t ntiles = (nsamp + kTile * kApplyJ - 1) / (kTile * kApplyJ);      // grid tiles of the apply kernel
     if (nrows * ntiles > 2147483647LL) return fail(DD_ERR_UNSUPPORTED, "series x time tiles exceed one grid: split the call");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     double* own_stats = nullptr;

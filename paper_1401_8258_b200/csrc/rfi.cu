@@ -55,10 +55,11 @@ __global__ void __launch_bounds__(kThreads)
 dd_rfi_window_sums_kernel(const float* __restrict__ X, int nchans, int64_t n, int64_t stride, int64_t beam_stride,
                           int window, int nwin, double* __restrict__ wsum)
 {
-    const int64_t row = blockIdx.y;
+    const unsigned urow = blockIdx.y, ubeam = urow / (unsigned)nchans;       // 32-bit index arithmetic
+    const int64_t row = urow;
     const int k = blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
     if (k >= nwin) return;
-    const float* x = X + (row / nchans) * beam_stride + (row % nchans) * stride;
+    const float* x = X + (int64_t)ubeam * beam_stride + (int64_t)(urow - ubeam * (unsigned)nchans) * stride;
     const int64_t a = (int64_t)k * window, e = min(n, a + window);
     double s = 0.0;
     if ((window & 3) == 0 && e - a == window && (((uintptr_t)(x + a)) & 15) == 0) {
@@ -97,6 +98,9 @@ dd_rfi_fit_kernel(const double* __restrict__ b, int nchans, int order, double* _
     __shared__ double red[kThreads / 32];
     __shared__ double G[(kMaxOrder + 1) * (kMaxOrder + 2)];   // augmented [p+1][p+2]
     __shared__ double coef[kMaxOrder + 1];
+    __shared__ double rk[kMaxOrder + 1];                      // 1 / k of the Legendre recurrence
+    if (threadIdx.x <= kMaxOrder) rk[threadIdx.x] = threadIdx.x ? 1.0 / (double)threadIdx.x : 0.0;
+    __syncthreads();
     const int beam = blockIdx.x;
     const double* bb = b + (int64_t)beam * nchans;
     const int p = min(order, nchans - 1), np1 = p + 1;
@@ -104,7 +108,7 @@ dd_rfi_fit_kernel(const double* __restrict__ b, int nchans, int order, double* _
     auto legendre = [&](double x, double* P) {                // P[0..p]
         P[0] = 1.0;
         if (p >= 1) P[1] = x;
-        for (int k = 2; k <= p; ++k) P[k] = ((2.0 * k - 1.0) * x * P[k - 1] - (k - 1.0) * P[k - 2]) / (double)k;
+        for (int k = 2; k <= p; ++k) P[k] = ((2.0 * k - 1.0) * x * P[k - 1] - (k - 1.0) * P[k - 2]) * rk[k];
     };
     for (int i = 0; i < np1; ++i)
         for (int j = i; j <= np1; ++j) {                      // j == np1: right-hand side
@@ -169,7 +173,7 @@ dd_rfi_fit_kernel(const double* __restrict__ b, int nchans, int order, double* _
 __global__ void __launch_bounds__(kThreads)
 dd_rfi_flags_kernel(const double* __restrict__ wsum, int64_t nrows, int nchans, int nwin, int window, int64_t n,
                     const double* __restrict__ B, const double* __restrict__ stats, double t_chan,
-                    uint8_t* __restrict__ flag, uint8_t* __restrict__ chan_flags)
+                    uint8_t* __restrict__ flag, uint8_t* __restrict__ chan_flags, uint8_t* __restrict__ dirty)
 {
     const int64_t total = nrows * nwin;
     for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < total; i += (int64_t)gridDim.x * kThreads) {
@@ -183,6 +187,7 @@ dd_rfi_flags_kernel(const double* __restrict__ wsum, int64_t nrows, int nchans, 
         const bool f = own(k) || (k > 0 && own(k - 1)) || (k + 1 < nwin && own(k + 1));
         flag[i] = f;
         if (chan_flags) chan_flags[i] = f;
+        if (f) dirty[(row / nchans) * nwin + k] = 1;       // some channel of this beam is replaced in window k
     }
 }
 
@@ -191,17 +196,22 @@ constexpr int kSpecQ = kThreads * 4 / kSpecT; // channel slices per block (threa
 
 // 3a. m[beam][t] = mean over channels of the channel-clipped spectrum t.  Block = 128 spectra x 8 channel
 // slices; a thread sums its slice's channels in ascending order (every load a coalesced row segment), the
-// slices' partial sums meet in shared memory and are added in slice order.
+// slices' partial sums meet in shared memory and are added in slice order.  Windows in which no channel of the
+// beam is replaced (dirty[k] = 0: the usual case) skip the flag look-ups.  The block also leaves the sums of
+// (m_t - bmean) and (m_t - bmean)^2 over its spectra in part[beam][block] (bmean = mean fitted bandpass: a
+// shift close to the mean of the m_t), from which 3b forms mu and sigma.
 __global__ void __launch_bounds__(kSpecT * kSpecQ)
 dd_rfi_spectrum_kernel(const float* __restrict__ X, int nchans, int64_t n, int64_t stride, int64_t beam_stride,
                        int window, int nwin, const double* __restrict__ B, const uint8_t* __restrict__ flag,
-                       double* __restrict__ m)
+                       const uint8_t* __restrict__ dirty, const double* __restrict__ stats, double* __restrict__ m,
+                       double* __restrict__ part)
 {
-    __shared__ double part[kSpecQ][kSpecT];
+    __shared__ double acc[kSpecQ][kSpecT];
+    __shared__ double red[2][kSpecT / 32];
     const int beam = blockIdx.y, tx = threadIdx.x, q = threadIdx.y;
     const int64_t t = (int64_t)blockIdx.x * kSpecT + tx;
     const int64_t tc = min(t, n - 1);
-    const int k = (int)(tc / window);
+    const int k = (int)((unsigned)tc / (unsigned)window);
     const float* x = X + (int64_t)beam * beam_stride + tc;
     const uint8_t* fl = flag + (int64_t)beam * nchans * nwin + k;
     const double* Bb = B + (int64_t)beam * nchans;
@@ -209,44 +219,82 @@ dd_rfi_spectrum_kernel(const float* __restrict__ X, int nchans, int64_t n, int64
     const int c_lo = min(nchans, q * cq), c_hi = min(nchans, c_lo + cq);
     double s = 0.0;
     int c = c_lo;
-    for (; c + 8 <= c_hi; c += 8) {
-        float v[8];
-        uint8_t f[8];
+    if (!dirty[(int64_t)beam * nwin + k]) {
+        for (; c + 8 <= c_hi; c += 8) {
+            float v[8];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            v[j] = __ldg(x + (int64_t)(c + j) * stride);
-            f[j] = __ldg(fl + (int64_t)(c + j) * nwin);
+            for (int j = 0; j < 8; ++j) v[j] = __ldg(x + (int64_t)(c + j) * stride);
+#pragma unroll
+            for (int j = 0; j < 8; ++j) s += (double)v[j];
         }
+        for (; c < c_hi; ++c) s += (double)__ldg(x + (int64_t)c * stride);
+    } else {
+        for (; c + 8 <= c_hi; c += 8) {
+            float v[8];
+            uint8_t f[8];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) s += f[j] ? Bb[c + j] : (double)v[j];
+            for (int j = 0; j < 8; ++j) {
+                v[j] = __ldg(x + (int64_t)(c + j) * stride);
+                f[j] = __ldg(fl + (int64_t)(c + j) * nwin);
+            }
+#pragma unroll
+            for (int j = 0; j < 8; ++j) s += f[j] ? Bb[c + j] : (double)v[j];
+        }
+        for (; c < c_hi; ++c) s += __ldg(fl + (int64_t)c * nwin) ? Bb[c] : (double)__ldg(x + (int64_t)c * stride);
     }
-    for (; c < c_hi; ++c) s += __ldg(fl + (int64_t)c * nwin) ? Bb[c] : (double)__ldg(x + (int64_t)c * stride);
-    part[q][tx] = s;
+    acc[q][tx] = s;
     __syncthreads();
-    if (q == 0 && t < n) {
-        double tot = part[0][tx];
+    if (q == 0) {
+        double d1 = 0.0, d2 = 0.0;
+        if (t < n) {
+            double tot = acc[0][tx];
 #pragma unroll
-        for (int j = 1; j < kSpecQ; ++j) tot += part[j][tx];
-        m[(int64_t)beam * n + t] = tot / (double)nchans;
+            for (int j = 1; j < kSpecQ; ++j) tot += acc[j][tx];
+            tot /= (double)nchans;
+            m[(int64_t)beam * n + t] = tot;
+            d1 = tot - stats[beam * 4 + 1];
+            d2 = d1 * d1;
+        }
+        d1 = warp_sum(d1);
+        d2 = warp_sum(d2);
+        if ((tx & 31) == 0) {
+            red[0][tx >> 5] = d1;
+            red[1][tx >> 5] = d2;
+        }
+    }
+    __syncthreads();
+    if (q == 0 && tx == 0) {
+        double s1 = 0.0, s2 = 0.0;
+#pragma unroll
+        for (int w = 0; w < kSpecT / 32; ++w) {
+            s1 += red[0][w];
+            s2 += red[1][w];
+        }
+        part[((int64_t)beam * gridDim.x + blockIdx.x) * 2 + 0] = s1;
+        part[((int64_t)beam * gridDim.x + blockIdx.x) * 2 + 1] = s2;
     }
 }
 
-// 3b. stats[beam][2..3] = mean and population standard deviation over time of m (one block per beam)
+// 3b. stats[beam][2..3] = mean and population standard deviation over time of m, from the blocks' partial
+// sums about bmean (one block per beam, fixed order):  mu = bmean + S1 / n,  sigma^2 = S2 / n - (S1 / n)^2
 __global__ void __launch_bounds__(kThreads)
-dd_rfi_spectrum_stats_kernel(const double* __restrict__ m, int64_t n, double* __restrict__ stats)
+dd_rfi_spectrum_stats_kernel(const double* __restrict__ part, int nblocks, int64_t n, double* __restrict__ stats)
 {
     __shared__ double red[kThreads / 32];
     const int beam = blockIdx.x;
-    const double* mm = m + (int64_t)beam * n;
-    double s = 0.0;
-    for (int64_t t = threadIdx.x; t < n; t += kThreads) s += mm[t];
-    const double mu = block_sum(s, red) / (double)n;
-    double q = 0.0;
-    for (int64_t t = threadIdx.x; t < n; t += kThreads) q += (mm[t] - mu) * (mm[t] - mu);
-    q = block_sum(q, red);
+    const double* pp = part + (int64_t)beam * nblocks * 2;
+    double s1 = 0.0, s2 = 0.0;
+    for (int i = threadIdx.x; i < nblocks; i += kThreads) {
+        s1 += pp[2 * i];
+        s2 += pp[2 * i + 1];
+    }
+    s1 = block_sum(s1, red);
+    s2 = block_sum(s2, red);
     if (threadIdx.x == 0) {
-        stats[beam * 4 + 2] = mu;
-        stats[beam * 4 + 3] = sqrt(q / (double)n);
+        const double d = s1 / (double)n;
+        const double var = s2 / (double)n - d * d;
+        stats[beam * 4 + 2] = stats[beam * 4 + 1] + d;
+        stats[beam * 4 + 3] = var > 0.0 ? sqrt(var) : 0.0;
     }
 }
 
@@ -271,50 +319,76 @@ dd_rfi_excess_kernel(const double* __restrict__ m, int64_t n, const double* __re
     any4[(int64_t)beam * ((n + 3) / 4) + g] = any;
 }
 
+// t / d for 0 <= t < 2^31 as a multiply and a shift: mul = ceil(2^(31+l) / d), shift = 31 + l, l = ceil(log2 d)
+// (exact: the error term t e / 2^(31+l), e = mul d - 2^(31+l) < 2^l, stays below 1 / d)
+struct FastDiv { uint32_t mul, shift; };
+__device__ __forceinline__ uint32_t fast_div(uint32_t t, FastDiv f)
+{
+    return (uint32_t)(((uint64_t)t * f.mul) >> f.shift);
+}
+
+constexpr int kApplyJ = 4;                     // block steps per thread of the write pass (amortises the row set-up)
+
 // 4. the single write pass: channel replacement, spectrum excess, bandpass subtraction; four consecutive
-// samples per thread (16-byte accesses when the row allows); every value is formed in double and rounded once
+// samples per thread and step (16-byte accesses when the row allows); every value is formed in double and
+// rounded once
 __global__ void __launch_bounds__(kThreads)
 dd_rfi_apply_kernel(float* __restrict__ X, int nchans, int64_t n, int64_t stride, int64_t beam_stride, int window,
-                    int nwin, const double* __restrict__ B, const uint8_t* __restrict__ flag,
+                    int nwin, FastDiv div_window, const double* __restrict__ B, const uint8_t* __restrict__ flag,
                     const double* __restrict__ excess, const uint8_t* __restrict__ any4)
 {
-    const int64_t row = blockIdx.y;
-    const int beam = (int)(row / nchans);
-    const int64_t g = (int64_t)blockIdx.x * kThreads + threadIdx.x, t0 = 4 * g;
-    if (t0 >= n) return;
-    float* x = X + (int64_t)beam * beam_stride + (row % nchans) * stride + t0;
+    const unsigned urow = blockIdx.y, ubeam = urow / (unsigned)nchans;       // 32-bit index arithmetic
+    const int64_t row = urow;
+    float* xrow = X + (int64_t)ubeam * beam_stride + (int64_t)(urow - ubeam * (unsigned)nchans) * stride;
     const double Bc = B[row];
     const uint8_t* fl = flag + row * nwin;
-    const int k0 = (int)(t0 / window), k1 = (int)(min(t0 + 3, n - 1) / window);
-    const bool cf0 = fl[k0], cf1 = k1 != k0 ? (bool)fl[k1] : cf0;
-    const int64_t next = (int64_t)(k0 + 1) * window;       // first sample of the next window
-    const bool vec = t0 + 4 <= n && ((((uintptr_t)x) & 15) == 0);
-    float v[4];
-    if (vec) {
-        const float4 q = *reinterpret_cast<const float4*>(x);
-        v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
-    } else {
+    const double* exb = excess + (int64_t)ubeam * n;
+    const uint8_t* anyb = any4 + (int64_t)ubeam * ((n + 3) / 4);
+    const unsigned uw = (unsigned)window;
+#pragma unroll 1
+    for (int j = 0; j < kApplyJ; ++j) {
+        const int64_t g = ((int64_t)blockIdx.x * kApplyJ + j) * kThreads + threadIdx.x, t0 = 4 * g;
+        if (t0 >= n) return;
+        float* x = xrow + t0;
+        // window flags of the four samples (nsamp < 2^31 is checked by the host)
+        const unsigned ut0 = (unsigned)t0;
+        bool cf[4];
+        if (window >= 4) {                                  // at most one window boundary inside the four samples
+            const unsigned k0 = fast_div(ut0, div_window), next = (k0 + 1) * uw - ut0;   // samples left in window k0
+            const bool cf0 = fl[k0], cf1 = next < 4 && k0 + 1 < (unsigned)nwin ? (bool)fl[k0 + 1] : cf0;
 #pragma unroll
-        for (int e = 0; e < 4; ++e) v[e] = t0 + e < n ? x[e] : 0.0f;
-    }
-    double ex[4] = {0.0, 0.0, 0.0, 0.0};
-    if (any4[(int64_t)beam * ((n + 3) / 4) + g]) {
+            for (int e = 0; e < 4; ++e) cf[e] = (unsigned)e >= next ? cf1 : cf0;
+        } else {
 #pragma unroll
-        for (int e = 0; e < 4; ++e)
-            if (t0 + e < n) ex[e] = excess[(int64_t)beam * n + t0 + e];
-    }
+            for (int e = 0; e < 4; ++e) cf[e] = fl[min(fast_div(ut0 + e, div_window), (unsigned)nwin - 1)];
+        }
+        const bool vec = t0 + 4 <= n && ((((uintptr_t)x) & 15) == 0);
+        float v[4];
+        if (vec) {
+            const float4 q = *reinterpret_cast<const float4*>(x);
+            v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
+        } else {
 #pragma unroll
-    for (int e = 0; e < 4; ++e) {
-        const bool cf = t0 + e >= next ? cf1 : cf0;
-        const double val = (cf ? Bc : (double)v[e]) - ex[e];
-        v[e] = (float)(val - Bc);
-    }
-    if (vec) {
-        *reinterpret_cast<float4*>(x) = make_float4(v[0], v[1], v[2], v[3]);
-    } else {
+            for (int e = 0; e < 4; ++e) v[e] = t0 + e < n ? x[e] : 0.0f;
+        }
+        double ex[4] = {0.0, 0.0, 0.0, 0.0};
+        if (anyb[g]) {
 #pragma unroll
-        for (int e = 0; e < 4; ++e)
-            if (t0 + e < n) x[e] = v[e];
+            for (int e = 0; e < 4; ++e)
+                if (t0 + e < n) ex[e] = exb[t0 + e];
+        }
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const double val = (cf[e] ? Bc : (double)v[e]) - ex[e];
+            v[e] = (float)(val - Bc);
+        }
+        if (vec) {
+            *reinterpret_cast<float4*>(x) = make_float4(v[0], v[1], v[2], v[3]);
+        } else {
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+                if (t0 + e < n) x[e] = v[e];
+        }
     }
 }
 
@@ -330,12 +404,13 @@ int rfi_mitigate(float* X, int nchans, int64_t nsamp, int64_t stride, int64_t be
     if (prm->window < 1) return fail(DD_ERR_BAD_ARG, "window must be >= 1");
     if (!(prm->t_chan >= 0.0f) || !(prm->t_spec >= 0.0f)) return fail(DD_ERR_BAD_ARG, "thresholds must be >= 0");
     if (nsamp == 0) return DD_OK;
+    if (nsamp > 2147483647LL) return fail(DD_ERR_UNSUPPORTED, "nsamp must fit int32: split the call in time");
     if (!X) return fail(DD_ERR_BAD_ARG, "X is null");
     if (stride < nsamp) return fail(DD_ERR_BAD_ARG, "stride is shorter than nsamp");
     if (nbeams > 1 && beam_stride < (int64_t)nchans * stride) return fail(DD_ERR_BAD_ARG, "beam stride is shorter than a beam");
     const int64_t nrows = (int64_t)nbeams * nchans;
     const int64_t nwin64 = (nsamp + prm->window - 1) / prm->window;
-    const int64_t ntile = (nsamp + 4 * kThreads - 1) / (4 * kThreads);
+    const int64_t ntile = (nsamp + 4 * kThreads * kApplyJ - 1) / (4 * kThreads * kApplyJ);
     const int64_t nspec = (nsamp + kSpecT - 1) / kSpecT;
     if (nrows > 65535 || nbeams > 65535 || nwin64 > 2147483647LL || nspec > 2147483647LL)
         return fail(DD_ERR_UNSUPPORTED, "more than 65535 channel rows in one call: split the call by beam");
@@ -343,11 +418,13 @@ int rfi_mitigate(float* X, int nchans, int64_t nsamp, int64_t stride, int64_t be
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (nbeams == 1) beam_stride = 0;
     // workspace (doubles): b [nrows], B [nrows], stats [nbeams][4], m and excess [nbeams][nsamp], wsum [nrows][nwin];
-    // (bytes): flag [nrows][nwin], any4 [nbeams][ceil(nsamp / 4)]
+    // part [nbeams][nspec][2]; (bytes): flag [nrows][nwin], any4 [nbeams][ceil(nsamp / 4)], dirty [nbeams][nwin]
     const int64_t ng4 = (nsamp + 3) / 4;
-    const size_t nd = (size_t)nrows * 2 + (size_t)nbeams * 4 + (size_t)2 * nbeams * nsamp + (size_t)nrows * nwin;
+    const size_t nd = (size_t)nrows * 2 + (size_t)nbeams * 4 + (size_t)2 * nbeams * nsamp + (size_t)nrows * nwin +
+                      (size_t)2 * nbeams * nspec;
     char* ws = nullptr;
-    int rc = workspace_alloc((void**)&ws, nd * sizeof(double) + (size_t)nrows * nwin + (size_t)nbeams * ng4, cuda_stream);
+    int rc = workspace_alloc((void**)&ws, nd * sizeof(double) + (size_t)nrows * nwin + (size_t)nbeams * ng4 +
+                                              (size_t)nbeams * nwin, cuda_stream);
     if (rc != DD_OK) return rc;
     double* b = (double*)ws;
     double* B = b + nrows;
@@ -355,22 +432,35 @@ int rfi_mitigate(float* X, int nchans, int64_t nsamp, int64_t stride, int64_t be
     double* m = stats + (size_t)nbeams * 4;
     double* excess = m + (size_t)nbeams * nsamp;
     double* wsum = excess + (size_t)nbeams * nsamp;
-    uint8_t* flag = (uint8_t*)(wsum + (size_t)nrows * nwin);
+    double* part = wsum + (size_t)nrows * nwin;
+    uint8_t* flag = (uint8_t*)(part + (size_t)2 * nbeams * nspec);
     uint8_t* any4 = flag + (size_t)nrows * nwin;
+    uint8_t* dirty = any4 + (size_t)nbeams * ng4;
+    if (cudaMemsetAsync(dirty, 0, (size_t)nbeams * nwin, st) != cudaSuccess) {
+        cudaFreeAsync(ws, st);
+        return fail(DD_ERR_CUDA, "RFI mitigation: clearing the workspace failed");
+    }
     constexpr int kWPB = kThreads / 32;                    // warps per block
     dd_rfi_window_sums_kernel<<<dim3((unsigned)((nwin + kWPB - 1) / kWPB), (unsigned)nrows), kThreads, 0, st>>>(
         X, nchans, nsamp, stride, beam_stride, prm->window, nwin, wsum);
     dd_rfi_bandpass_kernel<<<(unsigned)((nrows + kWPB - 1) / kWPB), kThreads, 0, st>>>(wsum, nrows, nwin, nsamp, b);
     dd_rfi_fit_kernel<<<(unsigned)nbeams, kThreads, 0, st>>>(b, nchans, prm->poly_order, B, stats);
     dd_rfi_flags_kernel<<<(unsigned)std::min<int64_t>((nrows * nwin + kThreads - 1) / kThreads, 4096), kThreads, 0, st>>>(
-        wsum, nrows, nchans, nwin, prm->window, nsamp, B, stats, (double)prm->t_chan, flag, chan_flags);
+        wsum, nrows, nchans, nwin, prm->window, nsamp, B, stats, (double)prm->t_chan, flag, chan_flags, dirty);
     dd_rfi_spectrum_kernel<<<dim3((unsigned)nspec, (unsigned)nbeams), dim3(kSpecT, kSpecQ), 0, st>>>(
-        X, nchans, nsamp, stride, beam_stride, prm->window, nwin, B, flag, m);
-    dd_rfi_spectrum_stats_kernel<<<(unsigned)nbeams, kThreads, 0, st>>>(m, nsamp, stats);
+        X, nchans, nsamp, stride, beam_stride, prm->window, nwin, B, flag, dirty, stats, m, part);
+    dd_rfi_spectrum_stats_kernel<<<(unsigned)nbeams, kThreads, 0, st>>>(part, (int)nspec, nsamp, stats);
     dd_rfi_excess_kernel<<<dim3((unsigned)((ng4 + kThreads - 1) / kThreads), (unsigned)nbeams), kThreads, 0, st>>>(
         m, nsamp, stats, (double)prm->t_spec, excess, any4, spec_flags);
+    FastDiv dw;
+    {
+        uint32_t l = 0;
+        while ((1ull << l) < (uint64_t)prm->window) ++l;
+        dw.shift = 31 + l;
+        dw.mul = (uint32_t)(((1ull << dw.shift) + (uint64_t)prm->window - 1) / (uint64_t)prm->window);
+    }
     dd_rfi_apply_kernel<<<dim3((unsigned)ntile, (unsigned)nrows), kThreads, 0, st>>>(
-        X, nchans, nsamp, stride, beam_stride, prm->window, nwin, B, flag, excess, any4);
+        X, nchans, nsamp, stride, beam_stride, prm->window, nwin, dw, B, flag, excess, any4);
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess && bandpass)
         e = cudaMemcpyAsync(bandpass, b, (size_t)nrows * sizeof(double), cudaMemcpyDeviceToDevice, st);
