@@ -31,6 +31,11 @@ struct dd_subband {
     int64_t ms1 = 0, ms2 = 0;
     std::vector<dd_plan*> sub;           // per subband: its channels at the nominal DMs
     std::vector<dd_plan*> grp;           // per nominal group: the reduced filterbank at the group's DMs
+    // the plans of a step are independent small launches: they are spread over a few internal streams
+    // (fork from / join to the caller's stream with events) so that their ramp-up and tails overlap
+    static constexpr int kStreams = 4;
+    cudaStream_t aux[kStreams] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t fork = nullptr, join[kStreams] = {nullptr, nullptr, nullptr, nullptr};
 };
 
 namespace dd {
@@ -238,6 +243,11 @@ void dd_subband_destroy(dd_subband* s)
         if (p) dd_plan_destroy(p);
     for (dd_plan* p : s->grp)
         if (p) dd_plan_destroy(p);
+    for (int i = 0; i < dd_subband::kStreams; ++i) {
+        if (s->aux[i]) cudaStreamDestroy(s->aux[i]);
+        if (s->join[i]) cudaEventDestroy(s->join[i]);
+    }
+    if (s->fork) cudaEventDestroy(s->fork);
     delete s;
 }
 
@@ -276,6 +286,14 @@ int dd_subband_create(dd_subband** out, int nchans, double fch1, double foff, do
                             d1 - d0);
         if (rc == DD_OK) s->ms2 = std::max(s->ms2, dd_plan_max_shift(s->grp[g]));
     }
+    if (rc == DD_OK && ndm > 0) {
+        cudaError_t e = cudaEventCreateWithFlags(&s->fork, cudaEventDisableTiming);
+        for (int i = 0; i < dd_subband::kStreams && e == cudaSuccess; ++i) {
+            e = cudaStreamCreateWithFlags(&s->aux[i], cudaStreamNonBlocking);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->join[i], cudaEventDisableTiming);
+        }
+        if (e != cudaSuccess) rc = fail(DD_ERR_CUDA, std::string("subband streams: ") + cudaGetErrorString(e));
+    }
     if (rc != DD_OK) {
         dd_subband_destroy(s);
         return rc;
@@ -306,13 +324,34 @@ int dd_subband_execute(dd_subband* s, const float* X, int64_t in_stride, float* 
     float* S = nullptr;
     int rc = workspace_alloc((void**)&S, (size_t)s->nsb * s->nnom * pitch * sizeof(float), cuda_stream);
     if (rc != DD_OK) return rc;
-    for (int b = 0; b < s->nsb && rc == DD_OK; ++b)
+    constexpr int K = dd_subband::kStreams;
+    // fork: the internal streams wait for everything queued on the caller's stream so far
+    auto fork = [&]() {
+        cudaError_t e = cudaEventRecord(s->fork, st);
+        for (int i = 0; i < K && e == cudaSuccess; ++i) e = cudaStreamWaitEvent(s->aux[i], s->fork, 0);
+        return e;
+    };
+    // join: the caller's stream waits for the internal streams
+    auto join = [&]() {
+        cudaError_t e = cudaSuccess;
+        for (int i = 0; i < K && e == cudaSuccess; ++i) {
+            e = cudaEventRecord(s->join[i], s->aux[i]);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(st, s->join[i], 0);
+        }
+        return e;
+    };
+    cudaError_t ce = fork();
+    for (int b = 0; b < s->nsb && rc == DD_OK && ce == cudaSuccess; ++b)
         rc = dd_execute(s->sub[b], X + (int64_t)b * s->ncs * in_stride, in_stride, 0, S + (int64_t)b * s->nnom * pitch,
-                        pitch, 0, n1, 1, cuda_stream);
-    for (int g = 0; g < s->nnom && rc == DD_OK; ++g)
+                        pitch, 0, n1, 1, s->aux[b % K]);
+    if (ce == cudaSuccess) ce = join();                   // (also after a failed launch: nothing is left running on S)
+    if (ce == cudaSuccess && rc == DD_OK) ce = fork();
+    for (int g = 0; g < s->nnom && rc == DD_OK && ce == cudaSuccess; ++g)
         rc = dd_execute(s->grp[g], S + (int64_t)g * pitch, (int64_t)s->nnom * pitch, 0,
-                        D + (int64_t)g * s->nds * out_stride, out_stride, 0, nsamp_out, 1, cuda_stream);
+                        D + (int64_t)g * s->nds * out_stride, out_stride, 0, nsamp_out, 1, s->aux[g % K]);
+    if (ce == cudaSuccess) ce = join();
     cudaFreeAsync(S, st);
+    if (ce != cudaSuccess) return fail(DD_ERR_CUDA, std::string("subband dedispersion: ") + cudaGetErrorString(ce));
     return rc;
 }
 

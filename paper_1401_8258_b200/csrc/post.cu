@@ -34,14 +34,18 @@ constexpr int kThreads = 512;
 constexpr int kPer = 4;                       // consecutive samples per thread
 constexpr int kTile = kThreads * kPer;        // samples per block step
 
+
+// min / max as single instructions (FMNMX / IMNMX); the series hold no NaN by contract (R14: not handled)
+__device__ __forceinline__ float mn(float a, float b) { return fminf(a, b); }
+__device__ __forceinline__ float mx(float a, float b) { return fmaxf(a, b); }
+__device__ __forceinline__ int32_t mn(int32_t a, int32_t b) { return min(a, b); }
+__device__ __forceinline__ int32_t mx(int32_t a, int32_t b) { return max(a, b); }
 template <typename T> __device__ __forceinline__ void cmpx(T& a, T& b)
 {
-    const T lo = a < b ? a : b, hi = a < b ? b : a;
+    const T lo = mn(a, b), hi = mx(a, b);
     a = lo;
     b = hi;
 }
-template <typename T> __device__ __forceinline__ T mn(T a, T b) { return a < b ? a : b; }
-template <typename T> __device__ __forceinline__ T mx(T a, T b) { return a < b ? b : a; }
 // median of W values: selection only (the result is one of the inputs), static indices, branch-free.
 // W = 3 and 5 use the short min / max forms (4 and 10 operations: the median of five is the median of
 // the fifth value, the larger of the two pair minima and the smaller of the two pair maxima); the
