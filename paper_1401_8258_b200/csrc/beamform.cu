@@ -15,11 +15,12 @@
 // (mma.sync m16n8k16) is the natural instruction: tcgen05 would need the unpacked voltages staged
 // through shared memory (4x the bytes of the packed input) for a K of only 64.  The weights are split
 // into two fp16 terms (hi + lo, |W - hi - lo| <= 2^-22 |W|), so the result has FP32 accuracy.
-// Measured (32 antennas, 16 beams, 1024 channels x 2^16 samples): 2.9 ms = 2.2 TB/s = 34 % of the HBM
-// copy bandwidth, 183 Tflop/s of fp16 MMAs issued (two per useful product); neither more resident warps
-// (128 / 158 registers) nor smaller weight chunks change the time: the bound is the issue rate of the
-// warp-level MMA on this part.  A tcgen05 version (voltages unpacked to shared memory, M padded to 64)
-// is the next step.
+// Measured (32 antennas, 16 beams, 1024 channels x 2^16 samples): 2.6 ms = 2.4 TB/s = 37 % of the HBM copy
+// bandwidth, 210 Tflop/s of fp16 MMAs issued (two per useful product).  What binds is the accumulate latency of
+// the warp-level MMA at two to three warps per scheduler (154-164 registers): with the k-step loop outermost every
+// MMA goes to a different accumulator (16 independent chains; 2.94 -> 2.63 ms); the tensor pipe is ~35 % busy, DRAM
+// latency is not exposed (prefetching the next voltages into L2 changes nothing), more resident warps at 128
+// registers spill.  A tcgen05 version (voltages unpacked to shared memory, M padded to 64) is the next step.
 // The thesis' kernel (Alg. 2) kept one FP32 accumulator per beam in registers and the weights in shared
 // memory, and was bound by shared-memory requests.
 #include <cuda_fp16.h>
@@ -134,24 +135,28 @@ dd_beamform_kernel(const uint8_t* __restrict__ V, const uint32_t* __restrict__ A
                     for (int e = 0; e < 4; ++e) ah[s][mt][e] = al[s][mt][e] = 0u;
                 }
             }
+        // the chunk's 2 kKC words of every sample of the warp (the four lanes of a quad read the same words), all
+        // loads first; then k-step outermost, so that consecutive MMAs go to different accumulators (16 independent
+        // chains instead of two: the accumulate latency of the warp-level MMA is what two warps per scheduler expose)
+        uint32_t w[kNT][2 * kKC];
 #pragma unroll
         for (int nt = 0; nt < kNT; ++nt) {
             const int64_t t = min(t0 + 8 * nt + g, nsamp - 1);            // the tail repeats the last sample (never stored)
             const uint32_t* vs = vrow + t * wps + 2 * kc;
-            // the chunk's 2 kKC words of this sample (32 antennas); the four lanes of a quad read the same words
-            uint32_t w[2 * kKC];
 #pragma unroll
-            for (int i = 0; i < 2 * kKC; ++i) w[i] = (2 * kc + i < wps) ? __ldg(vs + i) : 0u;
+            for (int i = 0; i < 2 * kKC; ++i) w[nt][i] = (2 * kc + i < wps) ? __ldg(vs + i) : 0u;
+        }
 #pragma unroll
-            for (int s = 0; s < kKC; ++s) {
+        for (int s = 0; s < kKC; ++s) {
+#pragma unroll
+            for (int nt = 0; nt < kNT; ++nt) {
                 // B fragment of k-step s: antenna 8 s + q (word 2 s, byte q) and antenna 8 s + q + 4 (word 2 s + 1, byte q)
-                const uint32_t b0 = nibbles_to_half2((w[2 * s] >> (8 * q)) & 0xffu);
-                const uint32_t b1 = nibbles_to_half2((w[2 * s + 1] >> (8 * q)) & 0xffu);
+                const uint32_t b0 = nibbles_to_half2((w[nt][2 * s] >> (8 * q)) & 0xffu);
+                const uint32_t b1 = nibbles_to_half2((w[nt][2 * s + 1] >> (8 * q)) & 0xffu);
 #pragma unroll
-                for (int mt = 0; mt < MT; ++mt) {
-                    mma16816(acc[mt][nt], ah[s][mt], b0, b1);
-                    mma16816(acc[mt][nt], al[s][mt], b0, b1);
-                }
+                for (int mt = 0; mt < MT; ++mt) mma16816(acc[mt][nt], ah[s][mt], b0, b1);
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) mma16816(acc[mt][nt], al[s][mt], b0, b1);
             }
         }
     }
