@@ -194,6 +194,9 @@ int beamform_power_u4(const uint8_t* V, int nants, int nchans, int64_t nsamp, co
     if (out_stride < nsamp) return fail(DD_ERR_BAD_ARG, "out_stride is shorter than nsamp");
     if (nbeams > 1 && out_beam_stride < (int64_t)nchans * out_stride)
         return fail(DD_ERR_BAD_ARG, "out_beam_stride is shorter than a beam");
+    // up to 128 antennas: the tcgen05 kernel (beamform_tc.cu); wider arrays: the warp-level MMA kernel below
+    if (beamform_tc_ok(nants, nbeams))
+        return beamform_tc_launch(V, nants, nchans, nsamp, W, nbeams, P, out_stride, out_beam_stride, cuda_stream);
     const int MT = nbeams > 8 ? 2 : 1;
     const int nbg = (nbeams + 8 * MT - 1) / (8 * MT);
     const int KS = (nants + 7) / 8;

@@ -95,6 +95,10 @@ int post_launches(const dd_post_params* prm, bool want_series);
 // coherent beamformer (beamform.cu)
 int beamform_power_u4(const uint8_t* V, int nants, int nchans, int64_t nsamp, const float* W, int nbeams, float* P,
                       int64_t out_stride, int64_t out_beam_stride, void* cuda_stream);
+// the same on the tcgen05 tensor cores (beamform_tc.cu): shapes it takes, and the launch
+bool beamform_tc_ok(int nants, int nbeams);
+int beamform_tc_launch(const uint8_t* V, int nants, int nchans, int64_t nsamp, const float* W, int nbeams, float* P,
+                       int64_t out_stride, int64_t out_beam_stride, void* cuda_stream);
 // RFI mitigation (rfi.cu)
 int rfi_mitigate(float* X, int nchans, int64_t nsamp, int64_t stride, int64_t beam_stride, int nbeams,
                  const dd_rfi_params* prm, double* bandpass, double* fit, double* stats, uint8_t* chan_flags,

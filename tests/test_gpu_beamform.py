@@ -43,7 +43,9 @@ def gpu_beamform(V, W, pad=0, beam_pad=0):
 
 
 @pytest.mark.parametrize("nch,nt,na,nb", [(4, 300, 32, 16), (3, 1000 + 13, 32, 5), (2, 64, 8, 1), (5, 257, 4, 3),
-                                          (2, 500, 64, 24), (1, 130, 36, 9), (2, 1, 32, 16)])
+                                          (2, 500, 64, 24), (1, 130, 36, 9), (2, 1, 32, 16),
+                                          (2, 300, 128, 40),     # four K atoms, two beam groups (tcgen05 kernel)
+                                          (1, 200, 132, 10)])    # more than 128 antennas: the warp-level MMA kernel
 def test_against_the_oracle(nch, nt, na, nb):
     g = np.random.default_rng(nch * 1000 + nt + na + nb)
     V = g.integers(0, 256, (nch, nt, na), dtype=np.uint8)
