@@ -164,47 +164,58 @@ dd_beamform_tc_kernel(const TcParams p)
             if (t < p.nsamp) {
                 const int beam0 = bg * p.NB + (c0 >> 1);
                 float* pp = p.P + (int64_t)beam0 * p.out_beam_stride + (int64_t)f * p.out_stride + t;
+                if (beam0 + 16 <= p.nbeams) {
 #pragma unroll
-                for (int q = 0; q < 16; ++q) {
-                    const float re = __uint_as_float(v[2 * q]), im = __uint_as_float(v[2 * q + 1]);
-                    if (beam0 + q < p.nbeams) *pp = re * re + im * im;
-                    pp += p.out_beam_stride;
+                    for (int q = 0; q < 16; ++q) {
+                        const float re = __uint_as_float(v[2 * q]), im = __uint_as_float(v[2 * q + 1]);
+                        *pp = re * re + im * im;
+                        pp += p.out_beam_stride;
+                    }
+                } else {
+#pragma unroll
+                    for (int q = 0; q < 16; ++q) {
+                        const float re = __uint_as_float(v[2 * q]), im = __uint_as_float(v[2 * q + 1]);
+                        if (beam0 + q < p.nbeams) *pp = re * re + im * im;
+                        pp += p.out_beam_stride;
+                    }
                 }
             }
         }
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     };
 
-    int ntiles = 0;
-#pragma unroll 1
-    for (int j = 0; j < kTcTilesPerBlock; ++j) {
+    // the packed voltages of this thread's sample of tile j: loaded one tile ahead (registers), so that the loads
+    // are in flight while the previous tile is multiplied and written out
+    uint32_t wv[natoms * 8];
+    auto load_tile = [&](int j) {
         const int64_t t = tblock + (int64_t)j * 128 + tid;
-        if (tblock + (int64_t)j * 128 >= p.nsamp) break;
-        ntiles = j + 1;
-        // unpack this thread's sample into row tid of A[j & 1]
-        uint8_t* a = As + (j & 1) * natoms * 16384;
-        const uint32_t* vs = vrow + min(t, p.nsamp - 1) * wps;
-        const uint32_t rowoff = (uint32_t)((tid >> 3) * 1024 + (tid & 7) * 128), rx = (uint32_t)(tid & 7);
+        const uint32_t* vs = vrow + min(t, p.nsamp - 1) * wps;       // the tail repeats the last sample (never stored)
         if ((wps & 3) == 0 && (((uintptr_t)vs) & 15) == 0) {
 #pragma unroll
             for (int c4 = 0; c4 < natoms * 2; ++c4) {
                 uint4 w = make_uint4(0u, 0u, 0u, 0u);
                 if (4 * c4 < wps) w = __ldg(reinterpret_cast<const uint4*>(vs) + c4);
-                const uint32_t ww[4] = {w.x, w.y, w.z, w.w};
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    const int c = 4 * c4 + i;
-                    *reinterpret_cast<uint4*>(a + (c >> 3) * 16384 + rowoff + (((uint32_t)(c & 7) ^ rx) << 4)) =
-                        unpack_word(ww[i]);                 // (a zero word unpacks to zeros)
-                }
+                wv[4 * c4] = w.x; wv[4 * c4 + 1] = w.y; wv[4 * c4 + 2] = w.z; wv[4 * c4 + 3] = w.w;
             }
         } else {
 #pragma unroll
-            for (int c = 0; c < natoms * 8; ++c) {
-                const uint32_t w = c < wps ? __ldg(vs + c) : 0u;
-                *reinterpret_cast<uint4*>(a + (c >> 3) * 16384 + rowoff + (((uint32_t)(c & 7) ^ rx) << 4)) = unpack_word(w);
-            }
+            for (int c = 0; c < natoms * 8; ++c) wv[c] = c < wps ? __ldg(vs + c) : 0u;
         }
+    };
+    const uint32_t rowoff = (uint32_t)((tid >> 3) * 1024 + (tid & 7) * 128), rx = (uint32_t)(tid & 7);
+    if (tblock < p.nsamp) load_tile(0);
+
+    int ntiles = 0;
+#pragma unroll 1
+    for (int j = 0; j < kTcTilesPerBlock; ++j) {
+        if (tblock + (int64_t)j * 128 >= p.nsamp) break;
+        ntiles = j + 1;
+        // unpack this thread's sample into row tid of A[j & 1] (a zero word unpacks to zeros)
+        uint8_t* a = As + (j & 1) * natoms * 16384;
+#pragma unroll
+        for (int c = 0; c < natoms * 8; ++c)
+            *reinterpret_cast<uint4*>(a + (c >> 3) * 16384 + rowoff + (((uint32_t)(c & 7) ^ rx) << 4)) = unpack_word(wv[c]);
+        if (j + 1 < kTcTilesPerBlock && tblock + (int64_t)(j + 1) * 128 < p.nsamp) load_tile(j + 1);
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();
         if (tid == 0) {
