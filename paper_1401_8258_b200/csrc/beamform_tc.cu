@@ -31,7 +31,7 @@ namespace dd {
 namespace {
 
 constexpr int kTcThreads = 128;               // one sample (accumulator row) per thread
-constexpr int kTcTilesPerBlock = 16;          // time tiles of 128 samples per block
+constexpr int kTcTilesPerBlock = 32;          // time tiles of 128 samples per block
 constexpr int kTcMaxAtoms = 4;                // 128-byte K atoms (32 antennas each): up to 128 antennas
 constexpr int kTcMaxNB = 32;                  // beams per group: N = 64 accumulator columns
 
