@@ -569,7 +569,7 @@ def next_rows(dd, torch, hbm_peak):
     rows["f4_beamformer"] = {"shape": "%d antennas (4-bit complex) x %d channels x %d samples -> %d beams, detected power float32" % (na, nch, nt, nb),
                              "ms": ms, "algorithmic_bytes": by, "bound": "hbm", "achieved_gbs": by / ms / 1e6, "peak_gbs": peak,
                              "frac": by / ms / 1e6 / peak, "tflops": flops / ms / 1e9, "gpu_launches": 2,
-                             "note": "8 Na Nb flops per (channel, sample) on the tensor cores (mma.sync fp16 x2, fp32 accumulate)"}
+                             "note": "8 Na Nb flops per (channel, sample) on the tensor cores (tcgen05.mma fp16 x2, fp32 accumulators in TMEM)"}
     del V, W, P
     # f2: subband (32 channels per subband, 16 trials per nominal DM) vs the exact kernel, config 2's shape as float32
     w2 = synth.scaled(synth.WORKLOADS[2], dtype="f32")
