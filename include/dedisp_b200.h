@@ -64,7 +64,9 @@ enum { DD_KERNEL_AUTO    = 0,
        DD_KERNEL_DIRECT  = 3,   /* one thread per output sample, operands straight from global memory / L2;
                                    AUTO takes it for tiny plans (nchans * ndm <= 4096), which are bound by
                                    launch latency and grid size, not by any pipe (decided from the plan
-                                   alone, so all calls of a plan add in the same order) */
+                                   alone, so all calls of a plan add in the same order); on series of
+                                   1e5 samples and more DD_KERNEL_PS / DD_KERNEL_GENERIC are up to 1.8x
+                                   faster for such plans: choose them with dd_plan_set_kernel */
        DD_KERNEL_PS      = 2 }; /* TMA-staged kernels (float32 and uint8) with partial sums of 4-8 adjacent
                                    channels shared between the trials of a 64/128-trial tile; plans whose
                                    per-trial delay steps are too coarse for them run DD_KERNEL_GENERIC
