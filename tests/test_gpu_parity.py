@@ -657,3 +657,49 @@ def test_random_shapes_against_the_oracle(dtype):
         assert_parity(w, X, D)
         done += 1
     assert dd.DD_KERNEL_PS in kinds and len(kinds) >= 2            # the draw exercises fast and fallback kernels
+
+
+def test_many_random_plans_partial_sum_kernel_agrees_with_the_channel_vector_kernel():
+    """Breadth beyond what the oracle can cover in seconds: 120 random plans (channel counts that are not multiples
+    of the group size, sorted random and uniform DM lists, one or two beams, ragged sizes) through the float32
+    partial-sum kernel and through the channel-vector kernel (itself compared with the oracle above); the two
+    add in different orders, so they must agree within twice north_star's tolerance, |D1 - D2| <= 2e-5 * A."""
+    import torch
+    rng = np.random.default_rng(20261105)
+    nps = 0
+    for it in range(120):
+        nch = int(rng.choice([16, 24, 37, 64, 100, 128, 200, 256, 333, 512]))
+        ndm = int(rng.integers(1, 400))
+        nsamp = int(rng.integers(1, 5000))
+        fch1 = float(rng.choice([150.0, 418.0, 800.0, 1550.0]))
+        band = float(rng.choice([5.0, 20.0, 100.0, 300.0])) * fch1 / 1550.0
+        tsamp = float(rng.choice([51.2e-6, 64e-6, 1e-3]))
+        step = float(rng.choice([0.01, 0.05, 0.1, 0.25, 1.0]))
+        dms = np.sort(rng.uniform(0, step * ndm, ndm)) if it % 3 else np.arange(ndm) * step
+        p = dd.Plan(dd.DD_F32, nch, fch1, -band / nch, tsamp, dms)
+        ms = p.max_shift()
+        if ms > 60000:
+            p.destroy()
+            continue
+        nb = int(rng.integers(1, 3))
+        stride = (nsamp + ms + 3) // 4 * 4
+        X = torch.randn((nb, nch, stride), device="cuda")
+        D1 = torch.empty((nb, ndm, nsamp), device="cuda")
+        D2, A = torch.empty_like(D1), torch.empty_like(D1)
+        a = lambda x, d: (x, stride, nch * stride, d, nsamp, ndm * nsamp, nsamp, nb)
+        p.set_kernel(dd.DD_KERNEL_GENERIC)
+        p.execute(*a(X, D2))
+        p.execute(*a(X.abs(), A))
+        try:
+            p.set_kernel(dd.DD_KERNEL_PS)
+        except dd.DedispError:                      # delay steps too coarse for shared partial sums
+            p.destroy()
+            continue
+        assert p.kernel_for(*a(X, D1)) == dd.DD_KERNEL_PS
+        p.execute(*a(X, D1))
+        torch.cuda.synchronize()
+        r = ((D1 - D2).abs() / (2e-5 * A + 1e-30)).max().item()
+        assert r <= 1.0, (it, nch, ndm, nsamp, fch1, band, tsamp, step, r)
+        nps += 1
+        p.destroy()
+    assert nps >= 60
