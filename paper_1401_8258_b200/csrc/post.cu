@@ -98,12 +98,26 @@ __device__ __forceinline__ void medians4(const T* __restrict__ row, int64_t t0, 
             x[i] = __ldg(row + j);
         }
     }
+    if constexpr (W == 5) {
+        // two adjacent windows share four values: with b <= c the middle two of the shared four, the median of
+        // the four and a fifth value e is e clamped to [b, c] -- 12 min / max operations per two medians
 #pragma unroll
-    for (int e = 0; e < kPer; ++e) {
-        T v[W];
+        for (int e = 0; e < kPer; e += 2) {
+            const T p0 = mn(x[e + 1], x[e + 2]), p1 = mx(x[e + 1], x[e + 2]);
+            const T q0 = mn(x[e + 3], x[e + 4]), q1 = mx(x[e + 3], x[e + 4]);
+            const T u = mx(p0, q0), v = mn(p1, q1);            // the middle two, in either order
+            const T b = mn(u, v), c = mx(u, v);
+            m[e] = (double)mn(mx(x[e], b), c);
+            m[e + 1] = (double)mn(mx(x[e + 5], b), c);
+        }
+    } else {
 #pragma unroll
-        for (int i = 0; i < W; ++i) v[i] = x[e + i];
-        m[e] = (double)median_of<T, W>(v);
+        for (int e = 0; e < kPer; ++e) {
+            T v[W];
+#pragma unroll
+            for (int i = 0; i < W; ++i) v[i] = x[e + i];
+            m[e] = (double)median_of<T, W>(v);
+        }
     }
 }
 
