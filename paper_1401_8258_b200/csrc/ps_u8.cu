@@ -68,7 +68,8 @@ constexpr int kCE = 8;                    // ints per step entry of the descript
 constexpr int kDNChunks = 0;
 constexpr int kDBytes = 1;                // bytes of this descriptor that are in use (multiple of 16)
 constexpr int kDBase = 4;                 // first staged sample of the group's rows, relative to t0 (multiple of 16)
-constexpr int kDTrial = 12;               // [KB] word offset of trial j's first operand in the partial sums
+constexpr int kDTrial = 12;               // [KB / 2] uint16 x KB: word offset of trial j's first operand in the partial sums
+                                          //      (the region keeps KB ints)
 // kDTrial + KB:                             [nchunks][kCE]: [0..3] byte offset, from the stage's first byte, of the
                                           //      aligned word lane 0 reads in channel k (zero pad if missing);
                                           //      [4], [5] first even-u / odd-u word the step writes (even numbers)
@@ -259,11 +260,23 @@ dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
                 if (lane == 0) mbar_arrive(&ready[bn]);
             }
             // Step 3: one word per trial, sample pair and group
+            // (16-bit offsets, two per int: one 8- or 16-byte read per warp)
             int tro[KW];
+            {
+                uint32_t tw[KW / 2];
+                const int32_t* tp = Ds + st * p.desc_ints + kDTrial + warp * (KW / 2);
+                if (KW == 8) {
+                    const uint4 tr = *reinterpret_cast<const uint4*>(tp);
+                    tw[0] = tr.x; tw[1] = tr.y; tw[KW / 2 - 2] = tr.z; tw[KW / 2 - 1] = tr.w;
+                } else {
+                    const uint2 tr = *reinterpret_cast<const uint2*>(tp);
+                    tw[0] = tr.x; tw[1] = tr.y;
+                }
 #pragma unroll
-            for (int q = 0; q < KW / 4; ++q) {
-                const int4 tr = *reinterpret_cast<const int4*>(Ds + st * p.desc_ints + kDTrial + warp * KW + 4 * q);
-                tro[4 * q] = tr.x; tro[4 * q + 1] = tr.y; tro[4 * q + 2] = tr.z; tro[4 * q + 3] = tr.w;
+                for (int q = 0; q < KW / 2; ++q) {
+                    tro[2 * q] = (int)(tw[q] & 0xffffu);
+                    tro[2 * q + 1] = (int)(tw[q] >> 16);
+                }
             }
             const uint32_t* ps = Ps + b * p.psw + lane;
             mbar_wait(&ready[b], (g / kPB) & 1);         // step 2 of g is done everywhere
@@ -415,8 +428,9 @@ static int try_build_psu8(dd_plan* p, int kw)
             for (int j = 0; j < kKB; ++j) {
                 const int d = std::min(tile * kKB + j, ndm - 1);
                 const int o = h.shift[(size_t)d * nch + c0] - rows[slot[j]].umin;
-                ds[kDTrial + j] = rowbase[2 * slot[j] + (o & 1)] + (o >> 1);
-                bounds_ok = bounds_ok && o >= 0 && ds[kDTrial + j] + kTB / 2 <= t->psw;
+                const int off = rowbase[2 * slot[j] + (o & 1)] + (o >> 1);
+                reinterpret_cast<uint16_t*>(ds + kDTrial)[j] = (uint16_t)off;
+                bounds_ok = bounds_ok && o >= 0 && off >= 0 && off < 65536 && off + kTB / 2 <= t->psw;
             }
         }
     wok[wk] = bounds_ok;
