@@ -62,7 +62,7 @@ constexpr int kMaxSmem = 200 * 1024;
 constexpr int kFlushGroups = 64;          // 64 groups * 4 channels * 255 = 65280 < 65536
 constexpr int kChunk = 64;                // even-u words (= 128 samples) a warp step writes ...
 constexpr int kStepW = 62;                // ... of which the last two are rewritten by the next step
-constexpr int kCE = 8;                    // ints per step entry of the descriptor
+constexpr int kCE = 4;                    // ints per step entry of the descriptor (six 16-bit fields: one 16-byte read)
 
 // descriptor layout (ints), one per (trial tile, channel group)
 constexpr int kDNChunks = 0;
@@ -153,10 +153,12 @@ dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
     struct Words { uint32_t w0, w1, w2, w3; };
     auto pre_load = [&](uint32_t xa, const int4 o) {
         Words r;
-        r.w0 = lds_u32(xa + o.x); r.w1 = lds_u32(xa + o.y); r.w2 = lds_u32(xa + o.z); r.w3 = lds_u32(xa + o.w);
+        r.w0 = lds_u32(xa + ((uint32_t)o.x & 0xffffu)); r.w1 = lds_u32(xa + ((uint32_t)o.x >> 16));
+        r.w2 = lds_u32(xa + ((uint32_t)o.y & 0xffffu)); r.w3 = lds_u32(xa + ((uint32_t)o.y >> 16));
         return r;
     };
-    auto pre_store = [&](uint32_t* ps, const int4 dst, const Words& r) {
+    auto pre_store = [&](uint32_t* ps, const int4 e, const Words& r) {
+        const uint2 dst = make_uint2((uint32_t)e.z & 0xffffu, (uint32_t)e.z >> 16);
         // (b0 | b1 << 16) and (b2 | b3 << 16) of each channel word, summed over the channels:
         // partial sums S0..S3 of this lane's four samples
         const uint32_t lo = __byte_perm(r.w0, 0, 0x4140) + __byte_perm(r.w1, 0, 0x4140) +
@@ -178,13 +180,15 @@ dd_ps_u8_kernel(const PsU8Params p, const __grid_constant__ CUtensorMap tmap)
         const int4* ct = reinterpret_cast<const int4*>(ds + kDChunk);
         int c = warp;
         for (; c + kWarps < nchunks; c += 2 * kWarps) {
-            const int4 ea = ct[2 * c], eb = ct[2 * (c + kWarps)];
-            const int4 da = ct[2 * c + 1], db = ct[2 * (c + kWarps) + 1];
+            const int4 ea = ct[c], eb = ct[c + kWarps];
             const Words a = pre_load(xa, ea), b = pre_load(xa, eb);
-            pre_store(ps, da, a);
-            pre_store(ps, db, b);
+            pre_store(ps, ea, a);
+            pre_store(ps, eb, b);
         }
-        if (c < nchunks) pre_store(ps, ct[2 * c + 1], pre_load(xa, ct[2 * c]));
+        if (c < nchunks) {
+            const int4 ea = ct[c];
+            pre_store(ps, ea, pre_load(xa, ea));
+        }
     };
 
     uint32_t acc[KW][NK];
@@ -409,7 +413,8 @@ static int try_build_psu8(dd_plan* p, int kw)
                 // x_k[u0 + r_k + 4 l ..+3], u0 = umin + 124 c, i.e. byte a0 + 4 l of the staged rows,
                 // a0 = u0 + r_k - base: copy (a0 & 3), word (a0 >> 2) + l
                 for (int c = 0; c < ns; ++c, ++step) {
-                    int32_t* ce = ds + kDChunk + kCE * step;
+                    uint16_t* ce16 = reinterpret_cast<uint16_t*>(ds + kDChunk + kCE * step);
+                    int ce[6];
                     for (int k = 0; k < kG; ++k) {
                         const int rk = k == 0 ? 0 : rows[r].key[k - 1];
                         const int a0 = rows[r].umin + 2 * kStepW * c + rk - base;
@@ -420,6 +425,10 @@ static int try_build_psu8(dd_plan* p, int kw)
                     ce[4] = rowbase[2 * r] + kStepW * c;
                     ce[5] = rowbase[2 * r + 1] + kStepW * c;
                     bounds_ok = bounds_ok && ce[4] + kChunk <= t->psw && ce[5] + kStepW <= t->psw;
+                    for (int k = 0; k < 6; ++k) {
+                        bounds_ok = bounds_ok && ce[k] >= 0 && ce[k] < 65536;
+                        ce16[k] = (uint16_t)ce[k];
+                    }
                 }
                 flat += 2 * (kStepW * ns + 2);
             }
