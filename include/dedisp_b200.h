@@ -218,6 +218,22 @@ int     dd_postprocess(int dtype, const void* D, int64_t stride, int64_t beam_st
                        float* Z, int64_t z_stride, int64_t z_beam_stride, double* stats,
                        dd_candidate* cand, int64_t capacity, unsigned long long* count,
                        void* cuda_stream);
+/* dd_postprocess for callers that must not allocate device memory (CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc): same steps, same kernels, same results, but the per-series statistics
+ * table -- the path's only scratch memory -- is a static device array inside the library instead of a
+ * workspace allocation, so the call reaches no cudaMalloc / cudaMallocAsync / cudaFree.  Arguments as
+ * dd_postprocess without `stats` (the caller still passes D, Z, cand, count: all DEVICE).
+ * Limits: nbeams * ndm <= DD_POSTPROCESS_STATIC_MAX_SERIES, else DD_ERR_UNSUPPORTED (nothing is enqueued).
+ * The array (3 doubles per series, 384 KiB) is held by every GPU that loads the library until the process
+ * exits, is shared by ALL calls on that device and keeps the last call's statistics (nothing needs to
+ * start at zero: each call writes every entry it reads).  Calls that overlap on the GPU (different
+ * streams, no ordering between them) race on it; calls on one stream, or ordered by events, are safe. */
+#define DD_POSTPROCESS_STATIC_MAX_SERIES 16384
+int     dd_postprocess_static(int dtype, const void* D, int64_t stride, int64_t beam_stride, int ndm,
+                              int64_t nsamp, int nbeams, const dd_post_params* params,
+                              float* Z, int64_t z_stride, int64_t z_beam_stride,
+                              dd_candidate* cand, int64_t capacity, unsigned long long* count,
+                              void* cuda_stream);
 /* number of kernels dd_postprocess launches for these parameters (bench.py's gpu_launches) */
 int     dd_postprocess_launches(const dd_post_params* params, int want_series);
 

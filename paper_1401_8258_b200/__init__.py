@@ -9,5 +9,6 @@ from .binding import (  # noqa: F401
     DedispError, Plan, Stream, TimeBin, Subband, lib, dd_diagonal_dm, dd_downsample2_f32,
     dd_version, dd_max_shift, dd_shift_table, dd_release_workspaces,
     dd_rfi_params, dd_rfi_mitigate, dd_beamform_power_u4, dd_post_params, post_params, CANDIDATE_DTYPE, dd_postprocess, dd_postprocess_launches,
+    dd_postprocess_static, POSTPROCESS_STATIC_MAX_SERIES,
     dd_dedisperse_f32, dd_dedisperse_u8_i32, dd_dedisperse_f32_host, dd_dedisperse_u8_i32_host,
 )

@@ -62,6 +62,8 @@ SIGNATURES = {
     "dd_execute_host": (C.c_int, [_vp, _vp, _i64, _i64, _vp, _i64, _i64, _i64, C.c_int]),
     "dd_postprocess": (C.c_int, [C.c_int, _vp, _i64, _i64, C.c_int, _i64, C.c_int, C.POINTER(dd_post_params),
                                  _vp, _i64, _i64, _vp, _vp, _i64, _vp, _vp]),
+    "dd_postprocess_static": (C.c_int, [C.c_int, _vp, _i64, _i64, C.c_int, _i64, C.c_int, C.POINTER(dd_post_params),
+                                        _vp, _i64, _i64, _vp, _i64, _vp, _vp]),
     "dd_postprocess_launches": (C.c_int, [C.POINTER(dd_post_params), C.c_int]),
     "dd_search_host": (C.c_int, [_vp, _vp, _i64, _i64, _i64, C.c_int, C.POINTER(dd_post_params), _vp, _i64,
                                  C.POINTER(_i64)]),
@@ -206,6 +208,17 @@ def dd_postprocess(dtype, D, stride, beam_stride, ndm, nsamp, nbeams, params, Z=
     _check(lib().dd_postprocess(dtype, _ptr(D), stride, beam_stride, ndm, nsamp, nbeams, C.byref(params), _ptr(Z),
                                 z_stride, z_beam_stride, _ptr(stats), _ptr(cand), capacity, _ptr(count),
                                 _stream_ptr(stream)), "dd_postprocess")
+
+
+POSTPROCESS_STATIC_MAX_SERIES = 16384      # DD_POSTPROCESS_STATIC_MAX_SERIES of include/dedisp_b200.h
+
+
+def dd_postprocess_static(dtype, D, stride, beam_stride, ndm, nsamp, nbeams, params, Z=None, z_stride=0,
+                          z_beam_stride=0, cand=None, capacity=0, count=None, stream=None) -> None:
+    """dd_postprocess without device allocations (statistics in the library's static device array)."""
+    _check(lib().dd_postprocess_static(dtype, _ptr(D), stride, beam_stride, ndm, nsamp, nbeams, C.byref(params),
+                                       _ptr(Z), z_stride, z_beam_stride, _ptr(cand), capacity, _ptr(count),
+                                       _stream_ptr(stream)), "dd_postprocess_static")
 
 
 def dd_rfi_mitigate(X, nchans, nsamp, stride, beam_stride, nbeams, params, bandpass=None, fit=None, stats=None,

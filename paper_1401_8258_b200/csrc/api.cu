@@ -608,6 +608,17 @@ int dd_postprocess(int dtype, const void* D, int64_t stride, int64_t beam_stride
                        cand, capacity, count, cuda_stream);
 }
 
+int dd_postprocess_static(int dtype, const void* D, int64_t stride, int64_t beam_stride, int ndm, int64_t nsamp,
+                          int nbeams, const dd_post_params* params, float* Z, int64_t z_stride,
+                          int64_t z_beam_stride, dd_candidate* cand, int64_t capacity, unsigned long long* count,
+                          void* cuda_stream)
+{
+    int rc = require_sm100(nullptr);
+    if (rc != DD_OK) return rc;
+    return postprocess_static(dtype, D, stride, beam_stride, ndm, nsamp, nbeams, params, Z, z_stride, z_beam_stride,
+                              cand, capacity, count, cuda_stream);
+}
+
 int dd_postprocess_launches(const dd_post_params* params, int want_series)
 {
     if (!params) return fail(DD_ERR_BAD_ARG, "params is null");

@@ -92,6 +92,9 @@ int postprocess(int dtype, const void* D, int64_t stride, int64_t beam_stride, i
                 const dd_post_params* prm, float* Z, int64_t z_stride, int64_t z_beam_stride, double* stats,
                 dd_candidate* cand, int64_t capacity, unsigned long long* count, void* cuda_stream);
 int post_launches(const dd_post_params* prm, bool want_series);
+int postprocess_static(int dtype, const void* D, int64_t stride, int64_t beam_stride, int ndm, int64_t nsamp,
+                       int nbeams, const dd_post_params* prm, float* Z, int64_t z_stride, int64_t z_beam_stride,
+                       dd_candidate* cand, int64_t capacity, unsigned long long* count, void* cuda_stream);
 // coherent beamformer (beamform.cu)
 int beamform_power_u4(const uint8_t* V, int nants, int nchans, int64_t nsamp, const float* W, int nbeams, float* P,
                       int64_t out_stride, int64_t out_beam_stride, void* cuda_stream);

@@ -23,6 +23,7 @@
 #include <cuda_runtime.h>
 
 #include <cmath>
+#include <mutex>
 
 #include "dd_internal.h"
 
@@ -332,6 +333,66 @@ int postprocess(int dtype, const void* D, int64_t stride, int64_t beam_stride, i
                                    : launch_t<int32_t>(w, D, nrows, ap, stats, st);
     if (own_stats) cudaFreeAsync(own_stats, st);
     return rc;
+}
+
+// ---- the entry point that allocates nothing (dd_postprocess_static) --------------------------------
+// The only scratch memory of the post-processing path is the table of per-series statistics (intercept,
+// slope, sigma: 3 doubles per series) that the statistics kernel writes and the apply kernel reads.
+// Here it lives in a file-scope device array (every GPU that loads the library holds these 384 KiB
+// until exit), so the call reaches no cudaMalloc / cudaMallocAsync / cudaFree.  Every entry the apply kernel
+// reads has been written by the statistics kernel of the SAME call (rows 0 .. nbeams*ndm-1), so nothing
+// has to start at zero and nothing is cleared; the array keeps the last call's statistics.  All calls
+// on one device share it: two calls that overlap on the GPU (different streams) race.
+namespace {
+
+constexpr int64_t kStaticMaxSeries = DD_POSTPROCESS_STATIC_MAX_SERIES;
+static __device__ __align__(256) double g_static_stats[kStaticMaxSeries * 3];
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mutex;
+double* g_static_addr[kStaticMaxDevices] = {};            // device address of g_static_stats, per device
+
+// In host code `g_static_stats` is the host-side stand-in of the symbol, not a device address: the
+// address is looked up once per device, with that device current.
+int static_stats_address(double** out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(DD_ERR_CUDA, std::string("cudaGetDevice: ") + cudaGetErrorString(e));
+    if (dev < 0 || dev >= kStaticMaxDevices) return fail(DD_ERR_UNSUPPORTED, "device ordinal beyond 63");
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[dev]) {
+        double* ptr = nullptr;
+        e = cudaGetSymbolAddress((void**)&ptr, g_static_stats);
+        if (e != cudaSuccess || !ptr) {
+            cudaGetLastError();
+            return fail(DD_ERR_CUDA, std::string("cudaGetSymbolAddress(static statistics table): ") +
+                                         cudaGetErrorString(e));
+        }
+        g_static_addr[dev] = ptr;
+    }
+    *out = g_static_addr[dev];
+    return DD_OK;
+}
+
+}  // namespace
+
+int postprocess_static(int dtype, const void* D, int64_t stride, int64_t beam_stride, int ndm, int64_t nsamp,
+                       int nbeams, const dd_post_params* prm, float* Z, int64_t z_stride, int64_t z_beam_stride,
+                       dd_candidate* cand, int64_t capacity, unsigned long long* count, void* cuda_stream)
+{
+    if (ndm < 0 || nbeams < 1) return fail(DD_ERR_BAD_ARG, "bad ndm / nbeams");
+    if ((int64_t)nbeams * ndm > kStaticMaxSeries)
+        return fail(DD_ERR_UNSUPPORTED,
+                    "dd_postprocess_static: nbeams * ndm = " + std::to_string((int64_t)nbeams * ndm) +
+                        " series exceed the static statistics table (DD_POSTPROCESS_STATIC_MAX_SERIES = " +
+                        std::to_string(kStaticMaxSeries) + "); split the call or use dd_postprocess");
+    double* stats = nullptr;
+    const int rc = static_stats_address(&stats);
+    if (rc != DD_OK) return rc;
+    // with a statistics table passed in, postprocess() allocates and frees nothing
+    return postprocess(dtype, D, stride, beam_stride, ndm, nsamp, nbeams, prm, Z, z_stride, z_beam_stride, stats,
+                       cand, capacity, count, cuda_stream);
 }
 
 }  // namespace dd
