@@ -24,6 +24,7 @@
 
 #include <cmath>
 #include <mutex>
+#include <type_traits>
 
 #include "dd_internal.h"
 
@@ -67,10 +68,11 @@ template <typename T, int W> __device__ __forceinline__ T median_of(T (&v)[W])
     }
 }
 
-// The kPer medians (as doubles) of samples t0 .. t0+kPer-1 of one series; window indices clamped to
-// [0, n-1] (R15).  Samples past the end give 0 (never used).
+// The kPer medians of samples t0 .. t0+kPer-1 of one series; window indices clamped to
+// [0, n-1] (R15).  Samples past the end give the clamped windows' medians (never used).
+// n < 2^31 (checked by the caller): 32-bit sample indices.
 template <typename T, int W>
-__device__ __forceinline__ void medians4(const T* __restrict__ row, int64_t t0, int64_t n, double (&m)[kPer])
+__device__ __forceinline__ void medians4(const T* __restrict__ row, unsigned t0, unsigned n, T (&m)[kPer])
 {
     constexpr int H = (W - 1) / 2;
     T x[kPer + 2 * H];
@@ -94,8 +96,8 @@ __device__ __forceinline__ void medians4(const T* __restrict__ row, int64_t t0, 
     } else {
 #pragma unroll
         for (int i = 0; i < kPer + 2 * H; ++i) {
-            int64_t j = t0 - H + i;
-            j = j < 0 ? 0 : (j > n - 1 ? n - 1 : j);
+            int64_t j = (int64_t)t0 - H + i;
+            j = j < 0 ? 0 : (j > (int64_t)n - 1 ? (int64_t)n - 1 : j);
             x[i] = __ldg(row + j);
         }
     }
@@ -108,8 +110,8 @@ __device__ __forceinline__ void medians4(const T* __restrict__ row, int64_t t0, 
             const T q0 = mn(x[e + 3], x[e + 4]), q1 = mx(x[e + 3], x[e + 4]);
             const T u = mx(p0, q0), v = mn(p1, q1);            // the middle two, in either order
             const T b = mn(u, v), c = mx(u, v);
-            m[e] = (double)mn(mx(x[e], b), c);
-            m[e + 1] = (double)mn(mx(x[e + 5], b), c);
+            m[e] = mn(mx(x[e], b), c);
+            m[e + 1] = mn(mx(x[e + 5], b), c);
         }
     } else {
 #pragma unroll
@@ -117,10 +119,12 @@ __device__ __forceinline__ void medians4(const T* __restrict__ row, int64_t t0, 
             T v[W];
 #pragma unroll
             for (int i = 0; i < W; ++i) v[i] = x[e + i];
-            m[e] = (double)median_of<T, W>(v);
+            m[e] = median_of<T, W>(v);
         }
     }
 }
+
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 __device__ __forceinline__ double block_sum(double v, double* red)
 {
@@ -150,22 +154,40 @@ dd_post_stats_kernel(const T* __restrict__ D, int64_t stride, int64_t beam_strid
     const int64_t r = blockIdx.x;
     const T* row = D + (r / ndm) * beam_stride + (r % ndm) * stride;
     const double tm = 0.5 * (double)(n - 1);
-    double first[kPer];
-    medians4<T, W>(row, 0, n, first);
-    const double y0 = first[0];
+    const unsigned n32 = (unsigned)n;
+    T first[kPer];
+    medians4<T, W>(row, 0u, n32, first);
+    const double y0 = (double)first[0];
     double su = 0.0, stu = 0.0, suu = 0.0;
-    for (int64_t t0 = (int64_t)threadIdx.x * kPer; t0 < n; t0 += kTile) {
-        double m[kPer];
-        medians4<T, W>(row, t0, n, m);
-        const double tc0 = (double)t0 - tm;               // (one integer conversion per four samples)
+    double tc0 = (double)(threadIdx.x * kPer) - tm;       // t0 - tm as a running double (exact: multiples of 1/2)
+    for (unsigned t0 = threadIdx.x * kPer; t0 < n32; t0 += kTile, tc0 += (double)kTile) {
+        // one load group per thread and trip leaves too few bytes in flight (3 blocks x 512 threads x 16 bytes
+        // per SM): ask L2 for the trip after next (no register cost; 1.01 -> 0.79 ms on config 3's plane)
+        if (t0 + 2 * kTile < n32) prefetch_l2(row + t0 + 2 * kTile);
+        T m[kPer];
+        medians4<T, W>(row, t0, n32, m);
+        double u[kPer];
 #pragma unroll
-        for (int e = 0; e < kPer; ++e)
-            if (t0 + e < n) {
-                const double u = m[e] - y0;
-                su += u;
-                stu += (tc0 + (double)e) * u;
-                suu += u * u;
-            }
+        for (int e = 0; e < kPer; ++e) u[e] = (double)m[e] - y0;
+        if (t0 + kPer <= n32) {
+            // four samples at once: sum u, sum e u and sum u^2 of the group, then tc0 (sum u) + sum e u:
+            // 16 double operations per four samples instead of 28 (the build has --fmad=false: the fused
+            // multiply-adds here are explicit)
+            const double s1 = (u[0] + u[1]) + (u[2] + u[3]);
+            const double s2 = fma(3.0, u[3], fma(2.0, u[2], u[1]));
+            const double q = fma(u[3], u[3], fma(u[2], u[2], fma(u[1], u[1], u[0] * u[0])));
+            su += s1;
+            stu = fma(tc0, s1, stu) + s2;
+            suu += q;
+        } else {
+#pragma unroll
+            for (int e = 0; e < kPer; ++e)
+                if (t0 + e < n32) {
+                    su += u[e];
+                    stu = fma(tc0 + (double)e, u[e], stu);
+                    suu = fma(u[e], u[e], suu);
+                }
+        }
     }
     su = block_sum(su, red);
     stu = block_sum(stu, red);
@@ -187,7 +209,7 @@ dd_post_stats_kernel(const T* __restrict__ D, int64_t stride, int64_t beam_strid
 struct ApplyParams {
     int64_t stride, beam_stride, n;
     int ndm;
-    unsigned ntiles;
+    unsigned ntiles, steps;                                // grid tiles per series, block steps per tile
     int detrend, normalise, threshold_on;
     double nsigma;
     const double* stats;
@@ -198,7 +220,7 @@ struct ApplyParams {
     unsigned long long* count;
 };
 
-constexpr int kApplyJ = 4;                     // block steps per thread of the apply kernel (amortises the row set-up)
+constexpr int kApplyJ = 16;                    // most block steps per thread of the apply kernel (long running prefetch, row set-up amortised)
 
 template <typename T, int W>
 __global__ void __launch_bounds__(kThreads)
@@ -215,24 +237,57 @@ dd_post_apply_kernel(const T* __restrict__ D, const ApplyParams p)
     }
     const double inv = sigma > 0.0 ? 1.0 / sigma : 0.0;    // sigma = 0: all-zero output (R17)
     float* zrow = p.Z ? p.Z + (int64_t)beam * p.z_beam_stride + (int64_t)dm * p.z_stride : nullptr;
-    const int64_t tile0 = (int64_t)(blockIdx.x - r * p.ntiles) * kApplyJ;
+    // Threshold-only calls (no series output) screen in single precision.  With sigma > 0 and n sigma >= 0 a
+    // sample passes  (m - line(t)) / sigma > n sigma  only if  m > line(t) + n sigma * sigma - delta =: L(t),
+    // delta <= 2^-48 S the rounding of the double evaluation, S = |slope| n + |intercept| + n sigma * sigma.
+    // lo(t) = fl32(b t + a), a = intercept + n sigma * sigma - 2^-21 S rounded down, lies below L(t) for all
+    // t < n (the float evaluation of the line is off by at most 2^-22 |slope| n + 2^-23 |a|).  Samples
+    // above lo(t) -- a handful per series at 6 sigma -- take the double-precision decision below, so the
+    // candidates are exactly those of the unscreened evaluation.
+    const bool screen = !zrow && p.threshold_on && sigma > 0.0 && p.nsigma >= 0.0;
+    float scr_a = 0.0f, scr_b = 0.0f;
+    if (screen) {
+        const double level = p.nsigma * sigma;
+        const double margin = 0x1p-21 * (fabs(slope) * (double)p.n + fabs(intercept) + level);
+        scr_a = __double2float_rd(intercept + level - margin);
+        scr_b = (float)slope;
+    }
+    const unsigned n32 = (unsigned)p.n;
+    const unsigned tile0 = (blockIdx.x - r * p.ntiles) * p.steps;
+    {   // as in the statistics kernel: ask L2 for the next two steps, then for the step after next in every step
+        const unsigned tp = (tile0 * kThreads + threadIdx.x) * kPer;
+        if (p.steps > 1 && tp + kTile < n32) prefetch_l2(row + tp + kTile);
+    }
 #pragma unroll 1
-    for (int j = 0; j < kApplyJ; ++j) {
-        const int64_t t0 = ((tile0 + j) * kThreads + threadIdx.x) * kPer;
-        if (t0 >= p.n) return;
-        double m[kPer];
-        medians4<T, W>(row, t0, p.n, m);
+    for (unsigned j = 0; j < p.steps; ++j) {
+        const unsigned t0 = ((tile0 + j) * kThreads + threadIdx.x) * kPer;
+        if (t0 >= n32) return;
+        if (j + 2 < p.steps && t0 + 2 * kTile < n32) prefetch_l2(row + t0 + 2 * kTile);
+        T m[kPer];
+        medians4<T, W>(row, t0, n32, m);
+        if (screen) {
+            const float tf = (float)t0;
+            bool any = false;
+#pragma unroll
+            for (int e = 0; e < kPer; ++e) {
+                float mf;
+                if constexpr (std::is_integral<T>::value) mf = __int2float_ru((int)m[e]);   // never below m
+                else mf = (float)m[e];
+                any |= mf > fmaf(scr_b, tf + (float)e, scr_a);
+            }
+            if (!any) continue;
+        }
         const double td0 = (double)t0;                     // exact; t0 + e as td0 + e is exact too
         float out[kPer];
 #pragma unroll
         for (int e = 0; e < kPer; ++e) {
-            double v = m[e];
+            double v = (double)m[e];
             if (p.detrend) v -= intercept + slope * (td0 + (double)e);
             // un-normalised series are compared against n * sigma; same decision, same precision
             const double snr = p.detrend ? v * inv : v;
             if (p.normalise) v = snr;
             out[e] = (float)v;
-            if (p.threshold_on && t0 + e < p.n && snr > p.nsigma) {
+            if (p.threshold_on && t0 + e < n32 && snr > p.nsigma) {
                 const unsigned long long at = atomicAdd(p.count, 1ull);
                 if ((int64_t)at < p.capacity) {
                     dd_candidate c;
@@ -246,12 +301,12 @@ dd_post_apply_kernel(const T* __restrict__ D, const ApplyParams p)
         }
         if (zrow) {
             float* z = zrow + t0;
-            if (t0 + kPer <= p.n && (((uintptr_t)z) & 15) == 0) {
+            if (t0 + kPer <= n32 && (((uintptr_t)z) & 15) == 0) {
                 *reinterpret_cast<float4*>(z) = make_float4(out[0], out[1], out[2], out[3]);
             } else {
 #pragma unroll
                 for (int e = 0; e < kPer; ++e)
-                    if (t0 + e < p.n) z[e] = out[e];
+                    if (t0 + e < n32) z[e] = out[e];
             }
         }
     }
@@ -317,7 +372,10 @@ int postprocess(int dtype, const void* D, int64_t stride, int64_t beam_stride, i
     if (Z && (const void*)Z == D && w > 1)
         return fail(DD_ERR_BAD_ARG, "in-place output needs median_window <= 1 (neighbours read each other's samples)");
     const int64_t nrows = (int64_t)nbeams * ndm;
-    const int64_t ntiles = (nsamp + kTile * kApplyJ - 1) / (kTile * kApplyJ);      // grid tiles of the apply kernel
+    // block steps per grid tile of the apply kernel: as many as still leave every SM a few waves of blocks
+    int steps = kApplyJ;
+    while (steps > 1 && nrows * ((nsamp + kTile * steps - 1) / (kTile * steps)) < 148 * 16) steps >>= 1;
+    const int64_t ntiles = (nsamp + (int64_t)kTile * steps - 1) / ((int64_t)kTile * steps);
     if (nrows * ntiles > 2147483647LL) return fail(DD_ERR_UNSUPPORTED, "series x time tiles exceed one grid: split the call");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     double* own_stats = nullptr;
@@ -326,7 +384,7 @@ int postprocess(int dtype, const void* D, int64_t stride, int64_t beam_stride, i
         if (rc != DD_OK) return rc;
         stats = own_stats;
     }
-    ApplyParams ap{stride, nbeams > 1 ? beam_stride : 0, nsamp, ndm, (unsigned)ntiles, prm->detrend, prm->normalise,
+    ApplyParams ap{stride, nbeams > 1 ? beam_stride : 0, nsamp, ndm, (unsigned)ntiles, (unsigned)steps, prm->detrend, prm->normalise,
                    prm->threshold_on, (double)prm->nsigma, stats, Z, z_stride, nbeams > 1 ? z_beam_stride : 0,
                    cand, capacity, count};
     const int rc = dtype == DD_F32 ? launch_t<float>(w, D, nrows, ap, stats, st)

@@ -181,6 +181,43 @@ def test_edges_and_argument_errors():
         assert ei.value.code == dd.DD_ERR_BAD_ARG
 
 
+def test_threshold_only_calls_list_exactly_the_candidates_of_calls_with_series_output():
+    """Without a series output the apply kernel screens samples in single precision before the double
+    decision (post.cu); the candidate list must be exactly the one of the unscreened evaluation.  Cases that
+    stress the screen: levels and slopes large against sigma (coarse float line), thresholds that many samples
+    sit next to (n sigma = 0, 0.5), integer series, ragged lengths."""
+    cases = []
+    for seed, (nb, ndm, n) in enumerate([(1, 7, 10001), (2, 3, 2049), (1, 2, 40000), (1, 3, 5)]):
+        cases.append((series(300 + seed, nb, ndm, n), "f32"))
+    D = series(310, 1, 4, 30011)
+    cases.append(((D + np.float32(3e6)).astype(np.float32), "level 3e6"))       # ulp(level) = 0.25 ~ sigma / 2 .. 100
+    t = np.arange(30011, dtype=np.float64)
+    cases.append(((D + 40.0 * t).astype(np.float32), "slope 40"))
+    cases.append(((D - 55.0 * t - 1e5).astype(np.float32), "slope -55"))
+    cases.append((series(311, 1, 3, 9000, dtype=np.int32), "i32"))
+    cases.append((series(312, 1, 3, 9000, dtype=np.int32) + np.int32(2 ** 30), "i32 level 2^30"))
+    cases.append((series(313, 1, 3, 9000, dtype=np.int32) - np.int32(2 ** 30), "i32 level -2^30"))
+    checked = 0
+    for D, name in cases:
+        for w in (0, 5):
+            for nsig in (0.0, 0.5, 3.0, 6.0):
+                prm = dd.post_params(w, True, True, nsigma=nsig)
+                cap = D.size + 1
+                _, _, c1, n1 = run_post(D, prm, want_series=True, capacity=cap)
+                _, _, c2, n2 = run_post(D, prm, want_series=False, capacity=cap, stats=False)
+                assert n1 == n2, (name, w, nsig, n1, n2)
+                k1 = sorted(zip(c1["beam"].tolist(), c1["dm"].tolist(), c1["t"].tolist(), c1["value"].tolist()))
+                k2 = sorted(zip(c2["beam"].tolist(), c2["dm"].tolist(), c2["t"].tolist(), c2["value"].tolist()))
+                assert k1 == k2, (name, w, nsig)
+                checked += n1
+        # un-normalised output compares against n * sigma with the same screen
+        prm = dd.post_params(3, True, False, nsigma=4.0)
+        _, _, c1, n1 = run_post(D, prm, want_series=True, capacity=D.size + 1)
+        _, _, c2, n2 = run_post(D, prm, want_series=False, capacity=D.size + 1, stats=False)
+        assert n1 == n2 and sorted(c1.tolist()) == sorted(c2.tolist()), name
+    assert checked > 100000
+
+
 # ------------------------------------------------------------------ the chain: dedisperse -> post-process -> candidates
 
 @pytest.mark.parametrize("idx,nchans,ndm,nsamp,w", [(3, 512, 50, 8192 + 100, 0), (2, 256, 70, 9000, 3), (4, 128, 40, 6000, 5)])
