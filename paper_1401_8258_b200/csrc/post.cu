@@ -50,15 +50,42 @@ template <typename T> __device__ __forceinline__ void cmpx(T& a, T& b)
 }
 // median of W values: selection only (the result is one of the inputs), static indices, branch-free.
 // W = 3 and 5 use the short min / max forms (4 and 10 operations: the median of five is the median of
-// the fifth value, the larger of the two pair minima and the smaller of the two pair maxima); the
-// other windows a full odd-even transposition sort.
+// the fifth value, the larger of the two pair minima and the smaller of the two pair maxima); W = 7 a
+// 13-comparator selection network of which the compiler keeps the 20 min / max that reach v[3]; W = 9 three
+// sorted triples (the median of nine is the median of: the largest minimum, the median of the middles, the
+// smallest maximum; 30 operations).  Both checked on all 0/1 inputs (min / max networks: the 0-1 principle).
+template <typename T> __device__ __forceinline__ T med3(T a, T b, T c) { return mx(mn(a, b), mn(mx(a, b), c)); }
+template <typename T> __device__ __forceinline__ void sort3(T& a, T& b, T& c)
+{
+    cmpx(a, b);
+    cmpx(b, c);
+    cmpx(a, b);
+}
+// median of nine from three ascending triples
+template <typename T> __device__ __forceinline__ T med9_sorted(const T (&p)[3], const T (&q)[3], const T (&r)[3])
+{
+    return med3(mx(mx(p[0], q[0]), r[0]), med3(p[1], q[1], r[1]), mn(mn(p[2], q[2]), r[2]));
+}
 template <typename T, int W> __device__ __forceinline__ T median_of(T (&v)[W])
 {
     if constexpr (W == 3) {
-        return mx(mn(v[0], v[1]), mn(mx(v[0], v[1]), v[2]));
+        return med3(v[0], v[1], v[2]);
     } else if constexpr (W == 5) {
         const T lo = mx(mn(v[0], v[1]), mn(v[2], v[3])), hi = mn(mx(v[0], v[1]), mx(v[2], v[3]));
         return mx(mn(lo, hi), mn(mx(lo, hi), v[4]));
+    } else if constexpr (W == 7) {
+        cmpx(v[0], v[5]); cmpx(v[0], v[3]); cmpx(v[1], v[6]); cmpx(v[2], v[4]); cmpx(v[0], v[1]);
+        cmpx(v[3], v[5]); cmpx(v[2], v[6]); cmpx(v[2], v[3]); cmpx(v[3], v[6]); cmpx(v[4], v[5]);
+        cmpx(v[1], v[4]); cmpx(v[1], v[3]); cmpx(v[3], v[4]);
+        return v[3];
+    } else if constexpr (W == 9) {
+        T t[3][3];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            t[i][0] = v[3 * i], t[i][1] = v[3 * i + 1], t[i][2] = v[3 * i + 2];
+            sort3(t[i][0], t[i][1], t[i][2]);
+        }
+        return med9_sorted(t[0], t[1], t[2]);
     } else {
 #pragma unroll
         for (int round = 0; round < W; ++round)
@@ -113,6 +140,16 @@ __device__ __forceinline__ void medians4(const T* __restrict__ row, unsigned t0,
             m[e] = mn(mx(x[e], b), c);
             m[e + 1] = mn(mx(x[e + 5], b), c);
         }
+    } else if constexpr (W == 9) {
+        // window e is the triples starting at e, e + 3, e + 6: the four windows need ten sorted triples, not twelve
+        T t[10][3];
+#pragma unroll
+        for (int i = 0; i < 10; ++i) {
+            t[i][0] = x[i], t[i][1] = x[i + 1], t[i][2] = x[i + 2];
+            sort3(t[i][0], t[i][1], t[i][2]);
+        }
+#pragma unroll
+        for (int e = 0; e < kPer; ++e) m[e] = med9_sorted(t[e], t[e + 3], t[e + 6]);
     } else {
 #pragma unroll
         for (int e = 0; e < kPer; ++e) {
