@@ -216,6 +216,11 @@ dd_beamform_tc_kernel(const TcParams p)
         for (int c = 0; c < natoms * 8; ++c)
             *reinterpret_cast<uint4*>(a + (c >> 3) * 16384 + rowoff + (((uint32_t)(c & 7) ^ rx) << 4)) = unpack_word(wv[c]);
         if (j + 1 < kTcTilesPerBlock && tblock + (int64_t)(j + 1) * 128 < p.nsamp) load_tile(j + 1);
+        {   // one 16-byte load per thread and tile leaves too little in flight: ask L2 for the tile three ahead
+            // (32 antennas: 1.37 -> 1.27 ms)
+            const int64_t tp = tblock + (int64_t)(j + 3) * 128 + tid;
+            if (j + 3 < kTcTilesPerBlock && tp < p.nsamp) asm volatile("prefetch.global.L2 [%0];" ::"l"(vrow + tp * wps));
+        }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();
         if (tid == 0) {
