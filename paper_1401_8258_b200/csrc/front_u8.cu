@@ -19,29 +19,55 @@ namespace {
 
 constexpr int64_t kTailPad = 2048 + 16;   // a time tile may over-read its window by up to one tensor-copy box
 
-// One thread per output word; rows on grid.x (no 65535 limit on nbeams * nchans).
+// One thread per 16 output bytes of each copy; rows on grid.x (no 65535 limit on nbeams * nchans).
+// With the row start rounded down to 16 bytes (sh = bytes cut off, 0..15), the 16 bytes of copy r at vector k
+// are source bytes 16 k + sh + r ..: five consecutive words out of the three aligned vectors k, k+1, k+2, funnel-
+// shifted by 8 ((sh + r) & 3) bits.  WO = sh >> 2 is a template argument (register arrays need static indices);
+// copy r starts at word WO or WO + 1.  Only aligned vectors that hold at least one valid byte of the row are read
+// (the rest count as 0), so no access leaves the pages of the caller's buffer.  Loads and stores are 16 bytes wide (the one-word-per-thread form took 0.22 ms of config 2's
+// 4.50 ms step; this one 0.13 ms).
+template <int WO>
+__device__ __forceinline__ void shift_row(const uint4* __restrict__ srcv, uint8_t* __restrict__ dst, int64_t wcopy,
+                                          int sh, int64_t nvec, int64_t lastv)
+{
+    const int sub = sh & 3;
+    for (int64_t k = (int64_t)blockIdx.y * blockDim.x + threadIdx.x; k < nvec; k += (int64_t)gridDim.y * blockDim.x) {
+        const uint4 z = make_uint4(0u, 0u, 0u, 0u);
+        const uint4 q0 = k <= lastv ? __ldg(srcv + k) : z;
+        const uint4 q1 = k + 1 <= lastv ? __ldg(srcv + k + 1) : z;
+        const uint4 q2 = k + 2 <= lastv ? __ldg(srcv + k + 2) : z;
+        const uint32_t w[12] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w, q2.x, q2.y, q2.z, q2.w};
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const bool up = sub + r >= 4;                              // copy r starts one word further
+            const int bits = 8 * ((sub + r) & 3);
+            uint32_t o[4];
+#pragma unroll
+            for (int m = 0; m < 4; ++m) {
+                const uint32_t lo = up ? w[WO + m + 1] : w[WO + m], hi = up ? w[WO + m + 2] : w[WO + m + 1];
+                o[m] = __funnelshift_r(lo, hi, bits);
+            }
+            *reinterpret_cast<uint4*>(dst + r * wcopy + 16 * k) = make_uint4(o[0], o[1], o[2], o[3]);
+        }
+    }
+}
+
 __global__ void __launch_bounds__(256)
 dd_shift_copies_u8(const uint8_t* __restrict__ X, uint8_t* __restrict__ W, int64_t wcopy, int64_t wpitch,
                    int nchans, int64_t rowlen, int64_t in_stride, int64_t in_beam_stride)
 {
     const int64_t row = blockIdx.x;                                   // beam * nchans + channel
     const uint8_t* src = X + (row / nchans) * in_beam_stride + (row % nchans) * in_stride;
-    const int sh = (int)((uintptr_t)src & 3);
-    const uint32_t* srcw = reinterpret_cast<const uint32_t*>(src - sh);   // aligned words covering the row
-    const int64_t nwords = (rowlen + 3) >> 2;
-    const int64_t lastw = (sh + rowlen - 1) >> 2;                     // last aligned word holding a valid byte
-    for (int64_t i = (int64_t)blockIdx.y * blockDim.x + threadIdx.x; i < nwords;
-         i += (int64_t)gridDim.y * blockDim.x) {
-        const uint32_t w0 = __ldg(srcw + i);
-        const uint32_t w1 = i + 1 <= lastw ? __ldg(srcw + i + 1) : 0u;
-        const uint32_t w2 = i + 2 <= lastw ? __ldg(srcw + i + 2) : 0u;
-#pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            const int b = sh + r;                                     // 0..6 bytes into (w0,w1,w2)
-            const uint32_t lo = b < 4 ? w0 : w1, hi = b < 4 ? w1 : w2;
-            const uint32_t v = __funnelshift_r(lo, hi, 8 * (b & 3));
-            reinterpret_cast<uint32_t*>(W + r * wcopy + row * wpitch)[i] = v;
-        }
+    const int sh = (int)((uintptr_t)src & 15);
+    const uint4* srcv = reinterpret_cast<const uint4*>(src - sh);     // aligned vectors covering the row
+    const int64_t nvec = (rowlen + 15) >> 4;                          // output vectors per copy (wcopy >= 16 nvec)
+    const int64_t lastv = (sh + rowlen - 1) >> 4;                     // last aligned vector holding a valid byte
+    uint8_t* dst = W + row * wpitch;
+    switch (sh >> 2) {
+        case 0: shift_row<0>(srcv, dst, wcopy, sh, nvec, lastv); break;
+        case 1: shift_row<1>(srcv, dst, wcopy, sh, nvec, lastv); break;
+        case 2: shift_row<2>(srcv, dst, wcopy, sh, nvec, lastv); break;
+        default: shift_row<3>(srcv, dst, wcopy, sh, nvec, lastv); break;
     }
 }
 
@@ -61,8 +87,8 @@ int make_shift_copies_u8(const dd_plan* p, const ExecArgs& a, uint8_t** W_out, i
     uint8_t* W = nullptr;
     int rc = workspace_alloc((void**)&W, (size_t)(nrows * wpitch), a.stream);
     if (rc != DD_OK) return rc;
-    const int64_t nwords = (rowlen + 3) / 4;
-    dim3 grid((unsigned)nrows, (unsigned)std::min<int64_t>((nwords + 255) / 256, 64));
+    const int64_t nvec = (rowlen + 15) / 16;
+    dim3 grid((unsigned)nrows, (unsigned)std::min<int64_t>((nvec + 255) / 256, 64));
     dd_shift_copies_u8<<<grid, 256, 0, st>>>((const uint8_t*)a.X, W, wcopy, wpitch, p->nchans, rowlen,
                                              a.in_stride, a.in_beam_stride);
     cudaError_t e = cudaGetLastError();
