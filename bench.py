@@ -555,8 +555,8 @@ def next_rows(dd, torch, hbm_peak):
     by = w.nchans * n_in * 8
     rows["f3_rfi"] = {"shape": "config 3 input, %d channels x %d samples float32; order 4, window 512, thresholds 7 / 5" % (w.nchans, n_in),
                       "ms": ms, "algorithmic_bytes": by, "bound": "hbm", "achieved_gbs": by / ms / 1e6, "peak_gbs": peak,
-                      "frac": by / ms / 1e6 / peak, "gpu_launches": 8,
-                      "note": "algorithmic = X read once + written once; the kernels read it three times (window sums, spectrum means, apply)"}
+                      "frac": by / ms / 1e6 / peak, "gpu_launches": 9,
+                      "note": "algorithmic = X read once + written once; the kernels read it twice (window + column sums in one pass, apply) plus the flagged (channel, window) pairs"}
     del X
     # f4: beamformer, BEST-II parameters of PAPER.md:1653 (32 antennas, 1024 channels, 16 beams) over 2^16 samples
     na, nch, nb, nt = 32, 1024, 16, 1 << 16

@@ -76,6 +76,101 @@ dd_rfi_window_sums_kernel(const float* __restrict__ X, int nchans, int64_t n, in
     if (lane == 0) wsum[row * nwin + k] = s;
 }
 
+// 1a (fused form).  A warp takes window k of C consecutive channels: besides the window sums (same lanes, same
+// order as above: identical values) every lane keeps the sums over those C channels of its 16 samples, and the
+// warp leaves them in colpart[beam][channel tile][t] -- the spectrum means of stage 3 then need X only in the few
+// windows where a channel is replaced.  For 16-byte aligned rows and window % 4 == 0, window <= 512.
+// Rows are staged through a per-warp ring of kRing rows in shared memory with cp.async (16 bytes per lane and copy):
+// three rows of every warp are in flight while it works on a fourth -- with plain loads the kernel held one row
+// per warp in flight and ran at 4.7 TB/s (80 registers: 24 warps per SM).
+constexpr int kRing = 4;
+constexpr int kFusedSmem = (kThreads / 32) * kRing * 128 * 16;         // 8 warps x 4 rows x 2 KB
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
+{
+    const uint32_t sa = (uint32_t)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
+__global__ void __launch_bounds__(kThreads)
+dd_rfi_window_col_sums_kernel(const float* __restrict__ X, int nchans, int64_t n, int64_t stride, int64_t beam_stride,
+                              int window, int nwin, int C, int ntiles, int64_t np, double* __restrict__ wsum,
+                              double* __restrict__ colpart)
+{
+    extern __shared__ float4 ring_all[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int k = blockIdx.x * (kThreads / 32) + warp;
+    if (k >= nwin) return;
+    float4* ring = ring_all + warp * (kRing * 128);
+    const unsigned tile = blockIdx.y, ubeam = tile / (unsigned)ntiles, ct = tile - ubeam * (unsigned)ntiles;
+    const int c0 = (int)ct * C;
+    const int64_t a = (int64_t)k * window;
+    const int len = (int)min((int64_t)window, n - a);                 // the last window may be shorter
+    const float* x = X + (int64_t)ubeam * beam_stride + (int64_t)c0 * stride + a;
+    double* ws = wsum + ((int64_t)ubeam * nchans + c0) * nwin + k;
+    double col[4][4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) col[j][e] = 0.0;
+    const int nfull = len >> 2;                                        // whole float4 groups of the window
+    auto issue = [&](int c) {                                          // row c of the tile -> slot c % kRing (own lanes only)
+        if (c < C) {
+            const float* xr = x + (int64_t)c * stride;
+            float4* slot = ring + (c % kRing) * 128;
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (lane + 32 * j < nfull) cp_async16(slot + lane + 32 * j, xr + 4 * (lane + 32 * j));
+        }
+        cp_async_commit();                                             // (an empty group keeps the count uniform)
+    };
+#pragma unroll
+    for (int c = 0; c < kRing - 1; ++c) issue(c);
+#pragma unroll 1
+    for (int c = 0; c < C; ++c, ws += nwin) {
+        issue(c + kRing - 1);
+        cp_async_wait<kRing - 1>();                                    // row c has landed (every lane reads its own copies)
+        const float4* slot = ring + (c % kRing) * 128;
+        const float* xr = x + (int64_t)c * stride;
+        double s = 0.0;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int i = lane + 32 * j;
+            float4 v = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            if (i < nfull) {
+                v = slot[i];
+            } else if (4 * i < len) {                                  // the window's last, partial group
+                v.x = __ldg(xr + 4 * i);
+                if (4 * i + 1 < len) v.y = __ldg(xr + 4 * i + 1);
+                if (4 * i + 2 < len) v.z = __ldg(xr + 4 * i + 2);
+            }
+            const double dx = (double)v.x, dy = (double)v.y, dz = (double)v.z, dw = (double)v.w;
+            if (4 * i < window) s += (dx + dy) + (dz + dw);
+            col[j][0] += dx;
+            col[j][1] += dy;
+            col[j][2] += dz;
+            col[j][3] += dw;
+        }
+        s = warp_sum(s);
+        if (lane == 0) *ws = s;
+    }
+    double* cp = colpart + ((int64_t)ubeam * ntiles + ct) * np + a;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const int i = lane + 32 * j;
+        if (i < nfull) {
+            reinterpret_cast<double2*>(cp + 4 * i)[0] = make_double2(col[j][0], col[j][1]);
+            reinterpret_cast<double2*>(cp + 4 * i)[1] = make_double2(col[j][2], col[j][3]);
+        } else if (4 * i < len) {
+            cp[4 * i] = col[j][0];
+            if (4 * i + 1 < len) cp[4 * i + 1] = col[j][1];
+            if (4 * i + 2 < len) cp[4 * i + 2] = col[j][2];
+        }
+    }
+}
+
 // 1a'. b[row] = mean over time of channel row = (sum of its window sums) / n  (one warp per row, fixed order)
 __global__ void __launch_bounds__(kThreads)
 dd_rfi_bandpass_kernel(const double* __restrict__ wsum, int64_t nrows, int nwin, int64_t n, double* __restrict__ b)
@@ -220,6 +315,32 @@ dd_rfi_flags_kernel(const double* __restrict__ wsum, int64_t nrows, int nchans, 
 constexpr int kSpecT = 128;                   // spectra per block of the spectrum-mean kernel
 constexpr int kSpecQ = kThreads * 4 / kSpecT; // channel slices per block (threads = kSpecT x kSpecQ)
 
+// 2'. (fused form) per beam, window with replaced channels and channel slice of the spectrum kernel: the replaced
+// channels of the slice, ascending, in list[beam][k][c_lo(q) .. c_lo(q) + cnt[beam][k][q])  (one warp per window and
+// slice; ballot compaction)
+__global__ void __launch_bounds__(kThreads)
+dd_rfi_flag_lists_kernel(const uint8_t* __restrict__ flag, const uint8_t* __restrict__ dirty, int nchans, int nwin,
+                         uint16_t* __restrict__ list, int* __restrict__ cnt)
+{
+    const int w = blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5), lane = threadIdx.x & 31, beam = blockIdx.y;
+    const int k = w / kSpecQ, q = w - k * kSpecQ;
+    if (k >= nwin) return;
+    const int cq = nchans / kSpecQ, c_lo = q * cq;                  // (the fused form needs nchans % kSpecQ == 0)
+    int count = 0;
+    if (dirty[(int64_t)beam * nwin + k]) {
+        const uint8_t* fl = flag + (int64_t)beam * nchans * nwin + k;
+        uint16_t* out = list + ((int64_t)beam * nwin + k) * nchans + c_lo;
+        for (int c0 = c_lo; c0 < c_lo + cq; c0 += 32) {
+            const int c = c0 + lane;
+            const bool f = c < c_lo + cq && fl[(int64_t)c * nwin];
+            const unsigned mask = __ballot_sync(0xffffffffu, f);
+            if (f) out[count + __popc(mask & ((1u << lane) - 1u))] = (uint16_t)c;
+            count += __popc(mask);
+        }
+    }
+    if (lane == 0) cnt[((int64_t)beam * nwin + k) * kSpecQ + q] = count;
+}
+
 // 3a. m[beam][t] = mean over channels of the channel-clipped spectrum t.  Block = 128 spectra x 8 channel
 // slices; a thread sums its slice's channels in ascending order (every load a coalesced row segment), the
 // slices' partial sums meet in shared memory and are added in slice order.  Windows in which no channel of the
@@ -230,7 +351,8 @@ __global__ void __launch_bounds__(kSpecT * kSpecQ)
 dd_rfi_spectrum_kernel(const float* __restrict__ X, int nchans, int64_t n, int64_t stride, int64_t beam_stride,
                        int window, int nwin, const double* __restrict__ B, const uint8_t* __restrict__ flag,
                        const uint8_t* __restrict__ dirty, const double* __restrict__ stats, double* __restrict__ m,
-                       double* __restrict__ part)
+                       double* __restrict__ part, const double* __restrict__ colpart, int C, int64_t np,
+                       const uint16_t* __restrict__ list, const int* __restrict__ cnt)
 {
     __shared__ double acc[kSpecQ][kSpecT];
     __shared__ double red[2][kSpecT / 32];
@@ -245,7 +367,19 @@ dd_rfi_spectrum_kernel(const float* __restrict__ X, int nchans, int64_t n, int64
     const int c_lo = min(nchans, q * cq), c_hi = min(nchans, c_lo + cq);
     double s = 0.0;
     int c = c_lo;
-    if (!dirty[(int64_t)beam * nwin + k]) {
+    if (colpart) {
+        // the first pass left the sums over tiles of C channels (slices are whole tiles); in a window where channels
+        // are replaced, each of them contributes B_c instead of its sample: X is read at those (channel, window)
+        // pairs only, taken from the slice's list of the window
+        const double* cp = colpart + ((int64_t)beam * (nchans / C) + c_lo / C) * np + tc;
+        for (int cc = c_lo; cc < c_hi; cc += C, cp += np) s += *cp;
+        const int ne = cnt[((int64_t)beam * nwin + k) * kSpecQ + q];
+        const uint16_t* le = list + ((int64_t)beam * nwin + k) * nchans + c_lo;
+        for (int e = 0; e < ne; ++e) {
+            const int cf = le[e];
+            s += Bb[cf] - (double)__ldg(x + (int64_t)cf * stride);
+        }
+    } else if (!dirty[(int64_t)beam * nwin + k]) {
         for (; c + 8 <= c_hi; c += 8) {
             float v[8];
 #pragma unroll
@@ -446,20 +580,39 @@ int rfi_mitigate(float* X, int nchans, int64_t nsamp, int64_t stride, int64_t be
     // workspace (doubles): b [nrows], B [nrows], stats [nbeams][4], m and excess [nbeams][nsamp], wsum [nrows][nwin];
     // part [nbeams][nspec][2]; (bytes): flag [nrows][nwin], any4 [nbeams][ceil(nsamp / 4)], dirty [nbeams][nwin]
     const int64_t ng4 = (nsamp + 3) / 4;
-    const size_t nd = (size_t)nrows * 2 + (size_t)nbeams * 4 + (size_t)2 * nbeams * nsamp + (size_t)nrows * nwin +
-                      (size_t)2 * nbeams * nspec;
+    // fused first pass (window sums + column sums of tiles of C channels): 16-byte aligned rows, window % 4 == 0 and
+    // <= 512, channel slices of the spectrum kernel made of whole tiles
+    int C = 0;
+    if ((prm->window & 3) == 0 && prm->window <= 512 && (stride & 3) == 0 && (beam_stride & 3) == 0 &&
+        (((uintptr_t)X) & 15) == 0 && nchans % kSpecQ == 0)
+        for (int c : {64, 32, 16, 8})
+            if ((nchans / kSpecQ) % c == 0) {
+                C = c;
+                break;
+            }
+    const int ntiles = C ? nchans / C : 0;
+    const int64_t np = (nsamp + 3) / 4 * 4;                            // pitch of a column-sum row
+    const size_t ncol = (size_t)nbeams * ntiles * np;
+    if ((int64_t)nbeams * ntiles > 65535) C = 0;
+    const size_t nd = (C ? ncol : 0) + (size_t)nrows * 2 + (size_t)nbeams * 4 + (size_t)2 * nbeams * nsamp +
+                      (size_t)nrows * nwin + (size_t)2 * nbeams * nspec;
+    // fused form only: cnt int32 [nbeams][nwin][kSpecQ], list uint16 [nbeams][nwin][nchans]
+    const size_t nlist = C ? (size_t)nbeams * nwin * kSpecQ * sizeof(int) + (size_t)nrows * nwin * sizeof(uint16_t) : 0;
     char* ws = nullptr;
-    int rc = workspace_alloc((void**)&ws, nd * sizeof(double) + (size_t)nrows * nwin + (size_t)nbeams * ng4 +
+    int rc = workspace_alloc((void**)&ws, nd * sizeof(double) + nlist + (size_t)nrows * nwin + (size_t)nbeams * ng4 +
                                               (size_t)nbeams * nwin, cuda_stream);
     if (rc != DD_OK) return rc;
-    double* b = (double*)ws;
+    double* colpart = C ? (double*)ws : nullptr;
+    double* b = (double*)ws + (C ? ncol : 0);
     double* B = b + nrows;
     double* stats = B + nrows;
     double* m = stats + (size_t)nbeams * 4;
     double* excess = m + (size_t)nbeams * nsamp;
     double* wsum = excess + (size_t)nbeams * nsamp;
     double* part = wsum + (size_t)nrows * nwin;
-    uint8_t* flag = (uint8_t*)(part + (size_t)2 * nbeams * nspec);
+    int* cnt = (int*)(part + (size_t)2 * nbeams * nspec);
+    uint16_t* list = (uint16_t*)(cnt + (C ? (size_t)nbeams * nwin * kSpecQ : 0));
+    uint8_t* flag = (uint8_t*)cnt + nlist;
     uint8_t* any4 = flag + (size_t)nrows * nwin;
     uint8_t* dirty = any4 + (size_t)nbeams * ng4;
     if (cudaMemsetAsync(dirty, 0, (size_t)nbeams * nwin, st) != cudaSuccess) {
@@ -467,14 +620,26 @@ int rfi_mitigate(float* X, int nchans, int64_t nsamp, int64_t stride, int64_t be
         return fail(DD_ERR_CUDA, "RFI mitigation: clearing the workspace failed");
     }
     constexpr int kWPB = kThreads / 32;                    // warps per block
-    dd_rfi_window_sums_kernel<<<dim3((unsigned)((nwin + kWPB - 1) / kWPB), (unsigned)nrows), kThreads, 0, st>>>(
-        X, nchans, nsamp, stride, beam_stride, prm->window, nwin, wsum);
+    if (C && ensure_dyn_smem((const void*)dd_rfi_window_col_sums_kernel, kFusedSmem) != DD_OK) {
+        cudaFreeAsync(ws, st);
+        return DD_ERR_CUDA;
+    }
+    if (C)
+        dd_rfi_window_col_sums_kernel<<<dim3((unsigned)((nwin + kWPB - 1) / kWPB), (unsigned)(nbeams * ntiles)), kThreads,
+                                        kFusedSmem, st>>>(X, nchans, nsamp, stride, beam_stride, prm->window, nwin, C, ntiles, np, wsum,
+                                              colpart);
+    else
+        dd_rfi_window_sums_kernel<<<dim3((unsigned)((nwin + kWPB - 1) / kWPB), (unsigned)nrows), kThreads, 0, st>>>(
+            X, nchans, nsamp, stride, beam_stride, prm->window, nwin, wsum);
     dd_rfi_bandpass_kernel<<<(unsigned)((nrows + kWPB - 1) / kWPB), kThreads, 0, st>>>(wsum, nrows, nwin, nsamp, b);
     dd_rfi_fit_kernel<<<(unsigned)nbeams, kThreads, 0, st>>>(b, nchans, prm->poly_order, B, stats);
     dd_rfi_flags_kernel<<<(unsigned)std::min<int64_t>((nrows * nwin + kThreads - 1) / kThreads, 4096), kThreads, 0, st>>>(
         wsum, nrows, nchans, nwin, prm->window, nsamp, B, stats, (double)prm->t_chan, flag, chan_flags, dirty);
+    if (C)
+        dd_rfi_flag_lists_kernel<<<dim3((unsigned)(((int64_t)nwin * kSpecQ + kWPB - 1) / kWPB), (unsigned)nbeams), kThreads, 0, st>>>(
+            flag, dirty, nchans, nwin, list, cnt);
     dd_rfi_spectrum_kernel<<<dim3((unsigned)nspec, (unsigned)nbeams), dim3(kSpecT, kSpecQ), 0, st>>>(
-        X, nchans, nsamp, stride, beam_stride, prm->window, nwin, B, flag, dirty, stats, m, part);
+        X, nchans, nsamp, stride, beam_stride, prm->window, nwin, B, flag, dirty, stats, m, part, colpart, C, np, list, cnt);
     dd_rfi_spectrum_stats_kernel<<<(unsigned)nbeams, kThreads, 0, st>>>(part, (int)nspec, nsamp, stats);
     dd_rfi_excess_kernel<<<dim3((unsigned)((ng4 + kThreads - 1) / kThreads), (unsigned)nbeams), kThreads, 0, st>>>(
         m, nsamp, stats, (double)prm->t_spec, excess, any4, spec_flags);

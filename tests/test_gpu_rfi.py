@@ -98,6 +98,23 @@ def test_against_the_oracle(nch, n, order, window):
         assert want["chan_flags"].any() and want["spec_flags"].any()   # the case exercises both stages
 
 
+@pytest.mark.parametrize("nch,n,order,window", [(64, 4099, 3, 256), (128, 6001, 4, 512), (256, 5000, 2, 100),
+                                                 (512, 9002, 8, 64), (1024, 3003, 4, 12), (64, 300, 1, 512)])
+def test_against_the_oracle_on_aligned_rows(nch, n, order, window):
+    """16-byte aligned rows, window % 4 == 0: the first pass is the fused one (window sums + column sums of tiles of
+    8 / 16 / 32 / 64 channels), the spectrum means come from the column sums except in windows with replaced
+    channels; ragged lengths, a last window shorter than the rest, a window longer than the series."""
+    X = noisy(nch * 5 + n, nch, n)
+    got = run([X], order, window, 5.0, 4.0, pad=(-n) % 4)[0]
+    want = compare(X, got, order, window, 5.0, 4.0)
+    if n >= 4096 and order >= 3:
+        assert want["chan_flags"].any() and want["spec_flags"].any()
+    # several beams, padded aligned strides
+    Xs = [noisy(nch + n + b, nch, n) for b in range(2)]
+    for Xb, gb in zip(Xs, run(Xs, order, window, 5.0, 4.0, pad=(-n) % 4 + 8, beam_pad=12)):
+        compare(Xb, gb, order, window, 5.0, 4.0)
+
+
 def test_beams_and_strides():
     Xs = [noisy(100 + b, 48, 3000) for b in range(3)]
     res = run(Xs, 3, 128, 5.0, 4.0, pad=5, beam_pad=11)
