@@ -12,10 +12,13 @@
 // with a write pass each.  Here everything stays on the device (the fit is one block solving the
 // normal equations in a Legendre basis in double precision) and the replacements are never written as
 // such: the window flags and the spectrum excesses are small side arrays, applied when the single
-// output pass subtracts the bandpass.  Passes over X: two reads (window sums -- from which both the
-// averaged bandpass and the window means follow -- and the spectrum means of the clipped data) and one
-// read + write -- all HBM-bound streaming kernels.  All means, the fit and the threshold comparisons are
-// evaluated in double precision; the output is rounded once, from double, to float32.
+// output pass subtracts the bandpass.  Passes over X, plain form: two reads (window sums -- from which both
+// the averaged bandpass and the window means follow -- and the spectrum means of the clipped data) and one
+// read + write.  Fused form (16-byte aligned rows, window a multiple of 4 and <= 512): the first pass also
+// leaves the column sums of tiles of 8-64 channels, the spectrum means come from those and from X at the
+// replaced (channel, window) pairs only: one read and one read + write -- all HBM-bound streaming kernels.
+// All means, the fit and the threshold comparisons are evaluated in double precision; the output is rounded
+// once, from double, to float32.
 #include <cuda_runtime.h>
 
 #include <algorithm>
