@@ -537,7 +537,7 @@ def next_rows(dd, torch, hbm_peak):
     rows["f1_postprocess"] = {"shape": "config 3 output, %d series x %d samples float32; median 5, detrend, normalise, 6 sigma -> candidates" % (w.ndm, w.nsamp),
                               "ms": ms, "algorithmic_bytes": by, "bound": "hbm", "achieved_gbs": by / ms / 1e6,
                               "peak_gbs": peak, "frac": by / ms / 1e6 / peak, "gpu_launches": dd.dd_postprocess_launches(prm, False),
-                              "note": "algorithmic = D read once; the kernels read it twice (regression statistics, apply)"}
+                              "note": "algorithmic = D read once; read once by the statistics pass (which leaves chunk maxima), then only the chunks that can hold a candidate"}
     del D
     # f3: RFI mitigation of config 3's input buffer, in place
     n_in = w.nsamp + 14845

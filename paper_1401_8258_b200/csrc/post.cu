@@ -17,8 +17,10 @@
 // exactly).  dd_post_apply_kernel: grid over (time tiles, series); every thread forms four
 // consecutive medians from 4 + (w - 1) loaded samples, subtracts the line, scales, optionally stores
 // the processed series (16-byte stores) and appends the samples above the threshold to the
-// candidate list through an atomic cursor.  HBM traffic: D is read twice and written at most once,
-// against seven passes for the step-by-step pipeline of §3.5; the kernels are HBM-bound.
+// candidate list through an atomic cursor.  Candidates-only calls: the statistics pass also leaves the largest
+// median of every 128-sample chunk and dd_post_scan_kernel reads D only in chunks that can hold a detection.
+// HBM traffic: D is read once (candidates only) or twice and written at most once, against seven passes for
+// the step-by-step pipeline of §3.5; the kernels are HBM-bound.
 // The thesis used one kernel per step with the series staged in shared memory.
 #include <cuda_runtime.h>
 
@@ -163,6 +165,25 @@ __device__ __forceinline__ void medians4(const T* __restrict__ row, unsigned t0,
 
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
+// chunk maxima are kept as signed integer keys: the value itself for int32 series, the order-preserving map of the
+// bit pattern for float32 series (its own inverse), so that the warp maximum is one REDUX
+__device__ __forceinline__ int32_t max_key(int32_t v) { return v; }
+__device__ __forceinline__ int32_t max_key(float v)
+{
+    const int32_t b = __float_as_int(v);
+    return b ^ ((b >> 31) & 0x7fffffff);
+}
+template <typename T> __device__ __forceinline__ float key_to_float_up(int32_t k)      // never below the value
+{
+    if constexpr (std::is_integral<T>::value) return __int2float_ru(k);
+    else return __int_as_float(k ^ ((k >> 31) & 0x7fffffff));
+}
+template <typename T> __device__ __forceinline__ T lowest_of();
+template <> __device__ __forceinline__ float lowest_of<float>() { return -INFINITY; }
+template <> __device__ __forceinline__ int32_t lowest_of<int32_t>() { return INT32_MIN; }
+
+constexpr int kChunk = 32 * kPer;             // samples of one warp step: the granularity of the chunk maxima
+
 __device__ __forceinline__ double block_sum(double v, double* red)
 {
 #pragma unroll
@@ -182,10 +203,10 @@ __device__ __forceinline__ double block_sum(double v, double* red)
 // with u_t = y_t - y_0 (the offset removes the level, so a constant series gives exact zeros) and
 // tc = t - (n-1)/2,  slope = sum tc u / sum tc^2,  mean = y_0 + sum u / n,
 // SS_res = sum u^2 - (sum u)^2 / n - slope^2 sum tc^2  (the normal equations' residual), all in double.
-template <typename T, int W>
+template <typename T, int W, bool CM>
 __global__ void __launch_bounds__(kThreads)
 dd_post_stats_kernel(const T* __restrict__ D, int64_t stride, int64_t beam_stride, int ndm, int64_t n,
-                     double* __restrict__ stats)
+                     double* __restrict__ stats, int32_t* __restrict__ cmax)
 {
     __shared__ double red[kThreads / 32];
     const int64_t r = blockIdx.x;
@@ -197,12 +218,30 @@ dd_post_stats_kernel(const T* __restrict__ D, int64_t stride, int64_t beam_strid
     const double y0 = (double)first[0];
     double su = 0.0, stu = 0.0, suu = 0.0;
     double tc0 = (double)(threadIdx.x * kPer) - tm;       // t0 - tm as a running double (exact: multiples of 1/2)
-    for (unsigned t0 = threadIdx.x * kPer; t0 < n32; t0 += kTile, tc0 += (double)kTile) {
+    // cmax (optional): the largest median of every chunk of 128 samples (one warp step), which lets a
+    // candidates-only second pass skip the chunks that cannot hold a detection.  The trip count is uniform over
+    // a warp (warp-wide maximum); threads past the end form clamped medians that are not used.
+    const unsigned lane4 = (threadIdx.x & 31) * kPer;
+    int32_t* cmrow = CM ? cmax + r * (int64_t)((n32 + kChunk - 1) / kChunk) : nullptr;
+    for (unsigned t0 = threadIdx.x * kPer; t0 - (CM ? lane4 : 0u) < n32; t0 += kTile, tc0 += (double)kTile) {
         // one load group per thread and trip leaves too few bytes in flight (3 blocks x 512 threads x 16 bytes
         // per SM): ask L2 for the trip after next (no register cost; 1.01 -> 0.79 ms on config 3's plane)
         if (t0 + 2 * kTile < n32) prefetch_l2(row + t0 + 2 * kTile);
         T m[kPer];
         medians4<T, W>(row, t0, n32, m);
+        if constexpr (CM) {
+            T top;
+            if (t0 + kPer <= n32) {
+                top = mx(mx(m[0], m[1]), mx(m[2], m[3]));
+            } else {
+                top = lowest_of<T>();
+#pragma unroll
+                for (int e = 0; e < kPer; ++e)
+                    if (t0 + e < n32) top = mx(top, m[e]);
+            }
+            const int32_t key = __reduce_max_sync(0xffffffffu, max_key(top));
+            if (lane4 == 0) cmrow[t0 / kChunk] = key;
+        }
         double u[kPer];
 #pragma unroll
         for (int e = 0; e < kPer; ++e) u[e] = (double)m[e] - y0;
@@ -250,6 +289,7 @@ struct ApplyParams {
     int detrend, normalise, threshold_on;
     double nsigma;
     const double* stats;
+    int32_t* cmax;                                         // chunk maxima (keys) of the statistics pass, or null
     float* Z;
     int64_t z_stride, z_beam_stride;
     dd_candidate* cand;
@@ -283,13 +323,13 @@ dd_post_apply_kernel(const T* __restrict__ D, const ApplyParams p)
     // candidates are exactly those of the unscreened evaluation.
     const bool screen = !zrow && p.threshold_on && sigma > 0.0 && p.nsigma >= 0.0;
     float scr_a = 0.0f, scr_b = 0.0f;
+    const unsigned n32 = (unsigned)p.n;
     if (screen) {
         const double level = p.nsigma * sigma;
         const double margin = 0x1p-21 * (fabs(slope) * (double)p.n + fabs(intercept) + level);
         scr_a = __double2float_rd(intercept + level - margin);
         scr_b = (float)slope;
     }
-    const unsigned n32 = (unsigned)p.n;
     const unsigned tile0 = (blockIdx.x - r * p.ntiles) * p.steps;
     {   // as in the statistics kernel: ask L2 for the next two steps, then for the step after next in every step
         const unsigned tp = (tile0 * kThreads + threadIdx.x) * kPer;
@@ -349,13 +389,77 @@ dd_post_apply_kernel(const T* __restrict__ D, const ApplyParams p)
     }
 }
 
+// Candidates-only second pass when the statistics pass has left the chunk maxima: a lane tests one chunk of 128
+// samples -- its largest median against lo at both ends of the chunk (L(t) = line(t) + n sigma * sigma is linear, so
+// its minimum over the chunk is at an end, and lo < L there: see the screen of the apply kernel) -- and the warp then
+// takes the chunks that can hold a detection one by one (medians again, double-precision decision for every
+// sample).  D is read only where candidates are: 4 bytes of keys per 512 bytes of D otherwise.
+template <typename T, int W>
+__global__ void __launch_bounds__(kThreads)
+dd_post_scan_kernel(const T* __restrict__ D, const ApplyParams p, unsigned blocks_per_row)
+{
+    const unsigned r = blockIdx.x / blocks_per_row;
+    const int beam = (int)(r / (unsigned)p.ndm), dm = (int)(r - (unsigned)beam * (unsigned)p.ndm);
+    const T* row = D + (int64_t)beam * p.beam_stride + (int64_t)dm * p.stride;
+    const double intercept = p.stats[(int64_t)r * 3 + 0], slope = p.stats[(int64_t)r * 3 + 1];
+    const double sigma = p.stats[(int64_t)r * 3 + 2];
+    if (!(sigma > 0.0)) return;                            // sigma = 0: all-zero series, nothing above n sigma >= 0
+    const double inv = 1.0 / sigma;
+    const double level = p.nsigma * sigma;
+    const double margin = 0x1p-21 * (fabs(slope) * (double)p.n + fabs(intercept) + level);
+    const float scr_a = __double2float_rd(intercept + level - margin), scr_b = (float)slope;
+    const unsigned n32 = (unsigned)p.n, nchunk = (n32 + kChunk - 1) / kChunk;
+    const int32_t* cmrow = p.cmax + (int64_t)r * nchunk;
+    const unsigned lane = threadIdx.x & 31;
+    const unsigned c = ((blockIdx.x - r * blocks_per_row) * (kThreads / 32) + (threadIdx.x >> 5)) * 32 + lane;
+    bool hot = false;
+    if (c < nchunk) {
+        const float tf = (float)(c * kChunk);
+        const float lo = fminf(fmaf(scr_b, tf, scr_a), fmaf(scr_b, tf + (float)(kChunk - 1), scr_a));
+        hot = key_to_float_up<T>(cmrow[c]) > lo;
+    }
+    unsigned todo = __ballot_sync(0xffffffffu, hot);
+    while (todo) {
+        const unsigned ch = c - lane + (unsigned)(__ffs(todo) - 1);
+        todo &= todo - 1;
+        const unsigned t0 = ch * kChunk + lane * kPer;
+        if (t0 >= n32) continue;
+        T m[kPer];
+        medians4<T, W>(row, t0, n32, m);
+        const double td0 = (double)t0;
+#pragma unroll
+        for (int e = 0; e < kPer; ++e) {
+            const double v = (double)m[e] - (intercept + slope * (td0 + (double)e));
+            const double snr = v * inv;
+            if (t0 + e < n32 && snr > p.nsigma) {
+                const unsigned long long at = atomicAdd(p.count, 1ull);
+                if ((int64_t)at < p.capacity) {
+                    dd_candidate cd;
+                    cd.beam = beam;
+                    cd.dm = dm;
+                    cd.t = (int32_t)(t0 + e);
+                    cd.value = (float)snr;
+                    p.cand[at] = cd;
+                }
+            }
+        }
+    }
+}
+
 template <typename T, int W>
 int launch_w(const void* D, int64_t nrows, const ApplyParams& ap, double* stats, cudaStream_t st)
 {
-    if (ap.detrend)
-        dd_post_stats_kernel<T, W><<<(unsigned)nrows, kThreads, 0, st>>>((const T*)D, ap.stride, ap.beam_stride, ap.ndm,
-                                                                          ap.n, stats);
-    if (ap.Z || ap.threshold_on) {
+    if (ap.detrend && ap.cmax)
+        dd_post_stats_kernel<T, W, true><<<(unsigned)nrows, kThreads, 0, st>>>(
+            (const T*)D, ap.stride, ap.beam_stride, ap.ndm, ap.n, stats, ap.cmax);
+    else if (ap.detrend)
+        dd_post_stats_kernel<T, W, false><<<(unsigned)nrows, kThreads, 0, st>>>(
+            (const T*)D, ap.stride, ap.beam_stride, ap.ndm, ap.n, stats, nullptr);
+    if (ap.cmax) {                                         // candidates only, chunk maxima at hand
+        const int64_t nchunk = (ap.n + kChunk - 1) / kChunk, per_block = (kThreads / 32) * 32;
+        const unsigned bpr = (unsigned)((nchunk + per_block - 1) / per_block);
+        dd_post_scan_kernel<T, W><<<(unsigned)(nrows * bpr), kThreads, 0, st>>>((const T*)D, ap, bpr);
+    } else if (ap.Z || ap.threshold_on) {
         dd_post_apply_kernel<T, W><<<(unsigned)(nrows * ap.ntiles), kThreads, 0, st>>>((const T*)D, ap);
     }
     cudaError_t e = cudaGetLastError();
@@ -383,9 +487,10 @@ int post_launches(const dd_post_params* prm, bool want_series)
     return (prm->detrend ? 1 : 0) + ((want_series || prm->threshold_on) ? 1 : 0);
 }
 
-int postprocess(int dtype, const void* D, int64_t stride, int64_t beam_stride, int ndm, int64_t nsamp, int nbeams,
-                const dd_post_params* prm, float* Z, int64_t z_stride, int64_t z_beam_stride, double* stats,
-                dd_candidate* cand, int64_t capacity, unsigned long long* count, void* cuda_stream)
+static int postprocess_impl(int dtype, const void* D, int64_t stride, int64_t beam_stride, int ndm, int64_t nsamp,
+                            int nbeams, const dd_post_params* prm, float* Z, int64_t z_stride, int64_t z_beam_stride,
+                            double* stats, dd_candidate* cand, int64_t capacity, unsigned long long* count,
+                            void* cuda_stream, bool may_allocate)
 {
     if (!prm) return fail(DD_ERR_BAD_ARG, "params is null");
     if (dtype != DD_F32 && dtype != DD_U8) return fail(DD_ERR_BAD_ARG, "dtype must be DD_F32 or DD_U8");
@@ -421,13 +526,32 @@ int postprocess(int dtype, const void* D, int64_t stride, int64_t beam_stride, i
         if (rc != DD_OK) return rc;
         stats = own_stats;
     }
+    // candidates-only calls: the statistics pass leaves the largest median of every 128-sample chunk (4 bytes per
+    // 512 of D), and the second pass reads D only in chunks that can hold a detection
+    int32_t* cmax = nullptr;
+    if (may_allocate && prm->detrend && prm->threshold_on && !Z && prm->nsigma >= 0.0f) {
+        int rc = workspace_alloc((void**)&cmax, (size_t)nrows * (size_t)((nsamp + kChunk - 1) / kChunk) * 4, cuda_stream);
+        if (rc != DD_OK) {
+            if (own_stats) cudaFreeAsync(own_stats, st);
+            return rc;
+        }
+    }
     ApplyParams ap{stride, nbeams > 1 ? beam_stride : 0, nsamp, ndm, (unsigned)ntiles, (unsigned)steps, prm->detrend, prm->normalise,
-                   prm->threshold_on, (double)prm->nsigma, stats, Z, z_stride, nbeams > 1 ? z_beam_stride : 0,
+                   prm->threshold_on, (double)prm->nsigma, stats, cmax, Z, z_stride, nbeams > 1 ? z_beam_stride : 0,
                    cand, capacity, count};
     const int rc = dtype == DD_F32 ? launch_t<float>(w, D, nrows, ap, stats, st)
                                    : launch_t<int32_t>(w, D, nrows, ap, stats, st);
     if (own_stats) cudaFreeAsync(own_stats, st);
+    if (cmax) cudaFreeAsync(cmax, st);
     return rc;
+}
+
+int postprocess(int dtype, const void* D, int64_t stride, int64_t beam_stride, int ndm, int64_t nsamp, int nbeams,
+                const dd_post_params* prm, float* Z, int64_t z_stride, int64_t z_beam_stride, double* stats,
+                dd_candidate* cand, int64_t capacity, unsigned long long* count, void* cuda_stream)
+{
+    return postprocess_impl(dtype, D, stride, beam_stride, ndm, nsamp, nbeams, prm, Z, z_stride, z_beam_stride, stats,
+                            cand, capacity, count, cuda_stream, true);
 }
 
 // ---- the entry point that allocates nothing (dd_postprocess_static) --------------------------------
@@ -485,9 +609,10 @@ int postprocess_static(int dtype, const void* D, int64_t stride, int64_t beam_st
     double* stats = nullptr;
     const int rc = static_stats_address(&stats);
     if (rc != DD_OK) return rc;
-    // with a statistics table passed in, postprocess() allocates and frees nothing
-    return postprocess(dtype, D, stride, beam_stride, ndm, nsamp, nbeams, prm, Z, z_stride, z_beam_stride, stats,
-                       cand, capacity, count, cuda_stream);
+    // with a statistics table passed in and the chunk-maximum workspace of candidates-only calls forgone (the second
+    // pass then reads all of D, same candidates), nothing is allocated or freed
+    return postprocess_impl(dtype, D, stride, beam_stride, ndm, nsamp, nbeams, prm, Z, z_stride, z_beam_stride, stats,
+                            cand, capacity, count, cuda_stream, false);
 }
 
 }  // namespace dd
