@@ -222,7 +222,7 @@ dd_post_stats_kernel(const T* __restrict__ D, int64_t stride, int64_t beam_strid
     // candidates-only second pass skip the chunks that cannot hold a detection.  The trip count is uniform over
     // a warp (warp-wide maximum); threads past the end form clamped medians that are not used.
     const unsigned lane4 = (threadIdx.x & 31) * kPer;
-    int32_t* cmrow = CM ? cmax + r * (int64_t)((n32 + kChunk - 1) / kChunk) : nullptr;
+    int32_t* cmp = CM ? cmax + r * (int64_t)((n32 + kChunk - 1) / kChunk) + (threadIdx.x >> 5) : nullptr;   // this warp's first chunk
     for (unsigned t0 = threadIdx.x * kPer; t0 - (CM ? lane4 : 0u) < n32; t0 += kTile, tc0 += (double)kTile) {
         // one load group per thread and trip leaves too few bytes in flight (3 blocks x 512 threads x 16 bytes
         // per SM): ask L2 for the trip after next (no register cost; 1.01 -> 0.79 ms on config 3's plane)
@@ -240,7 +240,8 @@ dd_post_stats_kernel(const T* __restrict__ D, int64_t stride, int64_t beam_strid
                     if (t0 + e < n32) top = mx(top, m[e]);
             }
             const int32_t key = __reduce_max_sync(0xffffffffu, max_key(top));
-            if (lane4 == 0) cmrow[t0 / kChunk] = key;
+            if (lane4 == 0) *cmp = key;
+            cmp += kTile / kChunk;
         }
         double u[kPer];
 #pragma unroll
