@@ -101,12 +101,13 @@ template <typename T, int W> __device__ __forceinline__ T median_of(T (&v)[W])
 // [0, n-1] (R15).  Samples past the end give the clamped windows' medians (never used).
 // n < 2^31 (checked by the caller): 32-bit sample indices.
 template <typename T, int W>
-__device__ __forceinline__ void medians4(const T* __restrict__ row, unsigned t0, unsigned n, T (&m)[kPer])
+__device__ __forceinline__ void medians4(const T* __restrict__ row, unsigned t0, unsigned n, T (&m)[kPer],
+                                         bool row_aligned)   // row is 16-byte aligned (t0 is a multiple of 4)
 {
     constexpr int H = (W - 1) / 2;
     T x[kPer + 2 * H];
     static_assert(sizeof(T) == 4 && kPer == 4 && H <= 4, "the aligned path loads three 16-byte vectors");
-    if (t0 >= 4 && t0 + 8 <= n && ((uintptr_t)(row + t0) & 15) == 0) {
+    if (row_aligned && t0 >= 4 && t0 + 8 <= n) {
         // interior, 16-byte aligned: the thread's four samples and the aligned vectors on either side
         // (the neighbours' own samples: L1 hits) instead of 4 + 2 H scalar loads
         const int4* src = reinterpret_cast<const int4*>(row + t0);
@@ -214,7 +215,8 @@ dd_post_stats_kernel(const T* __restrict__ D, int64_t stride, int64_t beam_strid
     const double tm = 0.5 * (double)(n - 1);
     const unsigned n32 = (unsigned)n;
     T first[kPer];
-    medians4<T, W>(row, 0u, n32, first);
+    const bool row_aligned = ((uintptr_t)row & 15) == 0;
+    medians4<T, W>(row, 0u, n32, first, row_aligned);
     const double y0 = (double)first[0];
     double su = 0.0, stu = 0.0, suu = 0.0;
     double tc0 = (double)(threadIdx.x * kPer) - tm;       // t0 - tm as a running double (exact: multiples of 1/2)
@@ -228,7 +230,7 @@ dd_post_stats_kernel(const T* __restrict__ D, int64_t stride, int64_t beam_strid
         // per SM): ask L2 for the trip after next (no register cost; 1.01 -> 0.79 ms on config 3's plane)
         if (t0 + 2 * kTile < n32) prefetch_l2(row + t0 + 2 * kTile);
         T m[kPer];
-        medians4<T, W>(row, t0, n32, m);
+        medians4<T, W>(row, t0, n32, m, row_aligned);
         if constexpr (CM) {
             T top;
             if (t0 + kPer <= n32) {
@@ -342,7 +344,7 @@ dd_post_apply_kernel(const T* __restrict__ D, const ApplyParams p)
         if (t0 >= n32) return;
         if (j + 2 < p.steps && t0 + 2 * kTile < n32) prefetch_l2(row + t0 + 2 * kTile);
         T m[kPer];
-        medians4<T, W>(row, t0, n32, m);
+        medians4<T, W>(row, t0, n32, m, ((uintptr_t)(row + t0) & 15) == 0);
         if (screen) {
             const float tf = (float)t0;
             bool any = false;
@@ -405,6 +407,7 @@ dd_post_scan_kernel(const T* __restrict__ D, const ApplyParams p, unsigned block
     const double intercept = p.stats[(int64_t)r * 3 + 0], slope = p.stats[(int64_t)r * 3 + 1];
     const double sigma = p.stats[(int64_t)r * 3 + 2];
     if (!(sigma > 0.0)) return;                            // sigma = 0: all-zero series, nothing above n sigma >= 0
+    const bool row_aligned = ((uintptr_t)row & 15) == 0;
     const double inv = 1.0 / sigma;
     const double level = p.nsigma * sigma;
     const double margin = 0x1p-21 * (fabs(slope) * (double)p.n + fabs(intercept) + level);
@@ -426,7 +429,7 @@ dd_post_scan_kernel(const T* __restrict__ D, const ApplyParams p, unsigned block
         const unsigned t0 = ch * kChunk + lane * kPer;
         if (t0 >= n32) continue;
         T m[kPer];
-        medians4<T, W>(row, t0, n32, m);
+        medians4<T, W>(row, t0, n32, m, row_aligned);
         const double td0 = (double)t0;
 #pragma unroll
         for (int e = 0; e < kPer; ++e) {
