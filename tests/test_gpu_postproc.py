@@ -218,6 +218,33 @@ def test_threshold_only_calls_list_exactly_the_candidates_of_calls_with_series_o
     assert checked > 100000
 
 
+@pytest.mark.parametrize("n", [1, 127, 128, 129, 2048 + 1, 3 * 2048 + 127, 70001])
+def test_candidates_only_calls_find_detections_at_chunk_edges(n):
+    """Candidates-only calls skip every 128-sample chunk whose largest median cannot pass (chunk maxima left by the
+    statistics pass): single-sample detections at the first and last sample of chunks, of block steps and of the
+    series (whose last chunk is partial) must all be listed, and nothing else."""
+    g = np.random.default_rng(n)
+    nb, ndm = 2, 3
+    D = (100.0 + 0.25 * g.standard_normal((nb, ndm, n))).astype(np.float32)
+    spots = sorted({t for t in (0, 1, 126, 127, 128, 129, 255, 256, 2047, 2048, 2049, 4095, 4096, n - 129, n - 128,
+                                n - 2, n - 1) if 0 <= t < n})
+    want = set()
+    for b in range(nb):
+        for d in range(ndm):
+            for t in spots[(b + d) % 2::2]:                           # a different subset per series
+                D[b, d, t] += 30.0 if n > 40 else 3.0
+                want.add((b, d, t))
+    # (the detections themselves inflate sigma of a short series: 30 / sigma is 5.6 at n = 127, 18 at n = 2049)
+    prm = dd.post_params(0, True, True, nsigma=8.0 if n > 2000 else (4.0 if n > 40 else 1.2))
+    _, _, c0, n0 = run_post(D, prm, want_series=True, capacity=1 << 12)
+    _, _, c1, n1 = run_post(D, prm, want_series=False, capacity=1 << 12, stats=False)
+    k0 = sorted(zip(c0["beam"].tolist(), c0["dm"].tolist(), c0["t"].tolist(), c0["value"].tolist()))
+    k1 = sorted(zip(c1["beam"].tolist(), c1["dm"].tolist(), c1["t"].tolist(), c1["value"].tolist()))
+    assert n0 == n1 and k0 == k1
+    if n > 40:
+        assert {(b, d, t) for b, d, t, _ in k1} == want
+
+
 # ------------------------------------------------------------------ the chain: dedisperse -> post-process -> candidates
 
 @pytest.mark.parametrize("idx,nchans,ndm,nsamp,w", [(3, 512, 50, 8192 + 100, 0), (2, 256, 70, 9000, 3), (4, 128, 40, 6000, 5)])
