@@ -115,6 +115,19 @@ def test_against_the_oracle_on_aligned_rows(nch, n, order, window):
         compare(Xb, gb, order, window, 5.0, 4.0)
 
 
+def test_aligned_rows_with_every_channel_replaced_in_some_windows():
+    """Fused first pass, worst case for the per-window lists of replaced channels: a broadband burst that lasts two
+    whole windows replaces ALL channels there (and in the neighbouring windows); a narrowband interferer keeps every
+    window of the buffer in the list path."""
+    nch, n, window = 256, 8192 + 40, 256
+    X = noisy(77, nch, n)
+    X[:, 3 * window: 5 * window] += 6.0
+    X[10, :] += 5.0
+    got = run([X], 3, window, 5.0, 4.0, pad=(-n) % 4)[0]
+    want = compare(X, got, 3, window, 5.0, 4.0)
+    assert want["chan_flags"][:, 2:6].all() and want["chan_flags"][10].all()
+
+
 def test_beams_and_strides():
     Xs = [noisy(100 + b, 48, 3000) for b in range(3)]
     res = run(Xs, 3, 128, 5.0, 4.0, pad=5, beam_pad=11)
